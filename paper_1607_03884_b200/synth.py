@@ -139,6 +139,18 @@ def _anticorrelated_uniforms(rng, rho: float = -0.9):
 
 
 def make_mechanism(kind: str = "h2co", seed: int = 0) -> dict:
+    """Seeded synthetic mechanism; a draw whose species set has too few balanced reactions is
+    redrawn with the next sub-seed (deterministic)."""
+    err = None
+    for attempt in range(64):
+        try:
+            return _make_mechanism(kind, seed, attempt)
+        except RuntimeError as e:       # structural rejection only
+            err = e
+    raise RuntimeError(f"no acceptable mechanism for seed {seed}: {err}")
+
+
+def _make_mechanism(kind: str, seed: int, attempt: int) -> dict:
     """Build the seeded synthetic mechanism `kind` ("h2co": 13 sp / 27 rxn, "gri": 53 / 325).
 
     All reactions are reversible and element-balanced by construction; reverse rates come
@@ -146,7 +158,7 @@ def make_mechanism(kind: str = "h2co", seed: int = 0) -> dict:
     direction at T_REF (so that reverse rate constants stay below the forward scale)."""
     spec = KINDS[kind]
     elements = spec["elements"]
-    rng = np.random.default_rng([seed, sum(map(ord, kind))])
+    rng = np.random.default_rng([seed, sum(map(ord, kind)), attempt])
     ne = len(elements)
 
     comps = _species_set(rng, spec)
