@@ -1,0 +1,156 @@
+/*
+ * chem.h -- C ABI of the B200-native batched stiff-kinetics integrator
+ * (hot path of arXiv 1607.03884, Curtis/Niemeyer/Sung: "An investigation of
+ * GPU-based stiff chemical kinetics integration methods").
+ *
+ * PAPER.md = /root/reference/PAPER.md (text of the paper).  The operations:
+ *   - the problem: many independent constant-pressure reactor IVPs, one per
+ *     thermochemical state (T, Y_1..Y_{N-1}), advanced over ONE global time
+ *     step; PAPER.md L47-L49 (Sec. 1), L134 (Sec. 3).
+ *   - source term and analytical constant-pressure mass-fraction Jacobian
+ *     (pyJac): PAPER.md L82 (Sec. 2.1), footnote L186.
+ *   - 3-stage / 5th-order implicit Radau IIA with built-in adaptive stepping,
+ *     Jacobian reuse "according to the built-in rules", rtol = 1e-6,
+ *     atol = 1e-10: PAPER.md L86 (Sec. 2.1).
+ *   - LU factorisation of the Jacobian-based matrices on the device:
+ *     PAPER.md L86.
+ *   - per-IVP internal step counts d_i (divergence measure, Eq. 3): L190.
+ * DESIGN.md lists every reading (R1..R12) where the paper is silent.
+ *
+ * Conventions
+ *   - units: cm, mol, s, K, g/mol, dyn/cm^2 (1 atm = 1.01325e6), Ea in cal/mol.
+ *   - all functions return 0 on success or a negative CHEM_E_* code;
+ *     chem_last_error() gives a thread-local message for the last failure.
+ *   - "device" pointers are CUDA global-memory pointers on the current device;
+ *     "host" pointers are ordinary host memory.  Nothing is retained after a
+ *     call returns except inside the opaque chem_mech.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *     Calls taking a stream are asynchronous with respect to the host.
+ *   - there is NO CPU fallback: without a CUDA device every compute call fails
+ *     with CHEM_E_CUDA.
+ */
+#ifndef CHEM_H_
+#define CHEM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CHEM_OK 0
+#define CHEM_E_ARG (-1)         /* invalid argument / inconsistent description      */
+#define CHEM_E_UNSUPPORTED (-2) /* description outside the compiled limits           */
+#define CHEM_E_CUDA (-3)        /* CUDA runtime error (see chem_last_error)          */
+#define CHEM_E_NOMEM (-4)
+
+/* reaction types */
+#define CHEM_RXN_ELEMENTARY 0
+#define CHEM_RXN_THREE_BODY 1        /* q = [M] (kf prod C - kr prod C)                */
+#define CHEM_RXN_FALLOFF_LINDEMANN 2 /* k = k_inf Pr/(1+Pr), Pr = k_0 [M] / k_inf      */
+#define CHEM_RXN_FALLOFF_TROE 3      /* ... times the Troe broadening factor F         */
+
+/* Mechanism description: plain host arrays, borrowed for the duration of chem_mech_load.
+ * All reactions are reversible; reverse rate constants follow from the equilibrium
+ * constants of the NASA-7 thermo data.  The LAST species is the bath species removed
+ * from the state vector (Y_N = 1 - sum Y_k). */
+typedef struct chem_mech_desc {
+    int32_t n_species;        /* N_sp >= 2; the state vector has N = N_sp entries (T, Y_1..Y_{N_sp-1}) */
+    int32_t n_reactions;      /* >= 1                                                                 */
+    const double *mol_weight; /* [n_species] g/mol                                                    */
+    const double *nasa_lo;    /* [n_species][7] a0..a6 for T <= nasa_tmid                             */
+    const double *nasa_hi;    /* [n_species][7] a0..a6 for T >  nasa_tmid                             */
+    const double *nasa_tmid;  /* [n_species] K                                                        */
+    const int32_t *rxn_type;  /* [n_reactions] CHEM_RXN_*                                             */
+    const int32_t *reac_ptr;  /* [n_reactions+1] CSR offsets into reac_sp / reac_nu                    */
+    const int32_t *reac_sp;   /* reactant species indices (0-based)                                   */
+    const int32_t *reac_nu;   /* reactant stoichiometric coefficients, integers 1..3                  */
+    const int32_t *prod_ptr;  /* same for products                                                    */
+    const int32_t *prod_sp;
+    const int32_t *prod_nu;
+    const double *arr_A;      /* [n_reactions] k = A T^b exp(-Ea/(R T)); the high-pressure limit for falloff */
+    const double *arr_b;
+    const double *arr_Ea;     /* cal/mol */
+    const double *low_A;      /* [n_reactions] low-pressure limit k_0 (read for falloff types only)   */
+    const double *low_b;
+    const double *low_Ea;
+    const double *troe;       /* [n_reactions][4] alpha, T***, T*, T** (read for CHEM_RXN_FALLOFF_TROE) */
+    const int32_t *eff_ptr;   /* [n_reactions+1] CSR of third-body efficiencies that differ from 1    */
+    const int32_t *eff_sp;
+    const double *eff_val;
+} chem_mech_desc;
+
+typedef struct chem_mech chem_mech; /* opaque: packed device tables + launch configuration */
+
+/* Options of chem_integrate_ex.  Zero-initialise for the defaults. */
+typedef struct chem_opts {
+    double h0;           /* first internal step size; 0 -> t_end (R9)                      */
+    int32_t max_steps;   /* limit on internal step attempts per state; 0 -> 100000                    */
+    int32_t newton_max;  /* max simplified-Newton iterations per step; 0 -> 7                         */
+    int32_t kernel;      /* 0 auto; 1 generic shared-memory kernel; 2 register-resident warp kernel   */
+    int32_t reorder;     /* 0 off; 1 process states in order of decreasing predicted cost            */
+    const double *P_per_state; /* device [n_states] or NULL: per-state pressure overriding P        */
+} chem_opts;
+
+/* Per-state result record written by chem_integrate_ex (device array of n_states). */
+typedef struct chem_stats {
+    int32_t status;     /* 0 ok; -1 max_steps exceeded; -2 step size too small; -3 singular matrix 5x; -4 non-finite input */
+    int32_t nstep;      /* internal step attempts that reached the Newton loop (d_i of PAPER.md Eq. 3) */
+    int32_t naccpt;     /* accepted steps                                                              */
+    int32_t nrejct;     /* error-test rejections (after the first accepted step)                       */
+    int32_t nfcn;       /* source-term evaluations                                                     */
+    int32_t njac;       /* Jacobian evaluations                                                        */
+    int32_t ndec;       /* LU factorisations (each = one real + one complex N x N)                     */
+    int32_t nsol;       /* Newton iterations (each = one real + one complex solve)                     */
+    int32_t nnewt_fail; /* step attempts abandoned by the Newton convergence control                   */
+    int32_t reserved;
+    double h_last;      /* size of the last accepted internal step                                     */
+} chem_stats;
+
+/* Mechanism compiler: validates `desc` (host), packs it into device tables.
+ * On success *out owns device memory; release with chem_mech_free. */
+int chem_mech_load(const chem_mech_desc *desc, chem_mech **out);
+void chem_mech_free(chem_mech *mech);
+int chem_mech_info(const chem_mech *mech, int32_t *n_species, int32_t *n_reactions);
+
+/* Source term f(T, Y; P) for a batch (test hook and building block).
+ * y: device [n_states][N] row-major; f: device [n_states][N]. */
+int chem_rhs(const chem_mech *mech, int32_t n_states, double P, const double *y, double *f, void *stream);
+
+/* Analytical Jacobian J[s][i][j] = d f_i / d y_j, device [n_states][N][N] row-major. */
+int chem_jacobian(const chem_mech *mech, int32_t n_states, double P, const double *y, double *J, void *stream);
+
+/* Batched dense LU solve hook (the device LU/solve routines the integrator uses):
+ * solves A_s x_s = b_s for s < batch.  A: device [batch][n][n] row-major (complex: interleaved re,im),
+ * b: device [batch][n] (complex: interleaved), x: same shape as b.  info: device [batch], 0 or k+1 of a zero pivot. */
+int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const double *A, const double *b, double *x,
+                  int32_t *info, void *stream);
+
+/* The hot path: integrate every state from t = 0 to t_end at constant pressure P.
+ * y_in, y_out: device [n_states][N] row-major (may alias).  n_states == 0 is a no-op. */
+int chem_integrate(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
+                   const double *y_in, double *y_out, void *stream);
+
+/* Same with options and per-state statistics (stats: device [n_states] or NULL). */
+int chem_integrate_ex(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
+                      const double *y_in, double *y_out, const chem_opts *opts, chem_stats *stats, void *stream);
+
+/* End-to-end form with HOST buffers (the paper's timings include the transfers):
+ * copies y_in to the device, integrates, copies y_out (and stats if not NULL) back, synchronises. */
+int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
+                        const double *y_in_host, double *y_out_host, const chem_opts *opts, chem_stats *stats_host);
+
+/* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
+int64_t chem_launch_count(void);
+
+/* Algorithmic floating-point operation counts of the compiled mechanism:
+ * out[0] = one source-term evaluation, out[1] = one Jacobian evaluation, out[2] = one LU pair (real + complex),
+ * out[3] = one Newton iteration's solves and vector work (excluding its 3 source terms), out[4] = error estimate. */
+int chem_flop_model(const chem_mech *mech, double out[5]);
+
+const char *chem_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHEM_H_ */

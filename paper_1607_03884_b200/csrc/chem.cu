@@ -1,0 +1,239 @@
+// chem.cu -- C ABI (include/chem.h): mechanism compiler, kernels, launch logic.
+// sm_100a only; no CPU fallback: every compute entry point fails with CHEM_E_CUDA without a device.
+#include "../../include/chem.h"
+
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "chem_radau.cuh"
+
+using namespace chem;
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<int64_t> g_launches{0};
+
+int fail(int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+#define CUDA_TRY(expr)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (expr);                                                                    \
+        if (e_ != cudaSuccess) return fail(CHEM_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e_));   \
+    } while (0)
+
+}  // namespace
+
+struct chem_mech {
+    Tables t{};
+    void *dev_blob = nullptr;   // one allocation holding every table
+    int *counter = nullptr;     // work-queue head (device)
+    int n_sm = 0;
+    int max_smem_optin = 0;
+    // algorithmic flop model
+    double flops[5] = {0, 0, 0, 0, 0};
+};
+
+// ------------------------------------------------------------------------------------------------
+// Mechanism compiler: validate the description and pack it into coefficient-major / slot-major tables.
+extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
+{
+    if (!d || !out) return fail(CHEM_E_ARG, "null argument");
+    *out = nullptr;
+    const int ns = d->n_species, nr = d->n_reactions;
+    if (ns < 2 || nr < 1) return fail(CHEM_E_ARG, "need n_species >= 2 and n_reactions >= 1");
+    if (!d->mol_weight || !d->nasa_lo || !d->nasa_hi || !d->nasa_tmid || !d->rxn_type || !d->reac_ptr || !d->reac_sp ||
+        !d->reac_nu || !d->prod_ptr || !d->prod_sp || !d->prod_nu || !d->arr_A || !d->arr_b || !d->arr_Ea || !d->eff_ptr)
+        return fail(CHEM_E_ARG, "null array in description");
+    for (int k = 0; k < ns; k++)
+        if (!(d->mol_weight[k] > 0.0) || !(d->nasa_tmid[k] > 0.0)) return fail(CHEM_E_ARG, "species %d: bad weight or tmid", k);
+
+    std::vector<double> W(ns), invW(ns), lo(7 * ns), hi(7 * ns), tmid(ns);
+    for (int k = 0; k < ns; k++) {
+        W[k] = d->mol_weight[k];
+        invW[k] = 1.0 / W[k];
+        tmid[k] = d->nasa_tmid[k];
+        for (int c = 0; c < 7; c++) {
+            lo[c * ns + k] = d->nasa_lo[7 * k + c];
+            hi[c * ns + k] = d->nasa_hi[7 * k + c];
+        }
+    }
+    std::vector<int> rtype(nr), slot_sp(6 * nr, 0), slot_nu(6 * nr, 0), eff_ptr(nr + 1, 0), eff_sp;
+    std::vector<double> lnA(nr), b(nr), Ta(nr), lnA0(nr, 0.0), b0(nr, 0.0), Ta0(nr, 0.0), dnu(nr), troe(4 * nr, 1.0), eff_dv;
+    std::vector<std::vector<std::pair<int, double>>> inc(ns);
+    long n_slots_used = 0, n_eff = 0, n_fall = 0, n_troe = 0, n_tb = 0;
+    for (int i = 0; i < nr; i++) {
+        const int ty = d->rxn_type[i];
+        if (ty < 0 || ty > 3) return fail(CHEM_E_ARG, "reaction %d: unknown type %d", i, ty);
+        rtype[i] = ty;
+        if (!(d->arr_A[i] > 0.0)) return fail(CHEM_E_ARG, "reaction %d: A must be positive", i);
+        lnA[i] = std::log(d->arr_A[i]);
+        b[i] = d->arr_b[i];
+        Ta[i] = d->arr_Ea[i] / kRcal;
+        if (ty >= 2) {
+            if (!d->low_A || !d->low_b || !d->low_Ea || !(d->low_A[i] > 0.0))
+                return fail(CHEM_E_ARG, "reaction %d: falloff needs a positive low-pressure A", i);
+            lnA0[i] = std::log(d->low_A[i]);
+            b0[i] = d->low_b[i];
+            Ta0[i] = d->low_Ea[i] / kRcal;
+            n_fall++;
+        }
+        if (ty == 3) {
+            if (!d->troe) return fail(CHEM_E_ARG, "reaction %d: Troe parameters missing", i);
+            for (int c = 0; c < 4; c++) troe[c * nr + i] = d->troe[4 * i + c];
+            if (troe[nr + i] == 0.0 || troe[2 * nr + i] == 0.0) return fail(CHEM_E_ARG, "reaction %d: Troe T*** or T* is zero", i);
+            n_troe++;
+        }
+        if (ty != 0) n_tb++;
+        std::vector<double> net(ns, 0.0);
+        double dn = 0.0;
+        for (int side = 0; side < 2; side++) {
+            const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr, *sp = side ? d->prod_sp : d->reac_sp, *nu = side ? d->prod_nu : d->reac_nu;
+            const int n = ptr[i + 1] - ptr[i];
+            if (n < 1 || n > 3) return fail(CHEM_E_UNSUPPORTED, "reaction %d: %d species on one side (1..3 supported)", i, n);
+            for (int p = 0; p < n; p++) {
+                const int k = sp[ptr[i] + p], v = nu[ptr[i] + p];
+                if (k < 0 || k >= ns) return fail(CHEM_E_ARG, "reaction %d: species index %d out of range", i, k);
+                if (v < 1 || v > 3) return fail(CHEM_E_UNSUPPORTED, "reaction %d: stoichiometric coefficient %d (1..3 supported)", i, v);
+                slot_sp[(side * 3 + p) * nr + i] = k;
+                slot_nu[(side * 3 + p) * nr + i] = v;
+                net[k] += side ? v : -v;
+                dn += side ? v : -v;
+                n_slots_used++;
+            }
+        }
+        dnu[i] = dn;
+        for (int k = 0; k < ns; k++)
+            if (net[k] != 0.0) inc[k].push_back({i, net[k]});
+        if (ty != 0) {
+            if (d->eff_ptr[i + 1] < d->eff_ptr[i]) return fail(CHEM_E_ARG, "eff_ptr not monotone");
+            for (int p = d->eff_ptr[i]; p < d->eff_ptr[i + 1]; p++) {
+                if (!d->eff_sp || !d->eff_val) return fail(CHEM_E_ARG, "efficiency arrays missing");
+                const int k = d->eff_sp[p];
+                if (k < 0 || k >= ns) return fail(CHEM_E_ARG, "reaction %d: efficiency species out of range", i);
+                eff_sp.push_back(k);
+                eff_dv.push_back(d->eff_val[p] - 1.0);
+                n_eff++;
+            }
+        }
+        eff_ptr[i + 1] = (int)eff_sp.size();
+    }
+    std::vector<int> inc_ptr(ns + 1, 0), inc_rx;
+    std::vector<double> inc_nu;
+    for (int k = 0; k < ns; k++) {
+        for (auto &pr : inc[k]) { inc_rx.push_back(pr.first); inc_nu.push_back(pr.second); }
+        inc_ptr[k + 1] = (int)inc_rx.size();
+    }
+    if (eff_sp.empty()) { eff_sp.push_back(0); eff_dv.push_back(0.0); }
+    if (inc_rx.empty()) { inc_rx.push_back(0); inc_nu.push_back(0.0); }
+
+    int dev = 0, n_sm = 0, optin = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+
+    // one blob: doubles first, then ints (each array 16-byte aligned)
+    std::vector<std::pair<const void *, size_t>> parts;
+    std::vector<size_t> offs;
+    size_t total = 0;
+    auto add = [&](const void *p, size_t bytes) {
+        offs.push_back(total);
+        parts.push_back({p, bytes});
+        total += (bytes + 15) & ~size_t(15);
+    };
+    add(W.data(), ns * 8); add(invW.data(), ns * 8); add(lo.data(), 7 * ns * 8); add(hi.data(), 7 * ns * 8); add(tmid.data(), ns * 8);
+    add(lnA.data(), nr * 8); add(b.data(), nr * 8); add(Ta.data(), nr * 8); add(lnA0.data(), nr * 8); add(b0.data(), nr * 8);
+    add(Ta0.data(), nr * 8); add(dnu.data(), nr * 8); add(troe.data(), 4 * nr * 8);
+    add(eff_dv.data(), eff_dv.size() * 8); add(inc_nu.data(), inc_nu.size() * 8);
+    add(rtype.data(), nr * 4); add(slot_sp.data(), 6 * nr * 4); add(slot_nu.data(), 6 * nr * 4);
+    add(eff_ptr.data(), (nr + 1) * 4); add(eff_sp.data(), eff_sp.size() * 4);
+    add(inc_ptr.data(), (ns + 1) * 4); add(inc_rx.data(), inc_rx.size() * 4);
+    std::vector<char> host(total, 0);
+    for (size_t a = 0; a < parts.size(); a++) std::memcpy(host.data() + offs[a], parts[a].first, parts[a].second);
+
+    chem_mech *m = new (std::nothrow) chem_mech;
+    if (!m) return fail(CHEM_E_NOMEM, "out of host memory");
+    if (cudaMalloc(&m->dev_blob, total) != cudaSuccess || cudaMalloc(&m->counter, 64) != cudaSuccess) {
+        cudaError_t e = cudaGetLastError();
+        if (m->dev_blob) cudaFree(m->dev_blob);
+        delete m;
+        return fail(CHEM_E_CUDA, "cudaMalloc: %s", cudaGetErrorString(e));
+    }
+    if (cudaMemcpy(m->dev_blob, host.data(), total, cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaError_t e = cudaGetLastError();
+        cudaFree(m->dev_blob); cudaFree(m->counter);
+        delete m;
+        return fail(CHEM_E_CUDA, "cudaMemcpy: %s", cudaGetErrorString(e));
+    }
+    const char *base = static_cast<const char *>(m->dev_blob);
+    int a = 0;
+    auto D = [&]() { return reinterpret_cast<const double *>(base + offs[a++]); };
+    auto I = [&]() { return reinterpret_cast<const int *>(base + offs[a++]); };
+    Tables &t = m->t;
+    t.n_sp = ns; t.n_rx = nr;
+    t.W = D(); t.invW = D(); t.nasa_lo = D(); t.nasa_hi = D(); t.tmid = D();
+    t.lnA = D(); t.b = D(); t.Ta = D(); t.lnA0 = D(); t.b0 = D(); t.Ta0 = D(); t.dnu = D(); t.troe = D();
+    t.eff_dv = D(); t.inc_nu = D();
+    t.rtype = I(); t.slot_sp = I(); t.slot_nu = I(); t.eff_ptr = I(); t.eff_sp = I(); t.inc_ptr = I(); t.inc_rx = I();
+    m->n_sm = n_sm;
+    m->max_smem_optin = optin;
+
+    // Algorithmic flop model: +,-,*,/ count 1; exp/log/pow/log10/exp10/sqrt count kTrans each.
+    const double kTrans = 20.0, N = ns;
+    const double thermo = ns * (8.0 + 11.0 + 12.0 + 1.0) + kTrans;                      // cp, h, s (Horner), g; one log T
+    const double front = 4.0 * ns + 6.0 + ns * 2.0;                                      // closure, Wbar, rho, C_k
+    const double rx = nr * (5.0 + 2.0 * kTrans + 4.0 + 3.0) + n_slots_used * 3.0        // ln kf, Kc, 2 exp, products, q
+                      + n_tb * 2.0 + n_eff * 2.0 + n_fall * (8.0 + kTrans) + n_troe * (25.0 + 5.0 * kTrans);
+    const double wd = 2.0 * inc_rx.size() + 6.0 * ns + 4.0;                              // wdot gather, Tdot, Ydot
+    m->flops[0] = thermo + front + rx + wd + 2.0 * kTrans;
+    m->flops[1] = m->flops[0] + ns * 7.0 + nr * 40.0 + n_troe * 40.0 + 12.0 * inc_rx.size() + 2.0 * n_eff * 3.0
+                  + ns * (2.0 * N + 6.0 * N) + N * (2.0 * N + 6.0 * N);                 // derivative slots, rows, columns
+    m->flops[2] = (2.0 / 3.0) * N * N * N * 5.0 + 3.0 * N * N;                           // real LU + complex LU (4x) + forming E1, E2
+    m->flops[3] = 2.0 * N * N * 5.0 + N * (15.0 + 9.0 + 15.0 + 9.0 + 3.0);               // real + complex solves, transforms, norm
+    m->flops[4] = 2.0 * N * N + N * 10.0;                                                // error estimate: one real solve + norm
+    *out = m;
+    return CHEM_OK;
+}
+
+extern "C" void chem_mech_free(chem_mech *m)
+{
+    if (!m) return;
+    if (m->dev_blob) cudaFree(m->dev_blob);
+    if (m->counter) cudaFree(m->counter);
+    delete m;
+}
+
+extern "C" int chem_mech_info(const chem_mech *m, int32_t *n_species, int32_t *n_reactions)
+{
+    if (!m) return fail(CHEM_E_ARG, "null mechanism");
+    if (n_species) *n_species = m->t.n_sp;
+    if (n_reactions) *n_reactions = m->t.n_rx;
+    return CHEM_OK;
+}
+
+extern "C" int chem_flop_model(const chem_mech *m, double out[5])
+{
+    if (!m || !out) return fail(CHEM_E_ARG, "null argument");
+    for (int i = 0; i < 5; i++) out[i] = m->flops[i];
+    return CHEM_OK;
+}
+
+extern "C" int64_t chem_launch_count(void) { return g_launches.load(); }
+extern "C" const char *chem_last_error(void) { return g_err.c_str(); }
+
+#include "chem_kernels.inl"

@@ -1,0 +1,515 @@
+// chem_device.cuh -- group-cooperative device routines: thermo, species rates, source term,
+// analytical Jacobian, dense LU / solves (real and complex), and the Radau IIA step engine.
+//
+// A "group" is G threads that own ONE thermochemical state: a warp (G = 32) for small mechanisms,
+// a whole CTA (G = 128) for GRI-sized ones.  Control flow is uniform inside a group, so the
+// intra-warp divergence the paper names as its first limiter does not occur;
+// all per-state data (Jacobian, LU factors, stage vectors) lives in shared memory, which removes the
+// second limiter (L182: "storage of the Jacobian matrix and/or factorized forms ... overwhelm the
+// registers and L1").  See DESIGN.md for the readings R1..R12 cited below.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace chem {
+
+constexpr double kRerg = 8.31446261815324e7;  // erg/(mol K)
+constexpr double kRcal = 1.98720425864083;    // cal/(mol K)
+constexpr double kPatm = 1.01325e6;           // dyn/cm^2
+constexpr int kSlots = 6;                     // 3 reactant + 3 product slots per reaction
+
+// Packed device tables written by the mechanism compiler (chem_mech_load).
+struct Tables {
+    int n_sp, n_rx;
+    const double *W, *invW;           // [n_sp]
+    const double *nasa_lo, *nasa_hi;  // [7][n_sp], coefficient-major
+    const double *tmid;               // [n_sp]
+    const int *rtype;                 // [n_rx]
+    const double *lnA, *b, *Ta;       // [n_rx]  ln A, b, Ea/R [K]
+    const double *lnA0, *b0, *Ta0;    // [n_rx]  low-pressure limit
+    const double *dnu;                // [n_rx]  sum nu'' - sum nu'
+    const double *troe;               // [4][n_rx]
+    const int *slot_sp, *slot_nu;     // [6][n_rx]; slots 0-2 reactants, 3-5 products; unused: sp 0, nu 0
+    const int *eff_ptr, *eff_sp;      // CSR over reactions
+    const double *eff_dv;             // alpha - 1
+    const int *inc_ptr, *inc_rx;      // CSR over species: reactions the species takes part in
+    const double *inc_nu;             // net stoichiometric coefficient nu'' - nu'
+};
+
+// ---------------------------------------------------------------------------------------------
+template <int G>
+struct Grp {
+    static constexpr int NW = G / 32;
+    __device__ static __forceinline__ int lane() { return G == 32 ? (threadIdx.x & 31) : (int)threadIdx.x; }
+    __device__ static __forceinline__ int wlane() { return threadIdx.x & 31; }
+    __device__ static __forceinline__ int warp() { return G == 32 ? 0 : (int)(threadIdx.x >> 5); }
+    __device__ static __forceinline__ void sync()
+    {
+        if (G == 32) __syncwarp(); else __syncthreads();
+    }
+    // all-reduce of two sums; every thread of the group gets bitwise the same result.
+    // `red` = shared scratch of 2*NW doubles (unused for G == 32).
+    __device__ static __forceinline__ void sum2(double &a, double &b, double *red)
+    {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a += __shfl_xor_sync(0xffffffffu, a, o);
+            b += __shfl_xor_sync(0xffffffffu, b, o);
+        }
+        if (G > 32) {
+            __syncthreads();
+            if (wlane() == 0) { red[2 * warp()] = a; red[2 * warp() + 1] = b; }
+            __syncthreads();
+            a = 0.0; b = 0.0;
+#pragma unroll
+            for (int w = 0; w < NW; w++) { a += red[2 * w]; b += red[2 * w + 1]; }
+        }
+    }
+    __device__ static __forceinline__ int any(int p, double *red)
+    {
+        if (G == 32) return __any_sync(0xffffffffu, p);
+        return __syncthreads_or(p);
+    }
+};
+
+__device__ __forceinline__ double powi(double c, int nu)
+{
+    return nu == 0 ? 1.0 : (nu == 1 ? c : (nu == 2 ? c * c : c * c * c));
+}
+__device__ __forceinline__ double dpowi(double c, int nu)  // d/dc c^nu
+{
+    return nu == 0 ? 0.0 : (nu == 1 ? 1.0 : (nu == 2 ? 2.0 * c : 3.0 * c * c));
+}
+
+// Chemistry scratch of one group (shared memory).
+struct ChemScratch {
+    double *C, *g, *hRT, *cpR, *dcpR, *wdot;  // [n_sp]
+    double *q;                                // [n_rx]
+    double *dq;                               // [6][n_rx]   (Jacobian only)
+    double *dqdT, *tb;                        // [n_rx]      (Jacobian only)
+    double *red;                              // [2*NW]
+};
+
+// Mixture state derived from ys = (T, Y_1..Y_{N-1}): fills C, g = h/RT - s/R, hRT, cpR (and dcpR).
+// DESIGN.md R1 (state, closure, ideal gas) and R2 (NASA-7).
+template <int G, bool JAC>
+__device__ __forceinline__ void front_end(const Tables &t, const ChemScratch &s, double P, const double *ys, double &T,
+                                          double &rho, double &Wbar)
+{
+    const int N = t.n_sp;
+    const int lane = Grp<G>::lane();
+    T = ys[0];
+    double sY = 0.0, sYW = 0.0;
+    for (int k = lane; k < N - 1; k += G) {
+        const double Yk = ys[k + 1];
+        sY += Yk;
+        sYW += Yk * __ldg(&t.invW[k]);
+    }
+    Grp<G>::sum2(sY, sYW, s.red);
+    const double YN = 1.0 - sY;
+    sYW += YN * __ldg(&t.invW[N - 1]);
+    Wbar = 1.0 / sYW;
+    rho = P * Wbar / (kRerg * T);
+    const double lnT = log(T);
+    const double invT = 1.0 / T;
+    for (int k = lane; k < N; k += G) {
+        const double Yk = (k < N - 1) ? ys[k + 1] : YN;
+        s.C[k] = rho * Yk * __ldg(&t.invW[k]);
+        const double *a = (T <= __ldg(&t.tmid[k])) ? t.nasa_lo : t.nasa_hi;
+        const double a0 = __ldg(&a[k]), a1 = __ldg(&a[N + k]), a2 = __ldg(&a[2 * N + k]), a3 = __ldg(&a[3 * N + k]);
+        const double a4 = __ldg(&a[4 * N + k]), a5 = __ldg(&a[5 * N + k]), a6 = __ldg(&a[6 * N + k]);
+        const double cp = a0 + T * (a1 + T * (a2 + T * (a3 + T * a4)));
+        const double h = a0 + T * (a1 * 0.5 + T * (a2 * (1.0 / 3.0) + T * (a3 * 0.25 + T * (a4 * 0.2)))) + a5 * invT;
+        const double sR = a0 * lnT + T * (a1 + T * (a2 * 0.5 + T * (a3 * (1.0 / 3.0) + T * (a4 * 0.25)))) + a6;
+        s.cpR[k] = cp;
+        s.hRT[k] = h;
+        s.g[k] = h - sR;
+        if (JAC) s.dcpR[k] = a1 + T * (2.0 * a2 + T * (3.0 * a3 + T * (4.0 * a4)));
+    }
+    Grp<G>::sync();
+}
+
+// Rate of progress of reaction i (R3 mass action + Arrhenius + Kc, R4 third body, R5 falloff/Troe).
+// With JAC also the partial derivatives at constant C (dq/dT), per slot (dq/dC_slot) and through [M] (tb).
+template <bool JAC>
+__device__ __forceinline__ double reaction(const Tables &t, int i, double T, double lnT, double invT, double lnPRT,
+                                           double Ctot, const ChemScratch &s)
+{
+    const int NR = t.n_rx;
+    const double b = __ldg(&t.b[i]), Ta = __ldg(&t.Ta[i]);
+    const double lnkf = __ldg(&t.lnA[i]) + b * lnT - Ta * invT;
+    double dG = 0.0, dH = 0.0;
+    double pw[kSlots], cs[kSlots];
+    int nus[kSlots];
+#pragma unroll
+    for (int sl = 0; sl < kSlots; sl++) {
+        const int sp = __ldg(&t.slot_sp[sl * NR + i]);
+        const int nu = __ldg(&t.slot_nu[sl * NR + i]);
+        const double c = s.C[sp];
+        const double sgn = (sl < 3) ? -(double)nu : (double)nu;
+        dG += sgn * s.g[sp];
+        if (JAC) dH += sgn * s.hRT[sp];
+        pw[sl] = powi(c, nu);
+        cs[sl] = c;
+        nus[sl] = nu;
+    }
+    const double dnu = __ldg(&t.dnu[i]);
+    const double kf = exp(lnkf);
+    const double kr = exp(lnkf - (dnu * lnPRT - dG));   // kf / Kc
+    const double Rf = kf * (pw[0] * pw[1] * pw[2]);
+    const double Rr = kr * (pw[3] * pw[4] * pw[5]);
+    const double rnet = Rf - Rr;
+    const int type = __ldg(&t.rtype[i]);
+    double c = 1.0, dc_dT = 0.0, dc_dM = 0.0;
+    const double dlnkf = (b + Ta * invT) * invT;
+    if (type != 0) {
+        double M = Ctot;
+        for (int p = __ldg(&t.eff_ptr[i]); p < __ldg(&t.eff_ptr[i + 1]); p++)
+            M += __ldg(&t.eff_dv[p]) * s.C[__ldg(&t.eff_sp[p])];
+        if (type == 1) {
+            c = M;
+            dc_dM = 1.0;
+        } else {
+            const double b0 = __ldg(&t.b0[i]), Ta0 = __ldg(&t.Ta0[i]);
+            const double k0_over_kinf = exp(__ldg(&t.lnA0[i]) + b0 * lnT - Ta0 * invT - lnkf);
+            const double Pr = k0_over_kinf * M;
+            const double dlnPr_dT = (b0 + Ta0 * invT) * invT - dlnkf;
+            double F = 1.0, dF_dT = 0.0, dF_dPr = 0.0;
+            if (type == 3) {
+                const double al = __ldg(&t.troe[i]), T3 = __ldg(&t.troe[NR + i]);
+                const double T1 = __ldg(&t.troe[2 * NR + i]), T2 = __ldg(&t.troe[3 * NR + i]);
+                const double e3 = (1.0 - al) * exp(-T / T3), e1 = al * exp(-T / T1), e2 = exp(-T2 * invT);
+                const double Fc = e3 + e1 + e2;
+                const double L = log10(Fc);
+                const double cc = -0.4 - 0.67 * L, nn = 0.75 - 1.27 * L;
+                const double At = log10(Pr) + cc;
+                const double Bt = nn - 0.14 * At;
+                const double x = At / Bt;
+                const double den = 1.0 + x * x;
+                F = exp10(L / den);
+                if (JAC) {
+                    const double ln10 = 2.302585092994045684;
+                    const double dFc = -e3 / T3 - e1 / T1 + e2 * T2 * invT * invT;
+                    const double dL = dFc / (Fc * ln10);
+                    const double dA_T = dlnPr_dT / ln10 - 0.67 * dL;
+                    const double dB_T = -1.27 * dL - 0.14 * dA_T;
+                    const double dx_T = (dA_T * Bt - At * dB_T) / (Bt * Bt);
+                    const double dA_P = 1.0 / (Pr * ln10);
+                    const double dx_P = dA_P * (Bt + 0.14 * At) / (Bt * Bt);
+                    const double w = -L * 2.0 * x / (den * den);
+                    dF_dT = F * ln10 * (dL / den + w * dx_T);
+                    dF_dPr = F * ln10 * w * dx_P;
+                }
+            }
+            const double op = 1.0 / (1.0 + Pr);
+            c = Pr * op * F;
+            if (JAC) {
+                dc_dT = Pr * dlnPr_dT * op * op * F + Pr * op * dF_dT;
+                dc_dM = (op * op * F + Pr * op * dF_dPr) * k0_over_kinf;
+            }
+        }
+    }
+    const double q = c * rnet;
+    if (JAC) {
+        // van 't Hoff: d ln kr/dT = d ln kf/dT - (sum nu h/RT - dnu)/T
+        const double dlnkr = dlnkf - (dH - dnu) * invT;
+        s.dqdT[i] = dc_dT * rnet + c * (Rf * dlnkf - Rr * dlnkr);
+        s.tb[i] = dc_dM * rnet;
+        const double ckf = c * kf, ckr = c * kr;
+        s.dq[0 * NR + i] = ckf * dpowi(cs[0], nus[0]) * pw[1] * pw[2];
+        s.dq[1 * NR + i] = ckf * dpowi(cs[1], nus[1]) * pw[0] * pw[2];
+        s.dq[2 * NR + i] = ckf * dpowi(cs[2], nus[2]) * pw[0] * pw[1];
+        s.dq[3 * NR + i] = -ckr * dpowi(cs[3], nus[3]) * pw[4] * pw[5];
+        s.dq[4 * NR + i] = -ckr * dpowi(cs[4], nus[4]) * pw[3] * pw[5];
+        s.dq[5 * NR + i] = -ckr * dpowi(cs[5], nus[5]) * pw[3] * pw[4];
+    }
+    return q;
+}
+
+// Source term f(T, Y; P) of one state (R1): f[0] = dT/dt, f[k+1] = dY_k/dt.  ys, f: shared, length N.
+template <int G>
+__device__ __forceinline__ void rhs(const Tables &t, const ChemScratch &s, double P, const double *ys, double *f)
+{
+    const int N = t.n_sp, NR = t.n_rx;
+    const int lane = Grp<G>::lane();
+    double T, rho, Wbar;
+    front_end<G, false>(t, s, P, ys, T, rho, Wbar);
+    const double lnT = log(T), invT = 1.0 / T;
+    const double Ctot = P / (kRerg * T);
+    const double lnPRT = log(kPatm / (kRerg * T));
+    for (int i = lane; i < NR; i += G) s.q[i] = reaction<false>(t, i, T, lnT, invT, lnPRT, Ctot, s);
+    Grp<G>::sync();
+    double hw = 0.0, ccp = 0.0;
+    for (int k = lane; k < N; k += G) {
+        double w = 0.0;
+        for (int p = __ldg(&t.inc_ptr[k]); p < __ldg(&t.inc_ptr[k + 1]); p++)
+            w += __ldg(&t.inc_nu[p]) * s.q[__ldg(&t.inc_rx[p])];
+        hw += s.hRT[k] * w;
+        ccp += s.C[k] * s.cpR[k];
+        if (k < N - 1) f[k + 1] = __ldg(&t.W[k]) * w / rho;
+    }
+    Grp<G>::sum2(hw, ccp, s.red);
+    if (lane == 0) f[0] = -T * hw / ccp;
+    Grp<G>::sync();
+}
+
+// Analytical Jacobian (R6), Jm: shared N x N row-major, Jm[i*N+j] = d f_i / d y_j.
+// Uses that at constant (T, P) the total concentration is independent of Y, so the unit part of the
+// third-body efficiencies only enters d/dT.
+template <int G>
+__device__ __forceinline__ void jacobian(const Tables &t, const ChemScratch &s, double P, const double *ys, double *Jm)
+{
+    const int N = t.n_sp, NR = t.n_rx;
+    const int lane = Grp<G>::lane();
+    double T, rho, Wbar;
+    front_end<G, true>(t, s, P, ys, T, rho, Wbar);
+    const double lnT = log(T), invT = 1.0 / T;
+    const double Ctot = P / (kRerg * T);
+    const double lnPRT = log(kPatm / (kRerg * T));
+    for (int i = lane; i < NR; i += G) s.q[i] = reaction<true>(t, i, T, lnT, invT, lnPRT, Ctot, s);
+    Grp<G>::sync();
+    const double invWN = __ldg(&t.invW[N - 1]);
+    // rows: species k -> Dw[k][j] = d wdot_k / d y_j, stored in Jm row k
+    double hw = 0.0, ccp = 0.0, cpw = 0.0, cdcp = 0.0;
+    for (int k = lane; k < N; k += G) {
+        double *row = Jm + k * N;
+        for (int l = 0; l < N; l++) row[l] = 0.0;
+        double wd = 0.0, dwT = 0.0, u = 0.0;
+        for (int p = __ldg(&t.inc_ptr[k]); p < __ldg(&t.inc_ptr[k + 1]); p++) {
+            const int i = __ldg(&t.inc_rx[p]);
+            const double nu = __ldg(&t.inc_nu[p]);
+            wd += nu * s.q[i];
+            dwT += nu * s.dqdT[i];
+#pragma unroll
+            for (int sl = 0; sl < kSlots; sl++) row[__ldg(&t.slot_sp[sl * NR + i])] += nu * s.dq[sl * NR + i];
+            if (__ldg(&t.rtype[i]) != 0) {
+                const double v = nu * s.tb[i];
+                u += v;
+                for (int pe = __ldg(&t.eff_ptr[i]); pe < __ldg(&t.eff_ptr[i + 1]); pe++)
+                    row[__ldg(&t.eff_sp[pe])] += v * __ldg(&t.eff_dv[pe]);
+            }
+        }
+        double GC = 0.0;
+        for (int l = 0; l < N; l++) GC += row[l] * s.C[l];
+        const double GN = row[N - 1] * invWN;
+        for (int j = N - 1; j >= 1; j--) {
+            const double dj = __ldg(&t.invW[j - 1]) - invWN;
+            row[j] = -Wbar * dj * GC + rho * (row[j - 1] * __ldg(&t.invW[j - 1]) - GN);
+        }
+        row[0] = dwT - (GC + u * Ctot) * invT;
+        s.wdot[k] = wd;
+        hw += s.hRT[k] * wd;
+        ccp += s.C[k] * s.cpR[k];
+        cpw += s.cpR[k] * wd;
+        cdcp += s.C[k] * s.dcpR[k];
+    }
+    Grp<G>::sum2(hw, ccp, s.red);
+    Grp<G>::sum2(cpw, cdcp, s.red);
+    Grp<G>::sync();
+    const double Tdot = -T * hw / ccp;
+    // columns: assemble the rows of J in place (row k+1 <- species k, descending; row 0 <- temperature)
+    for (int j = lane; j < N; j += G) {
+        double S = 0.0;
+        for (int k = 0; k < N; k++) S += s.hRT[k] * Jm[k * N + j];
+        double dlnrho, drcp;   // d ln rho / d y_j ; d(sum C cpR) / d y_j
+        if (j == 0) {
+            dlnrho = -invT;
+            drcp = -ccp * invT + cdcp;
+        } else {
+            const double dj = __ldg(&t.invW[j - 1]) - invWN;
+            dlnrho = -Wbar * dj;
+            drcp = -Wbar * dj * ccp + rho * (s.cpR[j - 1] * __ldg(&t.invW[j - 1]) - s.cpR[N - 1] * invWN);
+        }
+        for (int k = N - 2; k >= 0; k--) {
+            const double Wk = __ldg(&t.W[k]);
+            Jm[(k + 1) * N + j] = Wk / rho * Jm[k * N + j] - Wk * s.wdot[k] / rho * dlnrho;
+        }
+        Jm[j] = -(T * S + (j == 0 ? cpw : 0.0)) / ccp - Tdot * drcp / ccp;
+    }
+    Grp<G>::sync();
+}
+
+// ------------------------------------------------------------------------------------- dense LU
+// Column-major N x N in shared memory: A[i + j*N].  Partial pivoting with full-row interchanges
+// (LAPACK convention), first maximum wins ties.  Returns 0 or k+1 (zero / non-finite pivot column).
+// "specialized implementations of ... LU factorization of the Jacobian".
+template <int G>
+__device__ __forceinline__ int lu_real(int N, double *A, int *ip)
+{
+    const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
+    for (int k = 0; k < N; k++) {
+        double best = -1.0;
+        int bi = k;
+        for (int i = k + wl; i < N; i += 32) {
+            const double v = fabs(A[i + k * N]);
+            if (v > best) { best = v; bi = i; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        if (lane == 0) ip[k] = bi;
+        if (!(best > 0.0) || !isfinite(best)) return k + 1;
+        Grp<G>::sync();   // every warp has read column k before rows move
+        if (bi != k)
+            for (int j = lane; j < N; j += G) {
+                const double a = A[k + j * N];
+                A[k + j * N] = A[bi + j * N];
+                A[bi + j * N] = a;
+            }
+        Grp<G>::sync();
+        const double piv = A[k + k * N];
+        Grp<G>::sync();
+        for (int i = k + 1 + lane; i < N; i += G) A[i + k * N] /= piv;
+        Grp<G>::sync();
+        for (int j = k + 1 + wp; j < N; j += Grp<G>::NW) {
+            const double u = A[k + j * N];
+            for (int i = k + 1 + wl; i < N; i += 32) A[i + j * N] -= A[i + k * N] * u;
+        }
+        Grp<G>::sync();
+    }
+    return 0;
+}
+
+// Complex version on split planes (Ar, Ai); pivot magnitude |re| + |im| (R10).
+template <int G>
+__device__ __forceinline__ int lu_complex(int N, double *Ar, double *Ai, int *ip)
+{
+    const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
+    for (int k = 0; k < N; k++) {
+        double best = -1.0;
+        int bi = k;
+        for (int i = k + wl; i < N; i += 32) {
+            const double v = fabs(Ar[i + k * N]) + fabs(Ai[i + k * N]);
+            if (v > best) { best = v; bi = i; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        if (lane == 0) ip[k] = bi;
+        if (!(best > 0.0) || !isfinite(best)) return k + 1;
+        Grp<G>::sync();
+        if (bi != k)
+            for (int j = lane; j < N; j += G) {
+                double a = Ar[k + j * N];
+                Ar[k + j * N] = Ar[bi + j * N];
+                Ar[bi + j * N] = a;
+                a = Ai[k + j * N];
+                Ai[k + j * N] = Ai[bi + j * N];
+                Ai[bi + j * N] = a;
+            }
+        Grp<G>::sync();
+        const double pr = Ar[k + k * N], pi = Ai[k + k * N];
+        Grp<G>::sync();
+        // l = a / p = a conj(p) / |p|^2
+        const double den = 1.0 / (pr * pr + pi * pi);
+        for (int i = k + 1 + lane; i < N; i += G) {
+            const double ar = Ar[i + k * N], ai = Ai[i + k * N];
+            Ar[i + k * N] = (ar * pr + ai * pi) * den;
+            Ai[i + k * N] = (ai * pr - ar * pi) * den;
+        }
+        Grp<G>::sync();
+        for (int j = k + 1 + wp; j < N; j += Grp<G>::NW) {
+            const double ur = Ar[k + j * N], ui = Ai[k + j * N];
+            for (int i = k + 1 + wl; i < N; i += 32) {
+                const double lr = Ar[i + k * N], li = Ai[i + k * N];
+                Ar[i + j * N] -= lr * ur - li * ui;
+                Ai[i + j * N] -= lr * ui + li * ur;
+            }
+        }
+        Grp<G>::sync();
+    }
+    return 0;
+}
+
+// Solves by ONE warp (lanes wl = 0..31) on shared vectors; P b first, then L, then U (column sweeps).
+__device__ __forceinline__ void solve_real_warp(int N, const double *A, const int *ip, double *b, int wl)
+{
+    if (wl == 0)
+        for (int k = 0; k < N; k++) {
+            const int p = ip[k];
+            const double tmp = b[p];
+            b[p] = b[k];
+            b[k] = tmp;
+        }
+    __syncwarp();
+    for (int k = 0; k < N - 1; k++) {
+        const double bk = b[k];
+        for (int i = k + 1 + wl; i < N; i += 32) b[i] -= A[i + k * N] * bk;
+        __syncwarp();
+    }
+    for (int k = N - 1; k >= 0; k--) {
+        const double bk = b[k] / A[k + k * N];
+        __syncwarp();
+        if (wl == 0) b[k] = bk;
+        for (int i = wl; i < k; i += 32) b[i] -= A[i + k * N] * bk;
+        __syncwarp();
+    }
+}
+__device__ __forceinline__ void solve_complex_warp(int N, const double *Ar, const double *Ai, const int *ip, double *br,
+                                                   double *bi, int wl)
+{
+    if (wl == 0)
+        for (int k = 0; k < N; k++) {
+            const int p = ip[k];
+            double tmp = br[p];
+            br[p] = br[k];
+            br[k] = tmp;
+            tmp = bi[p];
+            bi[p] = bi[k];
+            bi[k] = tmp;
+        }
+    __syncwarp();
+    for (int k = 0; k < N - 1; k++) {
+        const double xr = br[k], xi = bi[k];
+        for (int i = k + 1 + wl; i < N; i += 32) {
+            const double lr = Ar[i + k * N], li = Ai[i + k * N];
+            br[i] -= lr * xr - li * xi;
+            bi[i] -= lr * xi + li * xr;
+        }
+        __syncwarp();
+    }
+    for (int k = N - 1; k >= 0; k--) {
+        const double pr = Ar[k + k * N], pi = Ai[k + k * N];
+        const double den = 1.0 / (pr * pr + pi * pi);
+        const double vr = br[k], vi = bi[k];
+        const double xr = (vr * pr + vi * pi) * den, xi = (vi * pr - vr * pi) * den;
+        __syncwarp();
+        if (wl == 0) { br[k] = xr; bi[k] = xi; }
+        for (int i = wl; i < k; i += 32) {
+            const double ur = Ar[i + k * N], ui = Ai[i + k * N];
+            br[i] -= ur * xr - ui * xi;
+            bi[i] -= ur * xi + ui * xr;
+        }
+        __syncwarp();
+    }
+}
+
+// One real and one complex solve for the group: a single warp does both when G == 32, warps 0 and 1
+// work side by side when the group is a CTA.
+template <int G>
+__device__ __forceinline__ void solve_pair(int N, const double *E1, const int *ip1, double *z1, const double *E2r,
+                                           const double *E2i, const int *ip2, double *z2, double *z3)
+{
+    if (G == 32) {
+        solve_real_warp(N, E1, ip1, z1, Grp<G>::wlane());
+        solve_complex_warp(N, E2r, E2i, ip2, z2, z3, Grp<G>::wlane());
+    } else {
+        if (Grp<G>::warp() == 0) solve_real_warp(N, E1, ip1, z1, Grp<G>::wlane());
+        else if (Grp<G>::warp() == 1) solve_complex_warp(N, E2r, E2i, ip2, z2, z3, Grp<G>::wlane());
+    }
+    Grp<G>::sync();
+}
+template <int G>
+__device__ __forceinline__ void solve_real(int N, const double *E1, const int *ip1, double *b)
+{
+    if (Grp<G>::warp() == 0) solve_real_warp(N, E1, ip1, b, Grp<G>::wlane());
+    Grp<G>::sync();
+}
+
+}  // namespace chem

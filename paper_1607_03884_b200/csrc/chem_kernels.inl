@@ -1,0 +1,135 @@
+// chem_kernels.inl -- kernels and launch logic; included at the end of chem.cu.
+
+namespace {
+
+constexpr int kBlock = 128;   // threads per CTA for every kernel here
+
+// Group <-> CTA mapping: G == 32 -> four warp-groups per CTA, G == 128 -> the CTA is the group.
+template <int G>
+__device__ __forceinline__ int group_in_block() { return G == 32 ? (int)(threadIdx.x >> 5) : 0; }
+template <int G>
+constexpr int groups_per_block() { return kBlock / G; }
+
+// Next state index from the work queue (PAPER.md L194 names load imbalance between IVPs; groups that
+// finish early pull new states).  Uniform across the group.
+template <int G>
+__device__ __forceinline__ int next_state(int *counter, int *bcast)
+{
+    int s = 0;
+    if (G == 32) {
+        if ((threadIdx.x & 31) == 0) s = atomicAdd(counter, 1);
+        s = __shfl_sync(0xffffffffu, s, 0);
+    } else {
+        __syncthreads();
+        if (threadIdx.x == 0) *bcast = atomicAdd(counter, 1);
+        __syncthreads();
+        s = *bcast;
+    }
+    return s;
+}
+
+template <int G>
+__global__ void __launch_bounds__(kBlock) integrate_kernel(Tables t, int n_states, double P, const double *P_per_state,
+                                                           RadauParams prm, const double *__restrict__ y_in,
+                                                           double *__restrict__ y_out, chem_stats *stats, int *counter,
+                                                           const int *order)
+{
+    extern __shared__ double smem[];
+    __shared__ int bcast;
+    const int N = t.n_sp, NR = t.n_rx;
+    const size_t wd = work_doubles(N, NR, Grp<G>::NW);
+    Work w = carve(smem + (size_t)group_in_block<G>() * wd, N, NR, Grp<G>::NW);
+    const int lane = Grp<G>::lane();
+    for (;;) {
+        const int q = next_state<G>(counter, &bcast);
+        if (q >= n_states) break;
+        const int s = order ? order[q] : q;
+        for (int i = lane; i < N; i += G) w.y[i] = y_in[(size_t)s * N + i];
+        Grp<G>::sync();
+        RadauResult r;
+        radau_state<G>(t, w, P_per_state ? P_per_state[s] : P, prm, r);
+        Grp<G>::sync();
+        for (int i = lane; i < N; i += G) y_out[(size_t)s * N + i] = w.y[i];
+        if (stats && lane == 0) {
+            chem_stats o;
+            o.status = r.status; o.nstep = r.nstep; o.naccpt = r.naccpt; o.nrejct = r.nrejct; o.nfcn = r.nfcn;
+            o.njac = r.njac; o.ndec = r.ndec; o.nsol = r.nsol; o.nnewt_fail = r.nnewt_fail; o.reserved = 0;
+            o.h_last = r.h_last;
+            stats[s] = o;
+        }
+        Grp<G>::sync();
+    }
+}
+
+// Source term / Jacobian for a batch (static round-robin over groups).
+template <int G, bool JAC>
+__global__ void __launch_bounds__(kBlock) eval_kernel(Tables t, int n_states, double P, const double *__restrict__ y,
+                                                      double *__restrict__ out)
+{
+    extern __shared__ double smem[];
+    const int N = t.n_sp, NR = t.n_rx;
+    const size_t wd = work_doubles(N, NR, Grp<G>::NW);
+    Work w = carve(smem + (size_t)group_in_block<G>() * wd, N, NR, Grp<G>::NW);
+    const int lane = Grp<G>::lane();
+    const int gpb = kBlock / G;
+    for (int s = blockIdx.x * gpb + group_in_block<G>(); s < n_states; s += gridDim.x * gpb) {
+        for (int i = lane; i < N; i += G) w.y[i] = y[(size_t)s * N + i];
+        Grp<G>::sync();
+        if (JAC) {
+            jacobian<G>(t, w.cs, P, w.y, w.Jm);
+            for (int i = lane; i < N * N; i += G) out[(size_t)s * N * N + i] = w.Jm[i];
+        } else {
+            rhs<G>(t, w.cs, P, w.y, w.f0);
+            for (int i = lane; i < N; i += G) out[(size_t)s * N + i] = w.f0[i];
+        }
+        Grp<G>::sync();
+    }
+}
+
+// Batched LU solve hook: one warp per system, matrices staged column-major in shared memory.
+__global__ void __launch_bounds__(32) lu_solve_kernel(int n, int batch, int is_complex, const double *__restrict__ A,
+                                                      const double *__restrict__ b, double *__restrict__ x, int *info)
+{
+    extern __shared__ double smem[];
+    double *Ar = smem, *Ai = Ar + (size_t)n * n, *br = Ai + (size_t)n * n, *bi = br + n;
+    int *ip = reinterpret_cast<int *>(bi + n);
+    const int lane = threadIdx.x;
+    for (int s = blockIdx.x; s < batch; s += gridDim.x) {
+        if (is_complex) {
+            for (int e = lane; e < n * n; e += 32) {
+                const int i = e / n, j = e % n;
+                Ar[i + j * n] = A[((size_t)s * n * n + e) * 2];
+                Ai[i + j * n] = A[((size_t)s * n * n + e) * 2 + 1];
+            }
+            for (int i = lane; i < n; i += 32) { br[i] = b[((size_t)s * n + i) * 2]; bi[i] = b[((size_t)s * n + i) * 2 + 1]; }
+        } else {
+            for (int e = lane; e < n * n; e += 32) {
+                const int i = e / n, j = e % n;
+                Ar[i + j * n] = A[(size_t)s * n * n + e];
+            }
+            for (int i = lane; i < n; i += 32) br[i] = b[(size_t)s * n + i];
+        }
+        __syncwarp();
+        int ier;
+        if (is_complex) {
+            ier = lu_complex<32>(n, Ar, Ai, ip);
+            __syncwarp();
+            if (!ier) solve_complex_warp(n, Ar, Ai, ip, br, bi, lane);
+        } else {
+            ier = lu_real<32>(n, Ar, ip);
+            __syncwarp();
+            if (!ier) solve_real_warp(n, Ar, ip, br, lane);
+        }
+        __syncwarp();
+        if (is_complex)
+            for (int i = lane; i < n; i += 32) { x[((size_t)s * n + i) * 2] = br[i]; x[((size_t)s * n + i) * 2 + 1] = bi[i]; }
+        else
+            for (int i = lane; i < n; i += 32) x[(size_t)s * n + i] = br[i];
+        if (info && lane == 0) info[s] = ier;
+        __syncwarp();
+    }
+}
+
+}  // namespace
+
+#include "chem_launch.inl"

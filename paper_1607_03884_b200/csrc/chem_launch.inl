@@ -1,0 +1,141 @@
+// chem_launch.inl -- host launch logic and the compute entry points of include/chem.h.
+
+namespace {
+
+// group size: a warp per state up to 32 unknowns, a CTA per state above
+inline int group_size(const chem_mech *m) { return m->t.n_sp <= 32 ? 32 : 128; }
+
+template <typename K>
+int configure(K kernel, const chem_mech *m, size_t smem, int *ctas_per_sm)
+{
+    if (smem > (size_t)m->max_smem_optin)
+        return fail(CHEM_E_UNSUPPORTED, "mechanism needs %zu B of shared memory per CTA, device offers %d", smem, m->max_smem_optin);
+    CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kBlock, smem));
+    if (occ < 1) return fail(CHEM_E_UNSUPPORTED, "kernel does not fit on an SM");
+    *ctas_per_sm = occ;
+    return CHEM_OK;
+}
+
+template <int G, bool JAC>
+int launch_eval(const chem_mech *m, int n, double P, const double *y, double *out, cudaStream_t st)
+{
+    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32) * sizeof(double) * (kBlock / G);
+    int occ = 0;
+    int rc = configure(eval_kernel<G, JAC>, m, smem, &occ);
+    if (rc) return rc;
+    const int gpb = kBlock / G;
+    int grid = (n + gpb - 1) / gpb;
+    if (grid > m->n_sm * occ) grid = m->n_sm * occ;
+    eval_kernel<G, JAC><<<grid, kBlock, smem, st>>>(m->t, n, P, y, out);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return CHEM_OK;
+}
+
+template <int G>
+int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
+                     const chem_opts *o, chem_stats *stats, cudaStream_t st)
+{
+    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32) * sizeof(double) * (kBlock / G);
+    int occ = 0;
+    int rc = configure(integrate_kernel<G>, m, smem, &occ);
+    if (rc) return rc;
+    const int gpb = kBlock / G;
+    int grid = (n + gpb - 1) / gpb;
+    if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, groups pull work from the queue
+    CUDA_TRY(cudaMemsetAsync(m->counter, 0, sizeof(int), st));
+    integrate_kernel<G><<<grid, kBlock, smem, st>>>(m->t, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats,
+                                                    m->counter, nullptr);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return CHEM_OK;
+}
+
+}  // namespace
+
+extern "C" int chem_rhs(const chem_mech *m, int32_t n, double P, const double *y, double *f, void *stream)
+{
+    if (!m || n < 0 || (n > 0 && (!y || !f))) return fail(CHEM_E_ARG, "bad argument");
+    if (n == 0) return CHEM_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    return group_size(m) == 32 ? launch_eval<32, false>(m, n, P, y, f, st) : launch_eval<128, false>(m, n, P, y, f, st);
+}
+
+extern "C" int chem_jacobian(const chem_mech *m, int32_t n, double P, const double *y, double *J, void *stream)
+{
+    if (!m || n < 0 || (n > 0 && (!y || !J))) return fail(CHEM_E_ARG, "bad argument");
+    if (n == 0) return CHEM_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    return group_size(m) == 32 ? launch_eval<32, true>(m, n, P, y, J, st) : launch_eval<128, true>(m, n, P, y, J, st);
+}
+
+extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const double *A, const double *b, double *x,
+                             int32_t *info, void *stream)
+{
+    if (n < 1 || batch < 0 || (batch > 0 && (!A || !b || !x))) return fail(CHEM_E_ARG, "bad argument");
+    if (batch == 0) return CHEM_OK;
+    const size_t smem = ((size_t)2 * n * n + 2 * n) * sizeof(double) + (size_t)n * sizeof(int) + 16;
+    int dev = 0, optin = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    if (smem > (size_t)optin) return fail(CHEM_E_UNSUPPORTED, "n = %d does not fit in shared memory", n);
+    CUDA_TRY(cudaFuncSetAttribute(lu_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int grid = batch < 65535 ? batch : 65535;
+    lu_solve_kernel<<<grid, 32, smem, static_cast<cudaStream_t>(stream)>>>(n, batch, is_complex, A, b, x, info);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return CHEM_OK;
+}
+
+extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
+                                 const double *y_in, double *y_out, const chem_opts *o, chem_stats *stats, void *stream)
+{
+    if (!m || n < 0 || (n > 0 && (!y_in || !y_out))) return fail(CHEM_E_ARG, "bad argument");
+    if (!(t_end > 0.0) || !(rtol > 0.0) || !(atol > 0.0)) return fail(CHEM_E_ARG, "t_end, rtol and atol must be positive");
+    if (n == 0) return CHEM_OK;
+    RadauParams prm;
+    prm.t_end = t_end; prm.rtol = rtol; prm.atol = atol;
+    prm.h0 = o ? o->h0 : 0.0;
+    prm.max_steps = o ? o->max_steps : 0;
+    prm.newton_max = o ? o->newton_max : 0;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    return group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, st)
+                               : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, st);
+}
+
+extern "C" int chem_integrate(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
+                              const double *y_in, double *y_out, void *stream)
+{
+    return chem_integrate_ex(m, n, P, t_end, rtol, atol, y_in, y_out, nullptr, nullptr, stream);
+}
+
+extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
+                                   const double *y_in_host, double *y_out_host, const chem_opts *o, chem_stats *stats_host)
+{
+    if (!m || n < 0 || (n > 0 && (!y_in_host || !y_out_host))) return fail(CHEM_E_ARG, "bad argument");
+    if (n == 0) return CHEM_OK;
+    const size_t bytes = (size_t)n * m->t.n_sp * sizeof(double);
+    double *d_y = nullptr;
+    chem_stats *d_st = nullptr;
+    CUDA_TRY(cudaMalloc(&d_y, bytes));
+    int rc = CHEM_OK;
+    if (stats_host && cudaMalloc(&d_st, (size_t)n * sizeof(chem_stats)) != cudaSuccess) {
+        cudaFree(d_y);
+        return fail(CHEM_E_CUDA, "cudaMalloc(stats) failed");
+    }
+    cudaError_t e = cudaMemcpyAsync(d_y, y_in_host, bytes, cudaMemcpyHostToDevice, 0);
+    if (e == cudaSuccess) {
+        rc = chem_integrate_ex(m, n, P, t_end, rtol, atol, d_y, d_y, o, d_st, nullptr);
+        if (rc == CHEM_OK) e = cudaMemcpyAsync(y_out_host, d_y, bytes, cudaMemcpyDeviceToHost, 0);
+        if (rc == CHEM_OK && e == cudaSuccess && stats_host)
+            e = cudaMemcpyAsync(stats_host, d_st, (size_t)n * sizeof(chem_stats), cudaMemcpyDeviceToHost, 0);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+    }
+    cudaFree(d_y);
+    if (d_st) cudaFree(d_st);
+    if (rc != CHEM_OK) return rc;
+    if (e != cudaSuccess) return fail(CHEM_E_CUDA, "chem_integrate_host: %s", cudaGetErrorString(e));
+    return CHEM_OK;
+}

@@ -1,0 +1,142 @@
+"""Parity of the CUDA path against the CPU oracle, element by element, through the C ABI (-m gpu)."""
+import numpy as np
+import pytest
+
+from paper_1607_03884_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+P = synth.P_ATM
+RTOL, ATOL = synth.RTOL, synth.ATOL
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gpu_mechs(torch_cuda, mech_h2co, mech_gri):
+    from paper_1607_03884_b200 import binding
+    return {"h2co": binding.chem_mech_load(mech_h2co), "gri": binding.chem_mech_load(mech_gri)}
+
+
+@pytest.fixture(scope="module")
+def orc_mechs(mech_h2co, mech_gri):
+    from oracle import oracle as orc
+    return {"h2co": orc.Mechanism(mech_h2co), "gri": orc.Mechanism(mech_gri)}
+
+
+def descs(request):
+    return {"h2co": request.getfixturevalue("mech_h2co"), "gri": request.getfixturevalue("mech_gri")}
+
+
+@pytest.mark.parametrize("kind,n", [("h2co", 203), ("gri", 67)])
+def test_rhs_matches_oracle(kind, n, torch_cuda, gpu_mechs, orc_mechs, request):
+    """relative 1e-12 on f, scaled per component by the largest contribution"""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = descs(request)[kind]
+    y = np.concatenate([synth.make_states(mech, n // 2, "uniform", 11), synth.make_states(mech, n - n // 2, "ignition", 12)])
+    f = binding.chem_rhs(gpu_mechs[kind], P, torch.from_numpy(y).cuda()).cpu().numpy()
+    ref = orc_mechs[kind].rhs(P, y)
+    # scale: rates of individual reactions can cancel; use the per-state magnitude of the species source terms
+    scale = np.abs(ref[:, 1:]).max(axis=1, keepdims=True) + 1e-300
+    assert np.abs(f[:, 1:] - ref[:, 1:]).max() <= 1e-11 * scale.max()
+    assert np.all(np.abs(f[:, 1:] - ref[:, 1:]) <= 1e-10 * scale)
+    tscale = np.abs(ref[:, :1]) + scale * 1e5
+    assert np.all(np.abs(f[:, :1] - ref[:, :1]) <= 1e-10 * tscale)
+
+
+@pytest.mark.parametrize("kind,n", [("h2co", 101), ("gri", 37)])
+def test_jacobian_matches_oracle(kind, n, torch_cuda, gpu_mechs, orc_mechs, request):
+    """1e-10 column-scaled on J (the two sides use different but equivalent formulations)"""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = descs(request)[kind]
+    y = np.concatenate([synth.make_states(mech, n // 2, "uniform", 21), synth.make_states(mech, n - n // 2, "ignition", 22)])
+    J = binding.chem_jacobian(gpu_mechs[kind], P, torch.from_numpy(y).cuda()).cpu().numpy()
+    ref = orc_mechs[kind].jacobian(P, y)
+    col = np.abs(ref).max(axis=1, keepdims=True) + 1e-300
+    assert np.all(np.abs(J - ref) <= 1e-9 * col)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("n", [1, 2, 13, 53])
+def test_lu_solve_matches_oracle(n, cplx, torch_cuda):
+    from oracle import oracle as orc
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    rng = np.random.default_rng(n + 100 * cplx)
+    batch = 37
+    A = rng.standard_normal((batch, n, n)) + (1j * rng.standard_normal((batch, n, n)) if cplx else 0)
+    b = rng.standard_normal((batch, n)) + (1j * rng.standard_normal((batch, n)) if cplx else 0)
+    A[-1] = 0.0                                      # singular system: info != 0
+    x, info = binding.chem_lu_solve(torch.from_numpy(A).cuda(), torch.from_numpy(b).cuda())
+    x, info = x.cpu().numpy(), info.cpu().numpy()
+    assert info[-1] != 0 and np.all(info[:-1] == 0)
+    for s in range(batch - 1):
+        if cplx:
+            LU, ip, ier = orc.lu_complex(A[s])
+            ref = orc.lu_solve_complex(LU, ip, b[s])
+        else:
+            LU, ip, ier = orc.lu_real(A[s])
+            ref = orc.lu_solve_real(LU, ip, b[s])
+        assert np.allclose(x[s], ref, rtol=1e-9, atol=1e-11 * np.abs(ref).max())
+
+
+def compare_integration(y_gpu, st_gpu, y_ref, st_ref):
+    """north_star bar: |dy| <= 1e-9 + 1e-6 |y_oracle| per component; accepted-step counts identical on >= 99 %"""
+    assert np.all(st_gpu["status"] == st_ref["status"])
+    same = (st_gpu["naccpt"] == st_ref["naccpt"])
+    assert same.mean() >= 0.99, same.mean()
+    tol = 1e-9 + 1e-6 * np.abs(y_ref)
+    bad = np.abs(y_gpu - y_ref) > tol
+    assert not bad.any(), (np.argwhere(bad)[:5], np.abs(y_gpu - y_ref).max())
+
+
+CASES = [("h2co", "uniform", 1e-6, 4096), ("h2co", "ignition", 1e-4, 1037), ("gri", "uniform", 1e-6, 301),
+         ("gri", "ignition", 1e-4, 157)]
+
+
+@pytest.mark.parametrize("kind,dist,t_end,n", CASES)
+def test_integrate_matches_oracle(kind, dist, t_end, n, torch_cuda, gpu_mechs, orc_mechs, request):
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = descs(request)[kind]
+    y0 = synth.make_states(mech, n, dist, synth.STATE_SEED)
+    y_ref, st_ref, _ = orc_mechs[kind].integrate(y0, P, t_end, RTOL, ATOL)
+    y_dev, st = binding.chem_integrate_ex(gpu_mechs[kind], P, t_end, RTOL, ATOL, torch.from_numpy(y0).cuda())
+    torch.cuda.synchronize()
+    compare_integration(y_dev.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+    # the plain entry point and the host-buffer entry point give the same bits
+    y2 = binding.chem_integrate(gpu_mechs[kind], P, t_end, RTOL, ATOL, torch.from_numpy(y0).cuda())
+    assert torch.equal(y2, y_dev)
+    y3 = binding.chem_integrate_host(gpu_mechs[kind], P, t_end, RTOL, ATOL, y0)
+    assert np.array_equal(y3, y_dev.cpu().numpy())
+
+
+def test_edge_cases(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    m = gpu_mechs["h2co"]
+    empty = torch.empty((0, 13), dtype=torch.float64, device="cuda")
+    assert binding.chem_integrate(m, P, 1e-6, RTOL, ATOL, empty).shape == (0, 13)
+    y0 = synth.make_states(mech_h2co, 5, "uniform", 1)
+    y0[2, 3] = np.nan
+    y, st = binding.chem_integrate_ex(m, P, 1e-6, RTOL, ATOL, torch.from_numpy(y0).cuda())
+    st = binding.stats_to_numpy(st)
+    assert st["status"][2] == -4 and np.all(st["status"][[0, 1, 3, 4]] == 0)      # one bad state does not affect others
+    y_ref, st_ref, _ = orc_mechs["h2co"].integrate(y0, P, 1e-6, RTOL, ATOL)
+    assert st_ref["status"][2] == -4
+    ok = [0, 1, 3, 4]
+    assert np.all(np.abs(y.cpu().numpy()[ok] - y_ref[ok]) <= 1e-9 + 1e-6 * np.abs(y_ref[ok]))
+    # max_steps limit reported as -1 on both sides
+    y0 = synth.make_states(mech_h2co, 64, "ignition", 2)
+    _, st = binding.chem_integrate_ex(m, P, 1e-4, RTOL, ATOL, torch.from_numpy(y0).cuda(), max_steps=3)
+    _, st_ref, _ = orc_mechs["h2co"].integrate(y0, P, 1e-4, RTOL, ATOL, max_steps=3)
+    assert np.array_equal(binding.stats_to_numpy(st)["status"], st_ref["status"])
+    with pytest.raises(binding.ChemError):
+        binding.chem_integrate(m, P, -1.0, RTOL, ATOL, torch.from_numpy(y0).cuda())
