@@ -1,0 +1,238 @@
+#!/usr/bin/env python
+"""bench.py -- states integrated per second over one global step (BASELINE.json metric).
+
+`python bench.py --gpus N --steps K --warmup W` : one "step" = one pass of the whole hot path
+(chem_integrate over the config's batch of synthetic states).  N = 1 workload: BASELINE.json
+configs[1] (h2co-shaped 13 species / 27 reactions, 1,048,576 states, dt = 1e-6 s).  N > 1: every rank
+integrates its own batch of that size (weak scaling, no collective on the data path).
+`--impl reference` times the CPU oracle as it stands on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1607_03884_b200 import shard, synth  # noqa: E402
+
+METRIC = "states integrated/sec per global step (fp64)"
+UNIT = "states/s"
+# ALU roofline: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# dram bytes per launch of integrate_kernel from the committed ncu --set full capture (profiles/), or None
+NCU_TRAFFIC_BYTES = {1: None}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 7 and r[3 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def algorithmic_flops(stats, fm):
+    """DESIGN.md flop model: per-state counters x per-operation algorithmic flops."""
+    s = {k: float(stats[k].astype(np.float64).sum()) for k in ("nfcn", "njac", "ndec", "nsol", "nstep")}
+    return s["nfcn"] * fm["rhs"] + s["njac"] * fm["jac"] + s["ndec"] * fm["lu"] + s["nsol"] * fm["newton"] + s["nstep"] * fm["err"]
+
+
+def cpu_baseline(mech, cfg, y0, seconds_target=12.0):
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    from oracle import oracle as orc
+    M = orc.Mechanism(mech)
+    probe = min(4096, y0.shape[0])
+    t0 = time.perf_counter()
+    _, _, cores = M.integrate(y0[:probe], synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL)
+    rate = probe / max(time.perf_counter() - t0, 1e-6)
+    n = int(min(y0.shape[0], max(probe, rate * seconds_target)))
+    t0 = time.perf_counter()
+    M.integrate(y0[:n], synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL)
+    dt = time.perf_counter() - t0
+    return {"value": n / dt, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": f"first {n} states of the {y0.shape[0]}-state batch, one global step, {dt:.2f} s"}
+
+
+def run_reference(args, cfg, mech):
+    """--impl reference: the CPU oracle, bounded sample per step, rank 0 only."""
+    rank, _, world = shard.env_world()
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    M = orc.Mechanism(mech)
+    n = min(cfg["n_states"], 65536)
+    y0 = synth.make_states(mech, n, cfg["dist"], synth.STATE_SEED)
+    cores = 0
+    for _ in range(args.warmup):
+        _, _, cores = M.integrate(y0[: max(n // 16, 1)], synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, _, cores = M.integrate(y0, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = f"first {n} states of the {cfg['n_states']}-state batch per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "states_per_step": n, "t_end": cfg["t_end"], "rtol": synth.RTOL, "atol": synth.ATOL},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(cores), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic shared-memory kernel, 2 warp kernel")
+    args = ap.parse_args()
+    cfg = synth.CONFIGS[args.config]
+    mech = synth.make_mechanism(cfg["kind"], synth.MECH_SEED)
+    if args.impl == "reference":
+        run_reference(args, cfg, mech)
+        return
+
+    import torch
+    from paper_1607_03884_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    rank, local_rank, world = shard.env_world()
+    torch.cuda.set_device(local_rank)
+    shard.init_process_group("nccl")
+    warmup = max(args.warmup, 3)
+
+    n = cfg["n_states"]                          # per rank (weak scaling)
+    y0 = synth.make_states(mech, n, cfg["dist"], synth.STATE_SEED + rank)
+    gm = binding.chem_mech_load(mech)
+    N = gm.n_species
+    y_dev = torch.from_numpy(y0).cuda()
+    y_out = torch.empty_like(y_dev)
+    y_pin = torch.from_numpy(y0).pin_memory()
+    y_out_pin = torch.empty_like(y_pin)
+    if args.kernel == 0:
+        run = lambda: binding.chem_integrate(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out)
+    else:
+        run = lambda: binding.chem_integrate_ex(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out,
+                                                want_stats=False, kernel=args.kernel)
+
+    # per-state counters for the flop model (outside the timed region)
+    _, st = binding.chem_integrate_ex(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out)
+    torch.cuda.synchronize()
+    stats = binding.stats_to_numpy(st)
+    failed = int((stats["status"] != 0).sum())
+    flops_per_launch = algorithmic_flops(stats, gm.flop_model())
+
+    for _ in range(warmup):
+        run()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    shard.barrier()
+    torch.cuda.synchronize()
+    l0 = binding.chem_launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record()
+    for i in range(args.steps):
+        run()
+        ev[i + 1].record()
+    torch.cuda.synchronize()
+    shard.barrier()
+    launches = binding.chem_launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    step_ms = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)])
+    total_s = float(ev[0].elapsed_time(ev[-1])) * 1e-3
+    total_s, units = shard.reduce_max_sum(total_s, float(n * args.steps), device="cuda")
+
+    # end to end through the C ABI with HOST (pinned) buffers: H2D + kernel + D2H inside the call
+    e2e_steps = max(3, min(args.steps, 5))
+    binding.chem_integrate_host(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_pin.numpy(), y_out_pin.numpy())
+    shard.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        binding.chem_integrate_host(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_pin.numpy(), y_out_pin.numpy())
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_s, e2e_units = shard.reduce_max_sum(e2e_s, float(n * e2e_steps), device="cuda")
+    assert np.array_equal(y_out_pin.numpy(), y_out.cpu().numpy()), "host-buffer path disagrees with device path"
+
+    if rank != 0:
+        return
+    peaks, which = load_peaks()
+    kernel_s = float(step_ms.mean()) * 1e-3
+    achieved = flops_per_launch / kernel_s / 1e12
+    out = {
+        "metric": METRIC, "value": units / total_s, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
+        "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "mechanism": f"{cfg['kind']}-shaped synthetic, {N} species / {gm.n_reactions} reactions",
+                   "states_per_gpu": n, "t_end": cfg["t_end"], "rtol": synth.RTOL, "atol": synth.ATOL, "P": synth.P_ATM,
+                   "parallelism": f"batch sharded over {world} GPU(s), no collective",
+                   "l2": f"inputs+outputs {2 * n * N * 8 / 1e6:.0f} MB per step exceed the 126 MB L2 (no flush)",
+                   "failed_states": failed, "us_per_state": 1e6 * total_s / units * world},
+        "clocks": clocks,
+        "e2e": {"value": e2e_units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": n * N * 8, "d2h_bytes_per_step": n * N * 8,
+                "steps": e2e_steps, "host_memory": "pinned"},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
+                     "kernel": "integrate_kernel", "kernel_ms": 1e3 * kernel_s, "flops_per_launch": flops_per_launch,
+                     "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
+                     "hbm_frac": (2 * n * N * 8 / kernel_s / 1e9) / peaks["hbm_gbs"], "hbm_peak_source": which},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(mech, cfg, y0)
+    print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

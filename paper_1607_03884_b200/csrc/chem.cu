@@ -12,7 +12,7 @@
 #include <string>
 #include <vector>
 
-#include "chem_radau.cuh"
+#include "chem_radau_warp.cuh"
 
 using namespace chem;
 
@@ -47,7 +47,11 @@ struct chem_mech {
     int max_smem_optin = 0;
     // algorithmic flop model
     double flops[5] = {0, 0, 0, 0, 0};
+    FastTables fast{};          // register-resident warp path (chem_warp.cuh), if eligible
+    void *fast_blob = nullptr;
 };
+
+#include "chem_fast.inl"
 
 // ------------------------------------------------------------------------------------------------
 // Mechanism compiler: validate the description and pack it into coefficient-major / slot-major tables.
@@ -206,6 +210,8 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     m->flops[2] = (2.0 / 3.0) * N * N * N * 5.0 + 3.0 * N * N;                           // real LU + complex LU (4x) + forming E1, E2
     m->flops[3] = 2.0 * N * N * 5.0 + N * (15.0 + 9.0 + 15.0 + 9.0 + 3.0);               // real + complex solves, transforms, norm
     m->flops[4] = 2.0 * N * N + N * 10.0;                                                // error estimate: one real solve + norm
+    const int rcf = build_fast(d, m);
+    if (rcf != CHEM_OK) { chem_mech_free(m); return rcf; }
     *out = m;
     return CHEM_OK;
 }
@@ -215,6 +221,7 @@ extern "C" void chem_mech_free(chem_mech *m)
     if (!m) return;
     if (m->dev_blob) cudaFree(m->dev_blob);
     if (m->counter) cudaFree(m->counter);
+    if (m->fast_blob) cudaFree(m->fast_blob);
     delete m;
 }
 

@@ -228,7 +228,7 @@ __device__ __forceinline__ double reaction(const Tables &t, int i, double T, dou
 
 // Source term f(T, Y; P) of one state (R1): f[0] = dT/dt, f[k+1] = dY_k/dt.  ys, f: shared, length N.
 template <int G>
-__device__ __forceinline__ void rhs(const Tables &t, const ChemScratch &s, double P, const double *ys, double *f)
+__device__ __noinline__ void rhs(const Tables &t, const ChemScratch &s, double P, const double *ys, double *f)
 {
     const int N = t.n_sp, NR = t.n_rx;
     const int lane = Grp<G>::lane();
@@ -257,7 +257,7 @@ __device__ __forceinline__ void rhs(const Tables &t, const ChemScratch &s, doubl
 // Uses that at constant (T, P) the total concentration is independent of Y, so the unit part of the
 // third-body efficiencies only enters d/dT.
 template <int G>
-__device__ __forceinline__ void jacobian(const Tables &t, const ChemScratch &s, double P, const double *ys, double *Jm)
+__device__ __noinline__ void jacobian(const Tables &t, const ChemScratch &s, double P, const double *ys, double *Jm)
 {
     const int N = t.n_sp, NR = t.n_rx;
     const int lane = Grp<G>::lane();
@@ -334,7 +334,7 @@ __device__ __forceinline__ void jacobian(const Tables &t, const ChemScratch &s, 
 // (LAPACK convention), first maximum wins ties.  Returns 0 or k+1 (zero / non-finite pivot column).
 // "specialized implementations of ... LU factorization of the Jacobian".
 template <int G>
-__device__ __forceinline__ int lu_real(int N, double *A, int *ip)
+__device__ __noinline__ int lu_real(int N, double *A, int *ip)
 {
     const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
     for (int k = 0; k < N; k++) {
@@ -375,7 +375,7 @@ __device__ __forceinline__ int lu_real(int N, double *A, int *ip)
 
 // Complex version on split planes (Ar, Ai); pivot magnitude |re| + |im| (R10).
 template <int G>
-__device__ __forceinline__ int lu_complex(int N, double *Ar, double *Ai, int *ip)
+__device__ __noinline__ int lu_complex(int N, double *Ar, double *Ai, int *ip)
 {
     const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
     for (int k = 0; k < N; k++) {
@@ -493,7 +493,7 @@ __device__ __forceinline__ void solve_complex_warp(int N, const double *Ar, cons
 // One real and one complex solve for the group: a single warp does both when G == 32, warps 0 and 1
 // work side by side when the group is a CTA.
 template <int G>
-__device__ __forceinline__ void solve_pair(int N, const double *E1, const int *ip1, double *z1, const double *E2r,
+__device__ __noinline__ void solve_pair(int N, const double *E1, const int *ip1, double *z1, const double *E2r,
                                            const double *E2i, const int *ip2, double *z2, double *z3)
 {
     if (G == 32) {
@@ -506,7 +506,7 @@ __device__ __forceinline__ void solve_pair(int N, const double *E1, const int *i
     Grp<G>::sync();
 }
 template <int G>
-__device__ __forceinline__ void solve_real(int N, const double *E1, const int *ip1, double *b)
+__device__ __noinline__ void solve_real(int N, const double *E1, const int *ip1, double *b)
 {
     if (Grp<G>::warp() == 0) solve_real_warp(N, E1, ip1, b, Grp<G>::wlane());
     Grp<G>::sync();

@@ -61,6 +61,40 @@ __global__ void __launch_bounds__(kBlock) integrate_kernel(Tables t, int n_state
     }
 }
 
+// Compact warp-per-state integrator (chem_warp.cuh / chem_radau_warp.cuh): 8 warps per CTA.
+constexpr int kWarpBlock = 256;
+
+__global__ void __launch_bounds__(kWarpBlock) integrate_warp_kernel(Tables t, FastTables ft, int n_states, double P,
+                                                                    const double *P_per_state, RadauParams prm,
+                                                                    const double *__restrict__ y_in, double *__restrict__ y_out,
+                                                                    chem_stats *stats, int *counter)
+{
+    extern __shared__ double smem[];
+    for (int i = threadIdx.x; i < ft.blob_doubles; i += kWarpBlock) smem[i] = ft.blob[i];   // stage the tables once per CTA
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int N = t.n_sp;
+    double *ws = smem + ft.blob_doubles + (size_t)wib * warp_ws_doubles(N, t.n_rx);
+    for (;;) {
+        int q = 0;
+        if (lane == 0) q = atomicAdd(counter, 1);
+        q = __shfl_sync(0xffffffffu, q, 0);
+        if (q >= n_states) break;
+        double y = lane < N ? y_in[(size_t)q * N + lane] : 0.0;
+        RadauResult r;
+        radau_state_warp(t, smem, ws, ft.tmid, P_per_state ? P_per_state[q] : P, prm, y, r);
+        if (lane < N) y_out[(size_t)q * N + lane] = y;
+        if (stats && lane == 0) {
+            chem_stats o;
+            o.status = r.status; o.nstep = r.nstep; o.naccpt = r.naccpt; o.nrejct = r.nrejct; o.nfcn = r.nfcn;
+            o.njac = r.njac; o.ndec = r.ndec; o.nsol = r.nsol; o.nnewt_fail = r.nnewt_fail; o.reserved = 0;
+            o.h_last = r.h_last;
+            stats[q] = o;
+        }
+        __syncwarp();
+    }
+}
+
 // Source term / Jacobian for a batch (static round-robin over groups).
 template <int G, bool JAC>
 __global__ void __launch_bounds__(kBlock) eval_kernel(Tables t, int n_states, double P, const double *__restrict__ y,

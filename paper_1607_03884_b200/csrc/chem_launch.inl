@@ -53,6 +53,28 @@ int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm
     return CHEM_OK;
 }
 
+int launch_integrate_warp(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
+                          const chem_opts *o, chem_stats *stats, cudaStream_t st)
+{
+    const int wpb = kWarpBlock / 32;
+    const size_t smem = ((size_t)m->fast.blob_doubles + (size_t)wpb * warp_ws_doubles(m->t.n_sp, m->t.n_rx)) * sizeof(double);
+    if (smem > (size_t)m->max_smem_optin) return fail(CHEM_E_UNSUPPORTED, "warp kernel: shared memory");
+    CUDA_TRY(cudaFuncSetAttribute(integrate_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, integrate_warp_kernel, kWarpBlock, smem));
+    if (occ < 1) return fail(CHEM_E_UNSUPPORTED, "warp kernel does not fit on an SM");
+    int grid = (n + wpb - 1) / wpb;
+    if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, warps pull states from the queue
+    CUDA_TRY(cudaMemsetAsync(m->counter, 0, sizeof(int), st));
+    integrate_warp_kernel<<<grid, kWarpBlock, smem, st>>>(m->t, m->fast, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out,
+                                                          stats, m->counter);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return CHEM_OK;
+}
+
+inline bool warp_path_available(const chem_mech *m) { return m->fast.enabled != 0; }
+
 }  // namespace
 
 extern "C" int chem_rhs(const chem_mech *m, int32_t n, double P, const double *y, double *f, void *stream)
@@ -101,6 +123,9 @@ extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double
     prm.max_steps = o ? o->max_steps : 0;
     prm.newton_max = o ? o->newton_max : 0;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int kernel = o ? o->kernel : 0;
+    if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "register-resident warp kernel not available for this mechanism");
+    if (kernel != 1 && warp_path_available(m)) return launch_integrate_warp(m, n, P, prm, y_in, y_out, o, stats, st);
     return group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, st)
                                : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, st);
 }

@@ -108,9 +108,12 @@ def test_integrate_matches_oracle(kind, dist, t_end, n, torch_cuda, gpu_mechs, o
     mech = descs(request)[kind]
     y0 = synth.make_states(mech, n, dist, synth.STATE_SEED)
     y_ref, st_ref, _ = orc_mechs[kind].integrate(y0, P, t_end, RTOL, ATOL)
-    y_dev, st = binding.chem_integrate_ex(gpu_mechs[kind], P, t_end, RTOL, ATOL, torch.from_numpy(y0).cuda())
-    torch.cuda.synchronize()
-    compare_integration(y_dev.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+    # kernel 1 = generic shared-memory groups, kernel 2 = register-resident warp path (h2co only), 0 = auto
+    for kernel in ((1, 2, 0) if kind == "h2co" else (1, 0)):
+        y_dev, st = binding.chem_integrate_ex(gpu_mechs[kind], P, t_end, RTOL, ATOL, torch.from_numpy(y0).cuda(),
+                                              kernel=kernel)
+        torch.cuda.synchronize()
+        compare_integration(y_dev.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
     # the plain entry point and the host-buffer entry point give the same bits
     y2 = binding.chem_integrate(gpu_mechs[kind], P, t_end, RTOL, ATOL, torch.from_numpy(y0).cuda())
     assert torch.equal(y2, y_dev)
