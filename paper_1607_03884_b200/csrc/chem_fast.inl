@@ -6,7 +6,8 @@
 //   kr_i      : ln kf - ln Kc,  ln Kc = dnu ln(P_atm/(R T)) - sum_k nu_ki (h_k/RT - s_k/R)   (NASA-7 folded in)
 //   k0/kinf   : (ln A0 - ln A) + (b0 - b) ln T - (Ta0 - Ta)/T
 //   Troe      : (1-alpha) exp(-T/T***), alpha exp(-T/T*), exp(-T**/T)
-// Eligibility: N_sp <= 16, N_rx <= 32, one common NASA switch temperature, 0 < alpha < 1, and the extra jobs
+// and every rate-of-progress product becomes three concentration factors per side (index 31 = unity).
+// Eligibility: N_sp <= 16, N_rx <= 32, molecularity <= 3 per side, one common NASA switch temperature, 0 < alpha < 1, and the extra jobs
 // (falloff, Troe) fit in the lanes the reactions leave free in two rounds of 32.
 
 namespace {
@@ -60,15 +61,18 @@ int build_fast(const chem_mech_desc *d, chem_mech *m)
         const double lnA = std::log(d->arr_A[i]), b = d->arr_b[i], Ta = d->arr_Ea[i] / kRcal;
         type[i] = d->rxn_type[i];
         double dnu = 0.0;
-        int sl = 0;
+        // concentration factors with multiplicity, three per side, index 31 = unity
         for (int side = 0; side < 2; side++) {
             const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr, *spi = side ? d->prod_sp : d->reac_sp, *nu = side ? d->prod_nu : d->reac_nu;
-            sl = side * 3;
-            for (int p = ptr[i]; p < ptr[i + 1]; p++, sl++) {
-                slots[i] |= spi[p] << (5 * sl);
-                nus[i] |= nu[p] << (2 * sl);
+            int sl = side * 3;
+            for (int p = ptr[i]; p < ptr[i + 1]; p++) {
                 dnu += side ? nu[p] : -nu[p];
+                for (int rep = 0; rep < nu[p]; rep++, sl++) {
+                    if (sl >= side * 3 + 3) return CHEM_OK;          // molecularity above 3: not eligible
+                    slots[i] |= spi[p] << (5 * sl);
+                }
             }
+            for (; sl < side * 3 + 3; sl++) slots[i] |= 31 << (5 * sl);
         }
         for (int r = 0; r < 2; r++) {
             double *kf = &job[r][i * kJobW], *kr = &job[r][(32 + i) * kJobW];

@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(kBlock) integrate_kernel(Tables t, int n_state
 // Compact warp-per-state integrator (chem_warp.cuh / chem_radau_warp.cuh): 8 warps per CTA.
 constexpr int kWarpBlock = 256;
 
-__global__ void __launch_bounds__(kWarpBlock) integrate_warp_kernel(Tables t, FastTables ft, int n_states, double P,
+__global__ void __launch_bounds__(kWarpBlock, 2) integrate_warp_kernel(Tables t, FastTables ft, int n_states, double P,
                                                                     const double *P_per_state, RadauParams prm,
                                                                     const double *__restrict__ y_in, double *__restrict__ y_out,
                                                                     chem_stats *stats, int *counter)
@@ -75,6 +75,8 @@ __global__ void __launch_bounds__(kWarpBlock) integrate_warp_kernel(Tables t, Fa
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int N = t.n_sp;
     double *ws = smem + ft.blob_doubles + (size_t)wib * warp_ws_doubles(N, t.n_rx);
+    if (lane >= N) ws[kWsC + lane] = 1.0;   // C[31] = 1: the unity factor of the rate products
+    __syncwarp();
     for (;;) {
         int q = 0;
         if (lane == 0) q = atomicAdd(counter, 1);

@@ -55,6 +55,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     const WarpMats M = warp_mats(ws, N, t.n_rx);
     const int LD = M.LD;
     const bool mine = lane < N;
+    const double invP = 1.0 / P;
 
     st.status = 0; st.nstep = 0; st.naccpt = 0; st.nrejct = 0; st.nfcn = 0; st.njac = 0; st.ndec = 0; st.nsol = 0;
     st.nnewt_fail = 0; st.h_last = 0.0;
@@ -68,8 +69,8 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     if (X + H * 1.0001 - XEND >= 0.0) { H = XEND - X; LAST = true; }
     double FACCON = 1.0, THETA = 0.0, HACC = 0.0, ERRACC = 0.0;
     int NSING = 0;
-    double scal = ATOL + RTOL * fabs(y);
-    double f0 = warp_rhs(tab, ws, tmid, P, y);
+    double iscal = 1.0 / (ATOL + RTOL * fabs(y));    // 1 / scal
+    double f0 = warp_rhs(tab, ws, tmid, P, invP, y);
     st.nfcn++;
     double z1 = 0, z2 = 0, z3 = 0, w1 = 0, w2 = 0, w3 = 0, c1 = 0, c2 = 0, c3 = 0;
     // LU factors
@@ -80,15 +81,14 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     int next = DO_JAC;
     for (;;) {
         if (next == DO_JAC) {
-            if (mine) ws[kWsYs + lane] = y;
-            __syncwarp();
-            jacobian<32>(t, M.cs, P, ws + kWsYs, M.Jm);
+            warp_jacobian(tab, ws, tmid, P, invP, y, M.Jm, M.E2r, M.cs.g);
             st.njac++;
             CALJAC = true;
             next = DO_FACT;
         }
         if (next == DO_FACT) {
-            const double FAC1 = U1 / H, ALPHN = ALPH / H, BETAN = BETA / H;
+            const double invH = 1.0 / H;
+            const double FAC1 = U1 * invH, ALPHN = ALPH * invH, BETAN = BETA * invH;
             bool nonfinite = false;
             if (mine)
                 for (int j = 0; j < N; j++) {
@@ -116,7 +116,8 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         st.nstep++;
         if (st.nstep > NMAX) { st.status = -1; return; }
         if (0.1 * fabs(H) <= fmax(fabs(X), XEND) * UROUND) { st.status = -2; return; }
-        const double FAC1 = U1 / H, ALPHN = ALPH / H, BETAN = BETA / H;
+        const double invH = 1.0 / H;
+        const double FAC1 = U1 * invH, ALPHN = ALPH * invH, BETAN = BETA * invH;
         if (FIRST) {
             z1 = z2 = z3 = 0.0; w1 = w2 = w3 = 0.0;
         } else {
@@ -135,9 +136,9 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         int outcome = 0;
         for (;;) {
             if (NEWT >= NIT) { outcome = 2; break; }
-            const double a1 = warp_rhs(tab, ws, tmid, P, y + z1);
-            const double a2 = warp_rhs(tab, ws, tmid, P, y + z2);
-            const double a3 = warp_rhs(tab, ws, tmid, P, y + z3);
+            const double a1 = warp_rhs(tab, ws, tmid, P, invP, y + z1);
+            const double a2 = warp_rhs(tab, ws, tmid, P, invP, y + z2);
+            const double a3 = warp_rhs(tab, ws, tmid, P, invP, y + z3);
             st.nfcn += 3;
             z1 = TI11 * a1 + TI12 * a2 + TI13 * a3 - w1 * FAC1;
             z2 = TI21 * a1 + TI22 * a2 + TI23 * a3 - w2 * ALPHN + w3 * BETAN;
@@ -151,7 +152,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             NEWT++;
             double dy = 0.0;
             if (mine) {
-                const double d = 1.0 / scal;
+                const double d = iscal;
                 const double q1 = z1 * d, q2 = z2 * d, q3 = z3 * d;
                 dy = q1 * q1 + q2 * q2 + q3 * q3;
             }
@@ -193,17 +194,17 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         // error estimate
         double ERR;
         {
-            const double f2 = (DD1 / H) * z1 + (DD2 / H) * z2 + (DD3 / H) * z3;
+            const double f2 = (DD1 * z1 + DD2 * z2 + DD3 * z3) * invH;
             double cont = solve_warp_real(M.E1, LD, N, M.perm1, myk1, rd1, f2 + f0);
             double e = 0.0;
-            if (mine) { const double q = cont / scal; e = q * q; }
+            if (mine) { const double q = cont * iscal; e = q * q; }
             ERR = fmax(sqrt(warp_sum(e) / N), 1.0e-10);
             if (ERR >= 1.0 && (FIRST || REJECT)) {
-                const double fr = warp_rhs(tab, ws, tmid, P, y + cont);
+                const double fr = warp_rhs(tab, ws, tmid, P, invP, y + cont);
                 st.nfcn++;
                 cont = solve_warp_real(M.E1, LD, N, M.perm1, myk1, rd1, fr + f2);
                 e = 0.0;
-                if (mine) { const double q = cont / scal; e = q * q; }
+                if (mine) { const double q = cont * iscal; e = q * q; }
                 ERR = fmax(sqrt(warp_sum(e) / N), 1.0e-10);
             }
         }
@@ -237,10 +238,10 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
                 const double k2 = (AK - k1) / C1M1;
                 c1 = k1; c2 = k2; c3 = k2 - ACONT3;
             }
-            scal = ATOL + RTOL * fabs(y);
+            iscal = 1.0 / (ATOL + RTOL * fabs(y));
             CALJAC = false;
             if (LAST) return;
-            f0 = warp_rhs(tab, ws, tmid, P, y);
+            f0 = warp_rhs(tab, ws, tmid, P, invP, y);
             st.nfcn++;
             HNEW = fmin(fabs(HNEW), XEND);
             if (REJECT) HNEW = fmin(HNEW, fabs(H));

@@ -47,79 +47,99 @@ __device__ __forceinline__ void warp_sum2(double &a, double &b)
     }
 }
 __device__ __noinline__ double pow_ni(double a, double b) { return pow(a, b); }
+__device__ __noinline__ double exp_ni(double a) { return exp(a); }
+__device__ __noinline__ double log_ni(double a) { return log(a); }
+constexpr double kLn10 = 2.302585092994045684, kInvLn10 = 0.4342944819032518277;
 
-// per-warp scratch layout (doubles): C[16] E[64] q[32] ys[16] then matrices
-constexpr int kWsC = 0, kWsE = 16, kWsQ = 16 + kJobs, kWsYs = kWsQ + 32, kWsMat = kWsYs + 16;
+// per-warp scratch layout (doubles): C[32] (C[31] = 1 for unused factor slots) E[64] q[32] ys[16] then matrices
+constexpr int kWsC = 0, kWsE = 32, kWsQ = 32 + kJobs, kWsYs = kWsQ + 32, kWsMat = kWsYs + 16;
+
+// exponent of job row c at T and its temperature derivative
+__device__ __forceinline__ double job_arg(const double *c, double T, double lnT, double invT)
+{
+    return c[0] + c[1] * lnT + c[2] * invT + T * (c[3] + T * (c[4] + T * (c[5] + T * c[6])));
+}
+__device__ __forceinline__ double job_darg(const double *c, double T, double invT)
+{
+    return (c[1] - c[2] * invT) * invT + c[3] + T * (2.0 * c[4] + T * (3.0 * c[5] + T * (4.0 * c[6])));
+}
+
+// Mixture front end shared by the source term and the Jacobian: returns T, fills C[], E[] (exp jobs).
+struct WarpMix {
+    double T, lnT, invT, rho, inv_rho, Wbar, Ck, invWk;
+    const double *spc, *jt;
+    bool lo;
+};
+__device__ __forceinline__ WarpMix warp_front(const double *tab, double *ws, double tmid, double P, double invP, double yc,
+                                              int lane, int N)
+{
+    WarpMix m;
+    double *C = ws + kWsC, *E = ws + kWsE;
+    m.T = __shfl_sync(0xffffffffu, yc, 0);
+    double Yk = __shfl_down_sync(0xffffffffu, yc, 1);     // species lane k holds Y_k = component k+1
+    if (lane >= N - 1) Yk = 0.0;
+    m.lo = (m.T <= tmid);
+    const double *spt = tab + (m.lo ? kOffSpLo : kOffSpHi);
+    m.spc = spt + (lane < N ? lane : 0) * kJobW;
+    m.invWk = m.spc[7];
+    double sY = Yk, sYW = Yk * m.invWk;
+    warp_sum2(sY, sYW);
+    const double YN = 1.0 - sY;                            // closure: last species
+    if (lane == N - 1) Yk = YN;
+    const double sW = sYW + YN * spt[(N - 1) * kJobW + 7]; // 1 / Wbar
+    m.Wbar = __drcp_rn(sW);
+    m.invT = __drcp_rn(m.T);
+    m.rho = P * m.Wbar * m.invT * (1.0 / kRerg);
+    m.inv_rho = kRerg * m.T * sW * invP;
+    m.lnT = log_ni(m.T);
+    m.Ck = m.rho * Yk * m.invWk;
+    if (lane < N) C[lane] = m.Ck;
+    m.jt = tab + (m.lo ? kOffJobLo : kOffJobHi);
+#pragma unroll 1
+    for (int r = 0; r < 2; r++)
+        E[32 * r + lane] = exp_ni(job_arg(m.jt + (32 * r + lane) * kJobW, m.T, m.lnT, m.invT));
+    __syncwarp();
+    return m;
+}
 
 // Source term for the state whose component `lane` is yc (lane 0: T, lanes 1..N-1: Y_1..Y_{N-1}).
 // Returns component `lane` of f.  DESIGN.md R1-R5; same mathematics as rhs<G>() in chem_device.cuh.
 // tab = staged table blob (shared), ws = this warp's scratch (shared).
-__device__ __noinline__ double warp_rhs(const double *tab, double *ws, double tmid, double P, double yc)
+__device__ __noinline__ double warp_rhs(const double *tab, double *ws, double tmid, double P, double invP, double yc)
 {
     const int lane = threadIdx.x & 31;
     const int *hdr = reinterpret_cast<const int *>(tab);
     const int N = hdr[0];
-    const int4 d0 = reinterpret_cast<const int4 *>(tab + kOffDesc)[2 * lane];       // slots, nus, type, jobs
+    const int4 d0 = reinterpret_cast<const int4 *>(tab + kOffDesc)[2 * lane];       // factors, -, type, jobs
     const int4 d1 = reinterpret_cast<const int4 *>(tab + kOffDesc)[2 * lane + 1];   // eff_lo, eff_hi, inc_lo, inc_hi
     double *C = ws + kWsC, *E = ws + kWsE, *q = ws + kWsQ;
-    const double T = __shfl_sync(0xffffffffu, yc, 0);
-    double Yk = __shfl_down_sync(0xffffffffu, yc, 1);     // species lane k holds Y_k = component k+1
-    if (lane >= N - 1) Yk = 0.0;
-    const bool lo = (T <= tmid);
-    const double *spt = tab + (lo ? kOffSpLo : kOffSpHi);
-    const double *spc = spt + (lane < N ? lane : 0) * kJobW;
-    const double invWk = spc[7];
-    double sY = Yk, sYW = Yk * invWk;
-    warp_sum2(sY, sYW);
-    const double YN = 1.0 - sY;                            // closure: last species
-    if (lane == N - 1) Yk = YN;
-    const double Wbar = 1.0 / (sYW + YN * spt[(N - 1) * kJobW + 7]);
-    const double rho = P * Wbar / (kRerg * T);
-    const double lnT = log(T), invT = 1.0 / T;
-    const double Ck = rho * Yk * invWk;
-    if (lane < N) C[lane] = Ck;
-    // two exp jobs per lane
-    const double *jt = tab + (lo ? kOffJobLo : kOffJobHi);
-    double Ej[2];
-#pragma unroll 1
-    for (int r = 0; r < 2; r++) {
-        const double *c = jt + (32 * r + lane) * kJobW;
-        Ej[r] = exp(c[0] + c[1] * lnT + c[2] * invT + T * (c[3] + T * (c[4] + T * (c[5] + T * c[6]))));
-        E[32 * r + lane] = Ej[r];
-    }
-    __syncwarp();
-    // rate of progress of reaction `lane`
+    const WarpMix m = warp_front(tab, ws, tmid, P, invP, yc, lane, N);
+    const double T = m.T;
+    // rate of progress of reaction `lane`: factors are species indices with multiplicity, 31 = unity
     double qi = 0.0;
     const int type = d0.z;
     if (type >= 0) {
-        double Rf = E[lane], Rr = E[32 + lane];
-#pragma unroll
-        for (int sl = 0; sl < 6; sl++) {
-            const int sp = (d0.x >> (5 * sl)) & 31, nu = (d0.y >> (2 * sl)) & 3;
-            const double pw = powi(C[sp], nu);
-            if (sl < 3) Rf *= pw; else Rr *= pw;
-        }
+        const double Rf = E[lane] * (C[d0.x & 31] * C[(d0.x >> 5) & 31] * C[(d0.x >> 10) & 31]);
+        const double Rr = E[32 + lane] * (C[(d0.x >> 15) & 31] * C[(d0.x >> 20) & 31] * C[(d0.x >> 25) & 31]);
         double c = 1.0;
         if (type != 0) {
             const double *eff_dv = tab + hdr[4];
             const int *eff_sp = reinterpret_cast<const int *>(tab + hdr[5]);
-            double M = P / (kRerg * T);
+            double M = P * m.invT * (1.0 / kRerg);
+#pragma unroll 1
             for (int p = d1.x; p < d1.y; p++) M += eff_dv[p] * C[eff_sp[p]];
-            if (type == 1) {
-                c = M;
-            } else {
+            c = M;
+            if (type >= 2) {
                 const double Pr = E[d0.w & 255] * M;
                 double F = 1.0;
                 if (type == 3) {
                     const int ts = (d0.w >> 8) & 255;
-                    const double Fc = E[ts] + E[ts + 1] + E[ts + 2];
-                    const double L = log10(Fc);
-                    const double At = log10(Pr) - 0.4 - 0.67 * L;
-                    const double Bt = 0.75 - 1.27 * L - 0.14 * At;
-                    const double x = At / Bt;
-                    F = exp10(L / (1.0 + x * x));
+                    const double L = log_ni(E[ts] + E[ts + 1] + E[ts + 2]) * kInvLn10;      // log10 Fcent
+                    const double At = log_ni(Pr) * kInvLn10 - 0.4 - 0.67 * L;
+                    const double x = At * __drcp_rn(0.75 - 1.27 * L - 0.14 * At);
+                    F = exp_ni(kLn10 * L * __drcp_rn(1.0 + x * x));
                 }
-                c = Pr / (1.0 + Pr) * F;
+                c = Pr * __drcp_rn(1.0 + Pr) * F;
             }
         }
         qi = c * (Rf - Rr);
@@ -130,16 +150,161 @@ __device__ __noinline__ double warp_rhs(const double *tab, double *ws, double tm
     const double *inc_nu = tab + hdr[2];
     const int *inc_rx = reinterpret_cast<const int *>(tab + hdr[3]);
     double w = 0.0;
+#pragma unroll 1
     for (int p = d1.z; p < d1.w; p++) w += inc_nu[p] * q[inc_rx[p]];
+    const double *spc = m.spc;
     const double cpR = spc[0] + T * (spc[1] + T * (spc[2] + T * (spc[3] + T * spc[4])));
-    const double hRT = spc[0] + T * (spc[1] * 0.5 + T * (spc[2] * (1.0 / 3.0) + T * (spc[3] * 0.25 + T * (spc[4] * 0.2)))) + spc[5] * invT;
-    double hw = (lane < N) ? hRT * w : 0.0, ccp = (lane < N) ? Ck * cpR : 0.0;
+    const double hRT = spc[0] + T * (spc[1] * 0.5 + T * (spc[2] * (1.0 / 3.0) + T * (spc[3] * 0.25 + T * (spc[4] * 0.2)))) + spc[5] * m.invT;
+    double hw = (lane < N) ? hRT * w : 0.0, ccp = (lane < N) ? m.Ck * cpR : 0.0;
     warp_sum2(hw, ccp);
-    const double Ydot = spc[6] * w / rho;                 // W_k wdot_k / rho in species lane k
+    const double Ydot = spc[6] * w * m.inv_rho;           // W_k wdot_k / rho in species lane k
     double f = __shfl_up_sync(0xffffffffu, Ydot, 1);      // component k+1
-    if (lane == 0) f = -T * hw / ccp;
+    if (lane == 0) f = -T * hw * __drcp_rn(ccp);
     __syncwarp();
     return f;
+}
+
+// Analytical Jacobian (R6) for the warp path: Jm[i*N + j] = d f_i / d y_j in shared memory.
+// Temperature derivatives of all rate constants come from the exp-job rows (d/dT exp(p(T)) = p'(T) exp(p(T))).
+// scr: 8*32 doubles (dq[6][32], dqdT[32], tb[32]); vec: 3*16 doubles (wdot, hRT, cpR per species).
+__device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double tmid, double P, double invP, double yc,
+                                           double *Jm, double *scr, double *vec)
+{
+    const int lane = threadIdx.x & 31;
+    const int *hdr = reinterpret_cast<const int *>(tab);
+    const int N = hdr[0];
+    const int4 *desc = reinterpret_cast<const int4 *>(tab + kOffDesc);
+    const int4 d0 = desc[2 * lane], d1 = desc[2 * lane + 1];
+    double *C = ws + kWsC, *E = ws + kWsE, *q = ws + kWsQ;
+    double *dq = scr, *dqdT = scr + 192, *tb = scr + 224;
+    const double *eff_dv = tab + hdr[4];
+    const int *eff_sp = reinterpret_cast<const int *>(tab + hdr[5]);
+    const WarpMix m = warp_front(tab, ws, tmid, P, invP, yc, lane, N);
+    const double T = m.T, invT = m.invT;
+    const double Ctot = P * invT * (1.0 / kRerg);
+    {
+        double qi = 0.0, dT = 0.0, tbi = 0.0, d[6] = {0, 0, 0, 0, 0, 0};
+        const int type = d0.z;
+        if (type >= 0) {
+            const double c0 = C[d0.x & 31], c1 = C[(d0.x >> 5) & 31], c2 = C[(d0.x >> 10) & 31];
+            const double c3 = C[(d0.x >> 15) & 31], c4 = C[(d0.x >> 20) & 31], c5 = C[(d0.x >> 25) & 31];
+            const double kf = E[lane], kr = E[32 + lane];
+            const double Rf = kf * (c0 * c1 * c2), Rr = kr * (c3 * c4 * c5), rnet = Rf - Rr;
+            const double dlnkf = job_darg(m.jt + lane * kJobW, T, invT), dlnkr = job_darg(m.jt + (32 + lane) * kJobW, T, invT);
+            double c = 1.0, dc_dT = 0.0, dc_dM = 0.0;
+            if (type != 0) {
+                double M = Ctot;
+#pragma unroll 1
+                for (int p = d1.x; p < d1.y; p++) M += eff_dv[p] * C[eff_sp[p]];
+                c = M;
+                dc_dM = 1.0;
+                if (type >= 2) {
+                    const int ks = d0.w & 255;
+                    const double k0k = E[ks], Pr = k0k * M, dlnPr = job_darg(m.jt + ks * kJobW, T, invT);
+                    double F = 1.0, dF_dT = 0.0, dF_dPr = 0.0;
+                    if (type == 3) {
+                        const int ts = (d0.w >> 8) & 255;
+                        const double e3 = E[ts], e1 = E[ts + 1], e2 = E[ts + 2];
+                        const double Fc = e3 + e1 + e2;
+                        const double dFc = e3 * job_darg(m.jt + ts * kJobW, T, invT) + e1 * job_darg(m.jt + (ts + 1) * kJobW, T, invT) +
+                                           e2 * job_darg(m.jt + (ts + 2) * kJobW, T, invT);
+                        const double L = log_ni(Fc) * kInvLn10, dL = dFc * __drcp_rn(Fc) * kInvLn10;
+                        const double At = log_ni(Pr) * kInvLn10 - 0.4 - 0.67 * L;
+                        const double Bt = 0.75 - 1.27 * L - 0.14 * At, rB = __drcp_rn(Bt);
+                        const double x = At * rB, rden = __drcp_rn(1.0 + x * x);
+                        F = exp_ni(kLn10 * L * rden);
+                        const double dA_T = dlnPr * kInvLn10 - 0.67 * dL, dB_T = -1.27 * dL - 0.14 * dA_T;
+                        const double dx_T = (dA_T * Bt - At * dB_T) * rB * rB;
+                        const double dx_P = __drcp_rn(Pr) * kInvLn10 * (Bt + 0.14 * At) * rB * rB;
+                        const double wF = -L * 2.0 * x * rden * rden;
+                        dF_dT = F * kLn10 * (dL * rden + wF * dx_T);
+                        dF_dPr = F * kLn10 * wF * dx_P;
+                    }
+                    const double op = __drcp_rn(1.0 + Pr);
+                    c = Pr * op * F;
+                    dc_dT = Pr * dlnPr * op * op * F + Pr * op * dF_dT;
+                    dc_dM = (op * op * F + Pr * op * dF_dPr) * k0k;
+                }
+            }
+            qi = c * rnet;
+            dT = dc_dT * rnet + c * (Rf * dlnkf - Rr * dlnkr);
+            tbi = dc_dM * rnet;
+            const double ckf = c * kf, ckr = -c * kr;
+            d[0] = ckf * c1 * c2; d[1] = ckf * c0 * c2; d[2] = ckf * c0 * c1;
+            d[3] = ckr * c4 * c5; d[4] = ckr * c3 * c5; d[5] = ckr * c3 * c4;
+        }
+        q[lane] = qi; dqdT[lane] = dT; tb[lane] = (type > 0) ? tbi : 0.0;
+#pragma unroll
+        for (int sl = 0; sl < 6; sl++) dq[sl * 32 + lane] = d[sl];
+    }
+    __syncwarp();
+    // rows: species lane k -> Dw[k][j] = d wdot_k / d y_j, stored in Jm row k
+    const double *spt = tab + (m.lo ? kOffSpLo : kOffSpHi);
+    const double *spc = m.spc;
+    const double invWN = spt[(N - 1) * kJobW + 7];
+    const double cpR = spc[0] + T * (spc[1] + T * (spc[2] + T * (spc[3] + T * spc[4])));
+    const double dcpR = spc[1] + T * (2.0 * spc[2] + T * (3.0 * spc[3] + T * (4.0 * spc[4])));
+    const double hRT = spc[0] + T * (spc[1] * 0.5 + T * (spc[2] * (1.0 / 3.0) + T * (spc[3] * 0.25 + T * (spc[4] * 0.2)))) + spc[5] * invT;
+    double hw = 0.0, ccp = 0.0, cpw = 0.0, cdcp = 0.0;
+    if (lane < N) {
+        const double *inc_nu = tab + hdr[2];
+        const int *inc_rx = reinterpret_cast<const int *>(tab + hdr[3]);
+        double *row = Jm + lane * N;
+        for (int l = 0; l < N; l++) row[l] = 0.0;
+        double wd = 0.0, dwT = 0.0, u = 0.0;
+#pragma unroll 1
+        for (int p = d1.z; p < d1.w; p++) {
+            const int i = inc_rx[p];
+            const double nu = inc_nu[p];
+            const int4 e0 = desc[2 * i], e1 = desc[2 * i + 1];
+            wd += nu * q[i];
+            dwT += nu * dqdT[i];
+#pragma unroll
+            for (int sl = 0; sl < 6; sl++) {
+                const int f = (e0.x >> (5 * sl)) & 31;
+                if (f != 31) row[f] += nu * dq[sl * 32 + i];
+            }
+            const double v = nu * tb[i];
+            u += v;
+            for (int pe = e1.x; pe < e1.y; pe++) row[eff_sp[pe]] += v * eff_dv[pe];
+        }
+        double GC = 0.0;
+        for (int l = 0; l < N; l++) GC += row[l] * C[l];
+        const double GN = row[N - 1] * invWN;
+        for (int j = N - 1; j >= 1; j--) {
+            const double iw = spt[(j - 1) * kJobW + 7];
+            row[j] = -m.Wbar * (iw - invWN) * GC + m.rho * (row[j - 1] * iw - GN);
+        }
+        row[0] = dwT - (GC + u * Ctot) * invT;
+        vec[lane] = wd; vec[16 + lane] = hRT; vec[32 + lane] = cpR;
+        hw = hRT * wd; ccp = m.Ck * cpR; cpw = cpR * wd; cdcp = m.Ck * dcpR;
+    }
+    warp_sum2(hw, ccp);
+    warp_sum2(cpw, cdcp);
+    __syncwarp();
+    const double rccp = __drcp_rn(ccp);
+    const double Tdot = -T * hw * rccp;
+    // columns: assemble the rows of J in place (row k+1 <- species k, descending; row 0 <- temperature)
+    if (lane < N) {
+        const int j = lane;
+        double S = 0.0;
+        for (int k = 0; k < N; k++) S += vec[16 + k] * Jm[k * N + j];
+        double dlnrho, drcp;
+        if (j == 0) {
+            dlnrho = -invT;
+            drcp = -ccp * invT + cdcp;
+        } else {
+            const double iw = spt[(j - 1) * kJobW + 7];
+            dlnrho = -m.Wbar * (iw - invWN);
+            drcp = dlnrho * ccp + m.rho * (vec[32 + j - 1] * iw - vec[32 + N - 1] * invWN);
+        }
+        for (int k = N - 2; k >= 0; k--) {
+            const double Wr = spt[k * kJobW + 6] * m.inv_rho;
+            Jm[(k + 1) * N + j] = Wr * (Jm[k * N + j] - vec[k] * dlnrho);
+        }
+        Jm[j] = -(T * S + (j == 0 ? cpw : 0.0)) * rccp - Tdot * drcp * rccp;
+    }
+    __syncwarp();
 }
 
 // ---------------------------------------------------------------------------- LU with rows owned by lanes
@@ -177,12 +342,13 @@ __device__ __noinline__ int lu_warp_real(double *A, int LD, int N, int *perm, in
         const double *prow = A + p * LD;
         const double pvv = prow[k];
         if (!isfinite(pvv)) return k + 1;
-        const double rp = 1.0 / pvv;
+        const double rp = __drcp_rn(pvv);
         if (lane == 0) perm[k] = p;
         if (lane == p) { myk = k; rdiag = rp; }
         if (act && lane != p) {
             const double l = ak * rp;
             row[k] = l;
+#pragma unroll 2
             for (int j = k + 1; j < N; j++) row[j] = fma(-l, prow[j], row[j]);
         }
         __syncwarp();
@@ -207,7 +373,7 @@ __device__ __noinline__ int lu_warp_complex(double *Ar, double *Ai, int LD, int 
         if (p < 0) return k + 1;
         const double *pr_ = Ar + p * LD, *pi_ = Ai + p * LD;
         const double pr = pr_[k], pi = pi_[k];
-        const double den = 1.0 / (pr * pr + pi * pi);
+        const double den = __drcp_rn(pr * pr + pi * pi);
         if (!isfinite(den)) return k + 1;
         const double qr = pr * den, qi = -pi * den;       // 1 / pivot
         if (lane == 0) perm[k] = p;
@@ -216,6 +382,7 @@ __device__ __noinline__ int lu_warp_complex(double *Ar, double *Ai, int LD, int 
             const double lr = akr * qr - aki * qi, li = akr * qi + aki * qr;
             rr[k] = lr;
             ri[k] = li;
+#pragma unroll 2
             for (int j = k + 1; j < N; j++) {
                 const double ur = pr_[j], ui = pi_[j];
                 rr[j] = fma(-lr, ur, fma(li, ui, rr[j]));
@@ -235,11 +402,13 @@ __device__ __noinline__ double solve_warp_real(const double *A, int LD, int N, c
 {
     const int lane = threadIdx.x & 31;
     const double *row = A + (lane < N ? lane : 0) * LD;
+#pragma unroll 1
     for (int k = 0; k < N - 1; k++) {
         const double bk = __shfl_sync(0xffffffffu, b, perm[k]);
         if (myk > k) b = fma(-row[k], bk, b);
     }
     double x = 0.0;
+#pragma unroll 1
     for (int k = N - 1; k >= 0; k--) {
         const double xk = __shfl_sync(0xffffffffu, b * rdiag, perm[k]);
         if (myk >= 0 && myk < k) b = fma(-row[k], xk, b);
@@ -254,6 +423,7 @@ __device__ __noinline__ double2 solve_warp_complex(const double *Ar, const doubl
     const int lane = threadIdx.x & 31;
     const int off = (lane < N ? lane : 0) * LD;
     const double *rr = Ar + off, *ri = Ai + off;
+#pragma unroll 1
     for (int k = 0; k < N - 1; k++) {
         const int p = perm[k];
         const double xr = __shfl_sync(0xffffffffu, br, p), xi = __shfl_sync(0xffffffffu, bi, p);
@@ -264,6 +434,7 @@ __device__ __noinline__ double2 solve_warp_complex(const double *Ar, const doubl
         }
     }
     double sr = 0.0, si = 0.0;
+#pragma unroll 1
     for (int k = N - 1; k >= 0; k--) {
         const int p = perm[k];
         const double vr = br * rdr - bi * rdi, vi = br * rdi + bi * rdr;
