@@ -33,7 +33,7 @@ int build_fast(const chem_mech_desc *d, chem_mech *m)
 
     std::vector<double> job[2] = {std::vector<double>(kJobs * kJobW, 0.0), std::vector<double>(kJobs * kJobW, 0.0)};
     std::vector<double> sp[2] = {std::vector<double>(16 * kJobW, 0.0), std::vector<double>(16 * kJobW, 0.0)};
-    std::vector<int> slots(32, 0), nus(32, 0), type(32, -1), jobs(32, 0);
+    std::vector<int> slots(32, 0), type(32, -1), jobs(32, 0);
     // idle jobs evaluate exp(-inf) = 0 harmlessly?  keep them at exp(0) = 1: all-zero rows.
     for (int k = 0; k < ns; k++)
         for (int r = 0; r < 2; r++) {
@@ -128,7 +128,12 @@ int build_fast(const chem_mech_desc *d, chem_mech *m)
     // incidence lists (species -> reactions with net coefficient) and efficiency lists (alpha - 1)
     std::vector<double> inc_nu, eff_dv;
     std::vector<int> inc_rx, eff_sp, desc(32 * 8, 0);
-    for (int l = 0; l < 32; l++) { desc[8 * l] = slots[l]; desc[8 * l + 1] = nus[l]; desc[8 * l + 2] = type[l]; desc[8 * l + 3] = jobs[l]; }
+    int n_falloff = 0;
+    for (int l = 0; l < 32; l++) {
+        desc[8 * l] = slots[l]; desc[8 * l + 2] = type[l]; desc[8 * l + 3] = jobs[l];
+        desc[8 * l + 1] = type[l] >= 2 ? n_falloff++ : 0;       // falloff ordinal: phase-2 lane group of warp_rhs3
+    }
+    if (n_falloff > 5) return CHEM_OK;                          // 6 phase-2 lanes per falloff reaction
     for (int i = 0; i < nr; i++) {
         desc[8 * i + 4] = (int)eff_sp.size();
         if (d->rxn_type[i] != 0)
@@ -152,7 +157,7 @@ int build_fast(const chem_mech_desc *d, chem_mech *m)
     std::vector<double> host(total, 0.0);
     int *hdr = reinterpret_cast<int *>(host.data());
     const int LD = ns | 1;
-    hdr[0] = ns; hdr[1] = nr; hdr[2] = o_inc_nu; hdr[3] = o_inc_rx; hdr[4] = o_eff_dv; hdr[5] = o_eff_sp; hdr[6] = LD;
+    hdr[0] = ns; hdr[1] = nr; hdr[2] = o_inc_nu; hdr[3] = o_inc_rx; hdr[4] = o_eff_dv; hdr[5] = o_eff_sp; hdr[6] = LD; hdr[7] = n_falloff;
     std::memcpy(&host[kOffJobLo], job[0].data(), kJobs * kJobW * 8);
     std::memcpy(&host[kOffJobHi], job[1].data(), kJobs * kJobW * 8);
     std::memcpy(&host[kOffSpLo], sp[0].data(), 16 * kJobW * 8);

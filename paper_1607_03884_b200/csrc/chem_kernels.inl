@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(kWarpBlock, 2) integrate_warp_kernel(Tables t,
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int N = t.n_sp;
     double *ws = smem + ft.blob_doubles + (size_t)wib * warp_ws_doubles(N, t.n_rx);
-    if (lane >= N) ws[kWsC + lane] = 1.0;   // C[31] = 1: the unity factor of the rate products
+    if (lane >= N) { ws[kWsC + lane] = 1.0; ws[kWsC + 32 + lane] = 1.0; ws[kWsC + 64 + lane] = 1.0; }   // C[s][31] = 1: unity factor
     __syncwarp();
     for (;;) {
         int q = 0;

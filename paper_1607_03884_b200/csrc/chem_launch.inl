@@ -122,6 +122,9 @@ extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double
     prm.h0 = o ? o->h0 : 0.0;
     prm.max_steps = o ? o->max_steps : 0;
     prm.newton_max = o ? o->newton_max : 0;
+    prm.rtol_t = 0.1 * std::pow(rtol, 2.0 / 3.0);
+    prm.atol_t = prm.rtol_t * (atol / rtol);
+    prm.fnewt = std::fmax(10.0 * 2.220446049250313e-16 / prm.rtol_t, std::fmin(0.03, std::sqrt(prm.rtol_t)));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int kernel = o ? o->kernel : 0;
     if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "register-resident warp kernel not available for this mechanism");

@@ -69,6 +69,7 @@ __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW)
 struct RadauParams {
     double t_end, rtol, atol, h0;
     int max_steps, newton_max;
+    double rtol_t, atol_t, fnewt;   // RADAU5's transformed tolerances and Newton stopping level (R8), set on the host
 };
 
 struct RadauResult {

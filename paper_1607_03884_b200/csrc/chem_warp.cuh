@@ -23,7 +23,7 @@ constexpr int kOffSpHi = kOffSpLo + 16 * kJobW, kOffDesc = kOffSpHi + 16 * kJobW
 constexpr int kOffLists = kOffDesc + 128;
 
 // Tables of the fast path: one blob in global memory, staged into shared memory once per CTA.
-// blob[0..7] is a header of ints: {n_sp, n_rx, off_inc_nu, off_inc_rx, off_eff_dv, off_eff_sp, LD, 0} (offsets in doubles).
+// blob[0..7] is a header of ints: {n_sp, n_rx, off_inc_nu, off_inc_rx, off_eff_dv, off_eff_sp, LD, n_falloff} (offsets in doubles).
 struct FastTables {
     int enabled;
     int n_sp, n_rx;
@@ -51,8 +51,9 @@ __device__ __noinline__ double exp_ni(double a) { return exp(a); }
 __device__ __noinline__ double log_ni(double a) { return log(a); }
 constexpr double kLn10 = 2.302585092994045684, kInvLn10 = 0.4342944819032518277;
 
-// per-warp scratch layout (doubles): C[32] (C[31] = 1 for unused factor slots) E[64] q[32] ys[16] then matrices
-constexpr int kWsC = 0, kWsE = 32, kWsQ = 32 + kJobs, kWsYs = kWsQ + 32, kWsMat = kWsYs + 16;
+// per-warp scratch layout (doubles), three stage slots each: C[3][32] (C[s][31] = 1 for unused factor slots),
+// E[3][64] exp-job results, q[3][32] rates of progress, X[48] stage parameters and phase-2 jobs; then matrices
+constexpr int kWsC = 0, kWsE = 96, kWsQ = kWsE + 3 * kJobs, kWsX = kWsQ + 96, kWsMat = kWsX + 48;
 
 // exponent of job row c at T and its temperature derivative
 __device__ __forceinline__ double job_arg(const double *c, double T, double lnT, double invT)
@@ -102,66 +103,176 @@ __device__ __forceinline__ WarpMix warp_front(const double *tab, double *ws, dou
     return m;
 }
 
-// Source term for the state whose component `lane` is yc (lane 0: T, lanes 1..N-1: Y_1..Y_{N-1}).
-// Returns component `lane` of f.  DESIGN.md R1-R5; same mathematics as rhs<G>() in chem_device.cuh.
-// tab = staged table blob (shared), ws = this warp's scratch (shared).
-__device__ __noinline__ double warp_rhs(const double *tab, double *ws, double tmid, double P, double invP, double yc)
+struct D3 { double a, b, c; };
+
+// Source term at THREE states at once (the three Radau stage points of one Newton iteration):
+// component `lane` of stage s is y.a / y.b / y.c (lane 0: T, lanes 1..N-1: Y_1..Y_{N-1}); returns component
+// `lane` of the three f.  DESIGN.md R1-R5; same mathematics as rhs<G>() in chem_device.cuh.
+// Batching the stages lets one instruction stream serve 3 x 64 exp jobs, lets single lanes take the serial
+// transcendentals (ln T, reciprocals, the Troe broadening factor of every (reaction, stage) pair) in
+// parallel, and shares every table read.  tab = staged table blob (shared), ws = this warp's scratch (shared).
+__device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid, double P, double invP, D3 y)
 {
     const int lane = threadIdx.x & 31;
     const int *hdr = reinterpret_cast<const int *>(tab);
     const int N = hdr[0];
-    const int4 d0 = reinterpret_cast<const int4 *>(tab + kOffDesc)[2 * lane];       // factors, -, type, jobs
+    const int4 d0 = reinterpret_cast<const int4 *>(tab + kOffDesc)[2 * lane];       // factors, troe ordinal, type, jobs
     const int4 d1 = reinterpret_cast<const int4 *>(tab + kOffDesc)[2 * lane + 1];   // eff_lo, eff_hi, inc_lo, inc_hi
-    double *C = ws + kWsC, *E = ws + kWsE, *q = ws + kWsQ;
-    const WarpMix m = warp_front(tab, ws, tmid, P, invP, yc, lane, N);
-    const double T = m.T;
-    // rate of progress of reaction `lane`: factors are species indices with multiplicity, 31 = unity
-    double qi = 0.0;
+    double *C = ws + kWsC, *E = ws + kWsE, *q = ws + kWsQ, *X = ws + kWsX;
+    const int row = lane < N ? lane : 0;
+    double T[3], Yk[3], sY[3], sYW[3];
+    T[0] = __shfl_sync(0xffffffffu, y.a, 0); T[1] = __shfl_sync(0xffffffffu, y.b, 0); T[2] = __shfl_sync(0xffffffffu, y.c, 0);
+    Yk[0] = __shfl_down_sync(0xffffffffu, y.a, 1); Yk[1] = __shfl_down_sync(0xffffffffu, y.b, 1);
+    Yk[2] = __shfl_down_sync(0xffffffffu, y.c, 1);
+    const double invWk = tab[kOffSpLo + row * kJobW + 7], invWN = tab[kOffSpLo + (N - 1) * kJobW + 7];
+#pragma unroll
+    for (int s = 0; s < 3; s++) {
+        if (lane >= N - 1) Yk[s] = 0.0;
+        sY[s] = Yk[s];
+        sYW[s] = Yk[s] * invWk;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int s = 0; s < 3; s++) {
+            sY[s] += __shfl_xor_sync(0xffffffffu, sY[s], o);
+            sYW[s] += __shfl_xor_sync(0xffffffffu, sYW[s], o);
+        }
+    double sW[3];
+#pragma unroll
+    for (int s = 0; s < 3; s++) {
+        const double YN = 1.0 - sY[s];                      // closure: last species
+        if (lane == N - 1) Yk[s] = YN;
+        sW[s] = sYW[s] + YN * invWN;                        // 1 / Wbar
+    }
+    // serial transcendentals, one lane each: lanes 0-2 take T_s (ln, 1/x), lanes 3-5 take 1/Wbar_s (1/x)
+    const int sl3 = lane % 3;
+    const double Tsel = sl3 == 0 ? T[0] : (sl3 == 1 ? T[1] : T[2]);
+    const double Wsel = sl3 == 0 ? sW[0] : (sl3 == 1 ? sW[1] : sW[2]);
+    const double lnsel = log(Tsel);
+    const double rsel = __drcp_rn((lane >= 3 && lane < 6) ? Wsel : Tsel);
+    double invT[3], rho[3], inv_rho[3], Ck[3];
+#pragma unroll
+    for (int s = 0; s < 3; s++) {
+        invT[s] = __shfl_sync(0xffffffffu, rsel, s);
+        const double Wbar = __shfl_sync(0xffffffffu, rsel, 3 + s);
+        const double lnT = __shfl_sync(0xffffffffu, lnsel, s);
+        rho[s] = P * Wbar * invT[s] * (1.0 / kRerg);
+        inv_rho[s] = kRerg * T[s] * sW[s] * invP;
+        Ck[s] = rho[s] * Yk[s] * invWk;
+        if (lane < N) C[32 * s + lane] = Ck[s];
+        if (lane == 0) { X[4 * s] = T[s]; X[4 * s + 1] = lnT; X[4 * s + 2] = invT[s]; }
+    }
+    __syncwarp();
+    // exp jobs: 3 stages x 2 rounds per lane, one rolled loop
+#pragma unroll 1
+    for (int it = 0; it < 6; it++) {
+        const int s = it >> 1, r = it & 1;
+        const double Ts = X[4 * s], lnT = X[4 * s + 1], iT = X[4 * s + 2];
+        const double *c = tab + (Ts <= tmid ? kOffJobLo : kOffJobHi) + (32 * r + lane) * kJobW;
+        E[kJobs * s + 32 * r + lane] = exp(job_arg(c, Ts, lnT, iT));
+    }
+    __syncwarp();
+    // rates of progress of reaction `lane` at the three stages; factors: species indices with multiplicity, 31 = unity
     const int type = d0.z;
+    double rnet[3] = {0.0, 0.0, 0.0}, cm[3] = {1.0, 1.0, 1.0};
     if (type >= 0) {
-        const double Rf = E[lane] * (C[d0.x & 31] * C[(d0.x >> 5) & 31] * C[(d0.x >> 10) & 31]);
-        const double Rr = E[32 + lane] * (C[(d0.x >> 15) & 31] * C[(d0.x >> 20) & 31] * C[(d0.x >> 25) & 31]);
-        double c = 1.0;
+#pragma unroll
+        for (int s = 0; s < 3; s++) {
+            const double *Cs = C + 32 * s, *Es = E + kJobs * s;
+            const double Rf = Es[lane] * (Cs[d0.x & 31] * Cs[(d0.x >> 5) & 31] * Cs[(d0.x >> 10) & 31]);
+            const double Rr = Es[32 + lane] * (Cs[(d0.x >> 15) & 31] * Cs[(d0.x >> 20) & 31] * Cs[(d0.x >> 25) & 31]);
+            rnet[s] = Rf - Rr;
+        }
         if (type != 0) {
             const double *eff_dv = tab + hdr[4];
             const int *eff_sp = reinterpret_cast<const int *>(tab + hdr[5]);
-            double M = P * m.invT * (1.0 / kRerg);
+#pragma unroll
+            for (int s = 0; s < 3; s++) cm[s] = P * invT[s] * (1.0 / kRerg);
 #pragma unroll 1
-            for (int p = d1.x; p < d1.y; p++) M += eff_dv[p] * C[eff_sp[p]];
-            c = M;
+            for (int p = d1.x; p < d1.y; p++) {
+                const double dv = eff_dv[p];
+                const int sp = eff_sp[p];
+                cm[0] += dv * C[sp]; cm[1] += dv * C[32 + sp]; cm[2] += dv * C[64 + sp];
+            }
             if (type >= 2) {
-                const double Pr = E[d0.w & 255] * M;
-                double F = 1.0;
-                if (type == 3) {
+                // hand (Fcent, Pr) of every (reaction, stage) pair to the phase-2 lanes; Lindemann: Fcent = 1
+                const int slot = 12 + 6 * d0.y;
+#pragma unroll
+                for (int s = 0; s < 3; s++) {
+                    const double *Es = E + kJobs * s;
                     const int ts = (d0.w >> 8) & 255;
-                    const double L = log_ni(E[ts] + E[ts + 1] + E[ts + 2]) * kInvLn10;      // log10 Fcent
-                    const double At = log_ni(Pr) * kInvLn10 - 0.4 - 0.67 * L;
-                    const double x = At * __drcp_rn(0.75 - 1.27 * L - 0.14 * At);
-                    F = exp_ni(kLn10 * L * __drcp_rn(1.0 + x * x));
+                    X[slot + 2 * s] = type == 3 ? Es[ts] + Es[ts + 1] + Es[ts + 2] : 1.0;
+                    X[slot + 2 * s + 1] = Es[d0.w & 255] * cm[s];
                 }
-                c = Pr * __drcp_rn(1.0 + Pr) * F;
             }
         }
-        qi = c * (Rf - Rr);
     }
-    q[lane] = qi;
     __syncwarp();
-    // species production rates, temperature equation
+    // phase 2: lane pair (2p, 2p+1) serves falloff pair p = (ordinal, stage): c = Pr/(1+Pr) F  (R5)
+    {
+        const int nfo = hdr[7];                                   // number of falloff reactions
+        const bool live = lane < 6 * nfo;
+        const double v = live ? X[12 + lane] : 1.0;
+        const double lg = log(v) * kInvLn10;                      // even lane: log10 Fcent, odd lane: log10 Pr
+        const double lPr = __shfl_down_sync(0xffffffffu, lg, 1);
+        const double Pr = __shfl_down_sync(0xffffffffu, v, 1);
+        const double At = lPr - 0.4 - 0.67 * lg;
+        const double x = At * __drcp_rn(0.75 - 1.27 * lg - 0.14 * At);
+        const double F = exp(kLn10 * lg * __drcp_rn(1.0 + x * x));
+        const double c = Pr * __drcp_rn(1.0 + Pr) * F;
+        __syncwarp();
+        if (live && !(lane & 1)) X[12 + lane] = c;
+    }
+    __syncwarp();
+    if (type >= 2) {
+        const int slot = 12 + 6 * d0.y;
+        cm[0] = X[slot]; cm[1] = X[slot + 2]; cm[2] = X[slot + 4];
+    }
+#pragma unroll
+    for (int s = 0; s < 3; s++) q[32 * s + lane] = type >= 0 ? cm[s] * rnet[s] : 0.0;
+    __syncwarp();
+    // species production rates (three stages per pass over the incidence list), temperature equation
     const double *inc_nu = tab + hdr[2];
     const int *inc_rx = reinterpret_cast<const int *>(tab + hdr[3]);
-    double w = 0.0;
+    double w[3] = {0.0, 0.0, 0.0};
 #pragma unroll 1
-    for (int p = d1.z; p < d1.w; p++) w += inc_nu[p] * q[inc_rx[p]];
-    const double *spc = m.spc;
-    const double cpR = spc[0] + T * (spc[1] + T * (spc[2] + T * (spc[3] + T * spc[4])));
-    const double hRT = spc[0] + T * (spc[1] * 0.5 + T * (spc[2] * (1.0 / 3.0) + T * (spc[3] * 0.25 + T * (spc[4] * 0.2)))) + spc[5] * m.invT;
-    double hw = (lane < N) ? hRT * w : 0.0, ccp = (lane < N) ? m.Ck * cpR : 0.0;
-    warp_sum2(hw, ccp);
-    const double Ydot = spc[6] * w * m.inv_rho;           // W_k wdot_k / rho in species lane k
-    double f = __shfl_up_sync(0xffffffffu, Ydot, 1);      // component k+1
-    if (lane == 0) f = -T * hw * __drcp_rn(ccp);
+    for (int p = d1.z; p < d1.w; p++) {
+        const double nu = inc_nu[p];
+        const int i = inc_rx[p];
+        w[0] += nu * q[i]; w[1] += nu * q[32 + i]; w[2] += nu * q[64 + i];
+    }
+    double hw[3], ccp[3];
+#pragma unroll
+    for (int s = 0; s < 3; s++) {
+        const double *spc = tab + (T[s] <= tmid ? kOffSpLo : kOffSpHi) + row * kJobW;
+        const double Ts = T[s];
+        const double cpR = spc[0] + Ts * (spc[1] + Ts * (spc[2] + Ts * (spc[3] + Ts * spc[4])));
+        const double hRT = spc[0] + Ts * (spc[1] * 0.5 + Ts * (spc[2] * (1.0 / 3.0) + Ts * (spc[3] * 0.25 + Ts * (spc[4] * 0.2)))) + spc[5] * invT[s];
+        hw[s] = lane < N ? hRT * w[s] : 0.0;
+        ccp[s] = lane < N ? Ck[s] * cpR : 0.0;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int s = 0; s < 3; s++) {
+            hw[s] += __shfl_xor_sync(0xffffffffu, hw[s], o);
+            ccp[s] += __shfl_xor_sync(0xffffffffu, ccp[s], o);
+        }
+    const double Wk = tab[kOffSpLo + row * kJobW + 6];
+    const double rc = __drcp_rn(sl3 == 0 ? ccp[0] : (sl3 == 1 ? ccp[1] : ccp[2]));
+    double f[3];
+#pragma unroll
+    for (int s = 0; s < 3; s++) {
+        const double Ydot = Wk * w[s] * inv_rho[s];               // W_k wdot_k / rho in species lane k
+        f[s] = __shfl_up_sync(0xffffffffu, Ydot, 1);               // component k+1
+        const double rccp = __shfl_sync(0xffffffffu, rc, s);
+        if (lane == 0) f[s] = -T[s] * hw[s] * rccp;
+    }
     __syncwarp();
-    return f;
+    D3 out;
+    out.a = f[0]; out.b = f[1]; out.c = f[2];
+    return out;
 }
 
 // Analytical Jacobian (R6) for the warp path: Jm[i*N + j] = d f_i / d y_j in shared memory.
