@@ -6,34 +6,31 @@
 
 namespace chem {
 
-// Per-warp scratch (doubles) after the fixed part [C E q ys]: Jm[N*N] E1[N*LD] E2[max(2 N LD, 8 NR)] perm[16] chem[5*16+2]
+// Per-warp scratch (doubles) after the fixed part [C E q X]: Jm[N*N] Ar[2][N*LD] Ai[2][N*LD] (>= 8*32 Jacobian scratch) perm[32 ints] vec[48]
 __host__ __device__ inline int warp_ws_doubles(int N, int NR)
 {
     const int LD = N | 1;
-    const int e2 = 2 * N * LD > 8 * NR ? 2 * N * LD : 8 * NR;
-    return kWsMat + N * N + N * LD + e2 + 16 + 5 * 16 + 2;
+    const int e = 4 * N * LD > 8 * 32 ? 4 * N * LD : 8 * 32;
+    (void)NR;
+    return kWsMat + N * N + e + 16 + 48;
 }
 
 struct WarpMats {
-    double *Jm, *E1, *E2r, *E2i;
-    int *perm1, *perm2;
-    ChemScratch cs;
+    double *Jm, *Ar, *Ai, *vec;
+    int *perm;
     int N, LD;
 };
 
-__device__ __forceinline__ WarpMats warp_mats(double *ws, int N, int NR)
+__device__ __forceinline__ WarpMats warp_mats(double *ws, int N)
 {
     WarpMats m;
     m.N = N; m.LD = N | 1;
     double *p = ws + kWsMat;
     m.Jm = p; p += N * N;
-    m.E1 = p; p += N * m.LD;
-    m.E2r = p; m.E2i = p + N * m.LD;
-    m.cs.dq = p; m.cs.dqdT = p + 6 * NR; m.cs.tb = p + 7 * NR;     // alive only inside jacobian()
-    p += (2 * N * m.LD > 8 * NR ? 2 * N * m.LD : 8 * NR);
-    m.perm1 = reinterpret_cast<int *>(p); m.perm2 = m.perm1 + 16; p += 16;
-    m.cs.C = ws + kWsC; m.cs.q = ws + kWsQ;
-    m.cs.g = p; m.cs.hRT = p + 16; m.cs.cpR = p + 32; m.cs.dcpR = p + 48; m.cs.wdot = p + 64; m.cs.red = p + 80;
+    m.Ar = p; m.Ai = p + 2 * N * m.LD;          // the Jacobian routine borrows Ar.. as its 8*32 scratch
+    p += (4 * N * m.LD > 8 * 32 ? 4 * N * m.LD : 8 * 32);
+    m.perm = reinterpret_cast<int *>(p); p += 16;
+    m.vec = p;
     return m;
 }
 
@@ -50,7 +47,8 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     const double CFAC = SAFE * (1 + 2 * NIT);
     const int lane = threadIdx.x & 31;
     const int N = t.n_sp;
-    const WarpMats M = warp_mats(ws, N, t.n_rx);
+    const WarpMats M = warp_mats(ws, N);
+    const int h = lane >> 4, r16 = lane & 15;
     const int LD = M.LD;
     const bool mine = lane < N;
     const double invP = 1.0 / P;
@@ -72,14 +70,14 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     st.nfcn++;
     double z1 = 0, z2 = 0, z3 = 0, w1 = 0, w2 = 0, w3 = 0, c1 = 0, c2 = 0, c3 = 0;
     // LU factors
-    int myk1 = -1, myk2 = -1;
-    double rd1 = 0, rd2r = 0, rd2i = 0;
+    int myk = -1;
+    double rdr = 0, rdi = 0;
 
     enum { DO_JAC, DO_FACT, DO_STEP };
     int next = DO_JAC;
     for (;;) {
         if (next == DO_JAC) {
-            warp_jacobian(tab, ws, tmid, P, invP, y, M.Jm, M.E2r, M.cs.g);
+            warp_jacobian(tab, ws, tmid, P, invP, y, M.Jm, M.Ar, M.vec);
             st.njac++;
             CALJAC = true;
             next = DO_FACT;
@@ -87,19 +85,21 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         if (next == DO_FACT) {
             const double invH = 1.0 / H;
             const double FAC1 = U1 * invH, ALPHN = ALPH * invH, BETAN = BETA * invH;
+            // half-warp 0: E1 = gamma/h I - J (imaginary plane zero), half-warp 1: E2 = (alpha + i beta)/h I - J
             bool nonfinite = false;
-            if (mine)
+            if (r16 < N) {
+                double *ar = M.Ar + h * N * LD + r16 * LD, *ai = M.Ai + h * N * LD + r16 * LD;
+                const double dre = h ? ALPHN : FAC1, dim = h ? BETAN : 0.0;
                 for (int j = 0; j < N; j++) {
-                    const double v = -M.Jm[lane * N + j];
+                    const double v = -M.Jm[r16 * N + j];
                     nonfinite |= !isfinite(v);
-                    M.E1[lane * LD + j] = (j == lane) ? v + FAC1 : v;
-                    M.E2r[lane * LD + j] = (j == lane) ? v + ALPHN : v;
-                    M.E2i[lane * LD + j] = (j == lane) ? BETAN : 0.0;
+                    ar[j] = (j == r16) ? v + dre : v;
+                    ai[j] = (j == r16) ? dim : 0.0;
                 }
+            }
             int ier = __any_sync(0xffffffffu, nonfinite);
             __syncwarp();
-            if (!ier) ier = lu_warp_real(M.E1, LD, N, M.perm1, myk1, rd1);
-            if (!ier) ier = lu_warp_complex(M.E2r, M.E2i, LD, N, M.perm2, myk2, rd2r, rd2i);
+            if (!ier) ier = lu_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi);
             __syncwarp();
             st.ndec++;
             if (ier) {
@@ -140,10 +140,13 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             z1 = TI11 * a1 + TI12 * a2 + TI13 * a3 - w1 * FAC1;
             z2 = TI21 * a1 + TI22 * a2 + TI23 * a3 - w2 * ALPHN + w3 * BETAN;
             z3 = TI31 * a1 + TI32 * a2 + TI33 * a3 - w3 * ALPHN - w2 * BETAN;
-            z1 = solve_warp_real(M.E1, LD, N, M.perm1, myk1, rd1, z1);
             {
-                const double2 zc = solve_warp_complex(M.E2r, M.E2i, LD, N, M.perm2, myk2, rd2r, rd2i, z2, z3);
-                z2 = zc.x; z3 = zc.y;
+                // lower half solves the real system for z1, upper half the complex system for (z2, z3)
+                const double t2 = __shfl_sync(0xffffffffu, z2, r16), t3 = __shfl_sync(0xffffffffu, z3, r16);
+                const double2 x = solve_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi, h ? t2 : z1, h ? t3 : 0.0);
+                z1 = x.x;
+                z2 = __shfl_sync(0xffffffffu, x.x, 16 + r16);
+                z3 = __shfl_sync(0xffffffffu, x.y, 16 + r16);
             }
             st.nsol++;
             NEWT++;
@@ -194,7 +197,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         double ERR;
         {
             const double f2 = (DD1 * z1 + DD2 * z2 + DD3 * z3) * invH;
-            double cont = solve_warp_real(M.E1, LD, N, M.perm1, myk1, rd1, f2 + f0);
+            double cont = solve_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi, h ? 0.0 : f2 + f0, 0.0).x;
             double e = 0.0;
             if (mine) { const double q = cont * iscal; e = q * q; }
             ERR = fmax(sqrt(warp_sum(e) / N), 1.0e-10);
@@ -202,7 +205,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
                 const double yc = y + cont;
                 const double fr = warp_rhs3(tab, ws, tmid, P, invP, D3{yc, yc, yc}).a;
                 st.nfcn++;
-                cont = solve_warp_real(M.E1, LD, N, M.perm1, myk1, rd1, fr + f2);
+                cont = solve_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi, h ? 0.0 : fr + f2, 0.0).x;
                 e = 0.0;
                 if (mine) { const double q = cont * iscal; e = q * q; }
                 ERR = fmax(sqrt(warp_sum(e) / N), 1.0e-10);

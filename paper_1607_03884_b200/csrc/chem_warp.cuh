@@ -437,59 +437,49 @@ __device__ __forceinline__ int warp_argmax(double v)
     return __ffs(cand) - 1;
 }
 
-// Real LU, A[i*LD + j] in shared memory, row i owned by lane i.  perm[k] = pivot lane of step k; myk = the
-// step at which this lane's row was the pivot row; rdiag = 1/U_kk held by the pivot lane of step k.
-__device__ __noinline__ int lu_warp_real(double *A, int LD, int N, int *perm, int &myk_out, double &rdiag_out)
+// argmax inside one half-warp (mask hm, half h): returns the row 0..15 of the maximum, or -1.
+__device__ __forceinline__ int half_argmax(double v, unsigned hm, int h)
 {
-    const int lane = threadIdx.x & 31;
-    double *row = A + (lane < N ? lane : 0) * LD;
-    int myk = -1;
-    double rdiag = 0.0;
-    for (int k = 0; k < N; k++) {
-        const bool act = (lane < N) && (myk < 0);
-        const double ak = row[k];
-        const int p = warp_argmax(act ? fabs(ak) : -1.0);
-        if (p < 0) return k + 1;
-        const double *prow = A + p * LD;
-        const double pvv = prow[k];
-        if (!isfinite(pvv)) return k + 1;
-        const double rp = __drcp_rn(pvv);
-        if (lane == 0) perm[k] = p;
-        if (lane == p) { myk = k; rdiag = rp; }
-        if (act && lane != p) {
-            const double l = ak * rp;
-            row[k] = l;
-#pragma unroll 2
-            for (int j = k + 1; j < N; j++) row[j] = fma(-l, prow[j], row[j]);
-        }
-        __syncwarp();
+    const bool act = v >= 0.0;
+    const unsigned hi = act ? (unsigned)__double2hiint(v) : 0u;
+    const unsigned m = __reduce_max_sync(hm, hi);
+    unsigned cand = __ballot_sync(hm, act && hi == m) & hm;
+    if (__popc(cand) != 1) {
+        const unsigned lo = (act && hi == m) ? (unsigned)__double2loint(v) : 0u;
+        const unsigned m2 = __reduce_max_sync(hm, lo);
+        cand = __ballot_sync(hm, act && hi == m && lo == m2) & hm;
+        if (m == 0u && m2 == 0u) return -1;
     }
-    myk_out = myk;
-    rdiag_out = rdiag;
-    return 0;
+    if (cand == 0u) return -1;
+    return __ffs(cand) - 1 - 16 * h;
 }
 
-__device__ __noinline__ int lu_warp_complex(double *Ar, double *Ai, int LD, int N, int *perm, int &myk_out, double &rdr_out,
-                                            double &rdi_out)
+// LU of BOTH Radau matrices in one instruction stream: half-warp 0 factors the real matrix E1 (imaginary plane
+// zero), half-warp 1 the complex matrix E2, both with complex arithmetic ("LU factorization of the
+// Jacobian"; one real and one complex N x N system per step).  Planes: Ar[h][N*LD], Ai[h][N*LD]; row r of half h is
+// owned by lane 16 h + r and never moves.  perm[16 h + k] = pivot row of step k; myk = step at which this lane's
+// row was the pivot row; (rdr, rdi) = 1/U_kk held by that lane.  Partial pivoting on |re| + |im| (R10).
+__device__ __noinline__ int lu_warp_pair(double *Ar, double *Ai, int LD, int N, int *perm, int &myk_out, double &rdr_out,
+                                         double &rdi_out)
 {
-    const int lane = threadIdx.x & 31;
-    const int off = (lane < N ? lane : 0) * LD;
-    double *rr = Ar + off, *ri = Ai + off;
+    const int lane = threadIdx.x & 31, h = lane >> 4, r = lane & 15;
+    const unsigned hm = h ? 0xffff0000u : 0x0000ffffu;
+    double *Pr_ = Ar + h * N * LD, *Pi_ = Ai + h * N * LD;
+    double *rr = Pr_ + (r < N ? r : 0) * LD, *ri = Pi_ + (r < N ? r : 0) * LD;
     int myk = -1;
     double rdr = 0.0, rdi = 0.0;
     for (int k = 0; k < N; k++) {
-        const bool act = (lane < N) && (myk < 0);
+        const bool act = (r < N) && (myk < 0);
         const double akr = rr[k], aki = ri[k];
-        const int p = warp_argmax(act ? fabs(akr) + fabs(aki) : -1.0);
-        if (p < 0) return k + 1;
-        const double *pr_ = Ar + p * LD, *pi_ = Ai + p * LD;
+        const int p = half_argmax(act ? fabs(akr) + fabs(aki) : -1.0, hm, h);
+        const double *pr_ = Pr_ + (p < 0 ? 0 : p) * LD, *pi_ = Pi_ + (p < 0 ? 0 : p) * LD;
         const double pr = pr_[k], pi = pi_[k];
         const double den = __drcp_rn(pr * pr + pi * pi);
-        if (!isfinite(den)) return k + 1;
+        if (__any_sync(0xffffffffu, p < 0 || !isfinite(den))) return k + 1;
         const double qr = pr * den, qi = -pi * den;       // 1 / pivot
-        if (lane == 0) perm[k] = p;
-        if (lane == p) { myk = k; rdr = qr; rdi = qi; }
-        if (act && lane != p) {
+        if (r == 0) perm[16 * h + k] = p;
+        if (r == p) { myk = k; rdr = qr; rdi = qi; }
+        if (act && r != p) {
             const double lr = akr * qr - aki * qi, li = akr * qi + aki * qr;
             rr[k] = lr;
             ri[k] = li;
@@ -508,35 +498,19 @@ __device__ __noinline__ int lu_warp_complex(double *Ar, double *Ai, int LD, int 
     return 0;
 }
 
-// Solves: b = component `lane` of the right-hand side (original row order); returns component `lane` of x.
-__device__ __noinline__ double solve_warp_real(const double *A, int LD, int N, const int *perm, int myk, double rdiag, double b)
+// Solve with both factorisations at once: lane 16 h + r passes row r of the right-hand side of system h
+// and receives component r of its solution.
+__device__ __noinline__ double2 solve_warp_pair(const double *Ar, const double *Ai, int LD, int N, const int *perm, int myk,
+                                                double rdr, double rdi, double br, double bi)
 {
-    const int lane = threadIdx.x & 31;
-    const double *row = A + (lane < N ? lane : 0) * LD;
-#pragma unroll 1
-    for (int k = 0; k < N - 1; k++) {
-        const double bk = __shfl_sync(0xffffffffu, b, perm[k]);
-        if (myk > k) b = fma(-row[k], bk, b);
-    }
-    double x = 0.0;
-#pragma unroll 1
-    for (int k = N - 1; k >= 0; k--) {
-        const double xk = __shfl_sync(0xffffffffu, b * rdiag, perm[k]);
-        if (myk >= 0 && myk < k) b = fma(-row[k], xk, b);
-        if (lane == k) x = xk;
-    }
-    return x;
-}
-
-__device__ __noinline__ double2 solve_warp_complex(const double *Ar, const double *Ai, int LD, int N, const int *perm, int myk,
-                                                   double rdr, double rdi, double br, double bi)
-{
-    const int lane = threadIdx.x & 31;
-    const int off = (lane < N ? lane : 0) * LD;
+    const int lane = threadIdx.x & 31, h = lane >> 4, r = lane & 15;
+    const int off = h * N * LD + (r < N ? r : 0) * LD;
     const double *rr = Ar + off, *ri = Ai + off;
+    const int *pm = perm + 16 * h;
+    const int base = 16 * h;
 #pragma unroll 1
     for (int k = 0; k < N - 1; k++) {
-        const int p = perm[k];
+        const int p = pm[k] + base;
         const double xr = __shfl_sync(0xffffffffu, br, p), xi = __shfl_sync(0xffffffffu, bi, p);
         if (myk > k) {
             const double lr = rr[k], li = ri[k];
@@ -547,7 +521,7 @@ __device__ __noinline__ double2 solve_warp_complex(const double *Ar, const doubl
     double sr = 0.0, si = 0.0;
 #pragma unroll 1
     for (int k = N - 1; k >= 0; k--) {
-        const int p = perm[k];
+        const int p = pm[k] + base;
         const double vr = br * rdr - bi * rdi, vi = br * rdi + bi * rdr;
         const double xr = __shfl_sync(0xffffffffu, vr, p), xi = __shfl_sync(0xffffffffu, vi, p);
         if (myk >= 0 && myk < k) {
@@ -555,7 +529,7 @@ __device__ __noinline__ double2 solve_warp_complex(const double *Ar, const doubl
             br = fma(-ur, xr, fma(ui, xi, br));
             bi = fma(-ur, xi, fma(-ui, xr, bi));
         }
-        if (lane == k) { sr = xr; si = xi; }
+        if (r == k) { sr = xr; si = xi; }
     }
     return make_double2(sr, si);
 }
