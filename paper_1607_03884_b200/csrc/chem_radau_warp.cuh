@@ -66,7 +66,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     double FACCON = 1.0, THETA = 0.0, HACC = 0.0, ERRACC = 0.0;
     int NSING = 0;
     double iscal = 1.0 / (ATOL + RTOL * fabs(y));    // 1 / scal
-    double f0 = warp_rhs3(tab, ws, tmid, P, invP, D3{y, y, y}).a;
+    double f0 = warp_rhs3(tab, ws, tmid, P, invP, D3{y, y, y}, 1).a;
     st.nfcn++;
     double z1 = 0, z2 = 0, z3 = 0, w1 = 0, w2 = 0, w3 = 0, c1 = 0, c2 = 0, c3 = 0;
     // LU factors
@@ -134,7 +134,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         int outcome = 0;
         for (;;) {
             if (NEWT >= NIT) { outcome = 2; break; }
-            const D3 fs = warp_rhs3(tab, ws, tmid, P, invP, D3{y + z1, y + z2, y + z3});
+            const D3 fs = warp_rhs3(tab, ws, tmid, P, invP, D3{y + z1, y + z2, y + z3}, 3);
             const double a1 = fs.a, a2 = fs.b, a3 = fs.c;
             st.nfcn += 3;
             z1 = TI11 * a1 + TI12 * a2 + TI13 * a3 - w1 * FAC1;
@@ -203,7 +203,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             ERR = fmax(sqrt(warp_sum(e) / N), 1.0e-10);
             if (ERR >= 1.0 && (FIRST || REJECT)) {
                 const double yc = y + cont;
-                const double fr = warp_rhs3(tab, ws, tmid, P, invP, D3{yc, yc, yc}).a;
+                const double fr = warp_rhs3(tab, ws, tmid, P, invP, D3{yc, yc, yc}, 1).a;
                 st.nfcn++;
                 cont = solve_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi, h ? 0.0 : fr + f2, 0.0).x;
                 e = 0.0;
@@ -244,7 +244,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             iscal = 1.0 / (ATOL + RTOL * fabs(y));
             CALJAC = false;
             if (LAST) return;
-            f0 = warp_rhs3(tab, ws, tmid, P, invP, D3{y, y, y}).a;
+            f0 = warp_rhs3(tab, ws, tmid, P, invP, D3{y, y, y}, 1).a;
             st.nfcn++;
             HNEW = fmin(fabs(HNEW), XEND);
             if (REJECT) HNEW = fmin(HNEW, fabs(H));

@@ -111,7 +111,7 @@ struct D3 { double a, b, c; };
 // Batching the stages lets one instruction stream serve 3 x 64 exp jobs, lets single lanes take the serial
 // transcendentals (ln T, reciprocals, the Troe broadening factor of every (reaction, stage) pair) in
 // parallel, and shares every table read.  tab = staged table blob (shared), ws = this warp's scratch (shared).
-__device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid, double P, double invP, D3 y)
+__device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid, double P, double invP, D3 y, int nstage)
 {
     const int lane = threadIdx.x & 31;
     const int *hdr = reinterpret_cast<const int *>(tab);
@@ -166,13 +166,18 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     __syncwarp();
     // exp jobs: 3 stages x 2 rounds per lane, one rolled loop
 #pragma unroll 1
-    for (int it = 0; it < 6; it++) {
+    for (int it = 0; it < 2 * nstage; it++) {     // nstage = 1: the three inputs are copies, stage 0 only
         const int s = it >> 1, r = it & 1;
         const double Ts = X[4 * s], lnT = X[4 * s + 1], iT = X[4 * s + 2];
         const double *c = tab + (Ts <= tmid ? kOffJobLo : kOffJobHi) + (32 * r + lane) * kJobW;
         E[kJobs * s + 32 * r + lane] = exp(job_arg(c, Ts, lnT, iT));
     }
     __syncwarp();
+    if (nstage == 1) {                                // replicate stage 0 (same state): keeps the rest branch-free
+        E[kJobs + lane] = E[lane]; E[kJobs + 32 + lane] = E[32 + lane];
+        E[2 * kJobs + lane] = E[lane]; E[2 * kJobs + 32 + lane] = E[32 + lane];
+        __syncwarp();
+    }
     // rates of progress of reaction `lane` at the three stages; factors: species indices with multiplicity, 31 = unity
     const int type = d0.z;
     double rnet[3] = {0.0, 0.0, 0.0}, cm[3] = {1.0, 1.0, 1.0};
