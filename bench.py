@@ -133,8 +133,12 @@ def main():
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic shared-memory kernel, 2 warp kernel")
+    ap.add_argument("--states", type=int, default=0, help="profiling aid: use only the first N states of the config (not a bench line)")
     args = ap.parse_args()
-    cfg = synth.CONFIGS[args.config]
+    cfg = dict(synth.CONFIGS[args.config])
+    if args.states > 0:
+        cfg["n_states"] = min(args.states, cfg["n_states"])
+        cfg["name"] += f"[first {cfg['n_states']} states: profiling subset]"
     mech = synth.make_mechanism(cfg["kind"], synth.MECH_SEED)
     if args.impl == "reference":
         run_reference(args, cfg, mech)

@@ -47,9 +47,90 @@ __device__ __forceinline__ void warp_sum2(double &a, double &b)
     }
 }
 __device__ __noinline__ double pow_ni(double a, double b) { return pow(a, b); }
-__device__ __noinline__ double exp_ni(double a) { return exp(a); }
-__device__ __noinline__ double log_ni(double a) { return log(a); }
 constexpr double kLn10 = 2.302585092994045684, kInvLn10 = 0.4342944819032518277;
+
+// Compact fp64 elementary functions for normal, finite arguments (the rates, temperatures and step-size ratios of
+// this path).  Polynomial coefficients sit in constant memory so that each Horner step is ONE DFMA with a constant-bank
+// operand (the libdevice versions spend two UMOVs per coefficient and are 2-3x larger, which matters for the 32 KB
+// instruction cache).  Accuracy ~1-2 ulp; no special-case handling beyond what is stated.
+__constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320, 1.0 / 362880,
+                                 1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
+__constant__ double kAtanhC[11] = {2.0, 2.0 / 3, 2.0 / 5, 2.0 / 7, 2.0 / 9, 2.0 / 11, 2.0 / 13, 2.0 / 15, 2.0 / 17, 2.0 / 19, 2.0 / 21};
+
+// 1/x for normal x: hardware seed (MUFU.RCP64H) + two Newton steps; no denormal / zero / inf handling
+__device__ __forceinline__ double rcp_f(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+// a / b with one residual correction (<= 1 ulp for normal operands)
+__device__ __forceinline__ double div_f(double a, double b)
+{
+    const double r = rcp_f(b);
+    const double q = a * r;
+    return fma(fma(-b, q, a), r, q);
+}
+// sqrt(x) for normal x > 0: rsqrt seed + Newton, final Heron correction
+__device__ __forceinline__ double sqrt_f(double x)
+{
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    const double h = 0.5 * r;
+    double g = x * r;                       // ~sqrt(x)
+    double e = fma(-g, h, 0.5);
+    g = fma(g, e, g);
+    const double h2 = fma(h, e, h);
+    e = fma(-g, g, x);
+    return fma(e, h2, g);
+}
+// sqrt for x >= 0 including 0; NaN / negative -> NaN, inf -> NaN (both "non-finite" for the controller, R11)
+__device__ __forceinline__ double sqrt_s(double x)
+{
+    return x > 1e-300 ? sqrt_f(x) : (x >= 0.0 ? 0.0 : __longlong_as_double(0x7ff8000000000000LL));
+}
+// exp(x): x = n ln2 + r, |r| <= ln2/2, Taylor degree 13; returns 0 below -700, inf above 709
+__device__ __forceinline__ double exp_f(double x)
+{
+    const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);      // round(x / ln2) in the low word
+    const int n = __double2loint(t);
+    const double fn = t - 6755399441055744.0;
+    double r = fma(fn, -6.93147180369123816490e-01, x);
+    r = fma(fn, -1.90821492927058770002e-10, r);
+    double p = kExpC[13];
+#pragma unroll
+    for (int k = 12; k >= 0; k--) p = fma(p, r, kExpC[k]);
+    // scale by 2^n in two steps so that n down to -1074 + ... stays correct enough; clamp the far tails
+    const int n1 = n >> 1, n2 = n - n1;
+    p *= __hiloint2double((1023 + n1) << 20, 0);
+    p *= __hiloint2double((1023 + n2) << 20, 0);
+    if (x < -700.0) p = 0.0;
+    if (x > 709.0) p = __longlong_as_double(0x7ff0000000000000LL);
+    return p;
+}
+// log(x) for normal x > 0: x = 2^e m, m in [sqrt(1/2), sqrt(2)), log m = 2 atanh((m-1)/(m+1)), 11 odd terms
+__device__ __forceinline__ double log_f(double x)
+{
+    int hi = __double2hiint(x);
+    const int lo = __double2loint(x);
+    int e = (hi >> 20) - 1023;
+    hi = (hi & 0x000fffff) | 0x3ff00000;
+    double m = __hiloint2double(hi, lo);
+    if (m > 1.4142135623730951) { m *= 0.5; e += 1; }
+    const double s = div_f(m - 1.0, m + 1.0);
+    const double z = s * s;
+    double p = kAtanhC[10];
+#pragma unroll
+    for (int k = 9; k >= 1; k--) p = fma(p, z, kAtanhC[k]);
+    const double fe = (double)e;
+    // log x = e ln2_hi + (2 s + (s z p + e ln2_lo))
+    return fma(fe, 6.93147180369123816490e-01, fma(2.0, s, fma(s * z, p, fe * 1.90821492927058770002e-10)));
+}
+__device__ __noinline__ double exp_ni(double a) { return exp_f(a); }
+__device__ __noinline__ double log_ni(double a) { return log_f(a); }
 
 // per-warp scratch layout (doubles), three stage slots each: C[3][32] (C[s][31] = 1 for unused factor slots),
 // E[3][64] exp-job results, q[3][32] rates of progress, X[48] stage parameters and phase-2 jobs; then matrices
@@ -88,8 +169,8 @@ __device__ __forceinline__ WarpMix warp_front(const double *tab, double *ws, dou
     const double YN = 1.0 - sY;                            // closure: last species
     if (lane == N - 1) Yk = YN;
     const double sW = sYW + YN * spt[(N - 1) * kJobW + 7]; // 1 / Wbar
-    m.Wbar = __drcp_rn(sW);
-    m.invT = __drcp_rn(m.T);
+    m.Wbar = rcp_f(sW);
+    m.invT = rcp_f(m.T);
     m.rho = P * m.Wbar * m.invT * (1.0 / kRerg);
     m.inv_rho = kRerg * m.T * sW * invP;
     m.lnT = log_ni(m.T);
@@ -149,8 +230,8 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     const int sl3 = lane % 3;
     const double Tsel = sl3 == 0 ? T[0] : (sl3 == 1 ? T[1] : T[2]);
     const double Wsel = sl3 == 0 ? sW[0] : (sl3 == 1 ? sW[1] : sW[2]);
-    const double lnsel = log(Tsel);
-    const double rsel = __drcp_rn((lane >= 3 && lane < 6) ? Wsel : Tsel);
+    const double lnsel = log_f(Tsel);
+    const double rsel = rcp_f((lane >= 3 && lane < 6) ? Wsel : Tsel);
     double invT[3], rho[3], inv_rho[3], Ck[3];
 #pragma unroll
     for (int s = 0; s < 3; s++) {
@@ -170,7 +251,7 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
         const int s = it >> 1, r = it & 1;
         const double Ts = X[4 * s], lnT = X[4 * s + 1], iT = X[4 * s + 2];
         const double *c = tab + (Ts <= tmid ? kOffJobLo : kOffJobHi) + (32 * r + lane) * kJobW;
-        E[kJobs * s + 32 * r + lane] = exp(job_arg(c, Ts, lnT, iT));
+        E[kJobs * s + 32 * r + lane] = exp_f(job_arg(c, Ts, lnT, iT));
     }
     __syncwarp();
     if (nstage == 1) {                                // replicate stage 0 (same state): keeps the rest branch-free
@@ -219,13 +300,13 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
         const int nfo = hdr[7];                                   // number of falloff reactions
         const bool live = lane < 6 * nfo;
         const double v = live ? X[12 + lane] : 1.0;
-        const double lg = log(v) * kInvLn10;                      // even lane: log10 Fcent, odd lane: log10 Pr
+        const double lg = log_f(v) * kInvLn10;                      // even lane: log10 Fcent, odd lane: log10 Pr
         const double lPr = __shfl_down_sync(0xffffffffu, lg, 1);
         const double Pr = __shfl_down_sync(0xffffffffu, v, 1);
         const double At = lPr - 0.4 - 0.67 * lg;
-        const double x = At * __drcp_rn(0.75 - 1.27 * lg - 0.14 * At);
-        const double F = exp(kLn10 * lg * __drcp_rn(1.0 + x * x));
-        const double c = Pr * __drcp_rn(1.0 + Pr) * F;
+        const double x = At * rcp_f(0.75 - 1.27 * lg - 0.14 * At);
+        const double F = exp_f(kLn10 * lg * rcp_f(1.0 + x * x));
+        const double c = Pr * rcp_f(1.0 + Pr) * F;
         __syncwarp();
         if (live && !(lane & 1)) X[12 + lane] = c;
     }
@@ -265,7 +346,7 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
             ccp[s] += __shfl_xor_sync(0xffffffffu, ccp[s], o);
         }
     const double Wk = tab[kOffSpLo + row * kJobW + 6];
-    const double rc = __drcp_rn(sl3 == 0 ? ccp[0] : (sl3 == 1 ? ccp[1] : ccp[2]));
+    const double rc = rcp_f(sl3 == 0 ? ccp[0] : (sl3 == 1 ? ccp[1] : ccp[2]));
     double f[3];
 #pragma unroll
     for (int s = 0; s < 3; s++) {
@@ -324,19 +405,19 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
                         const double Fc = e3 + e1 + e2;
                         const double dFc = e3 * job_darg(m.jt + ts * kJobW, T, invT) + e1 * job_darg(m.jt + (ts + 1) * kJobW, T, invT) +
                                            e2 * job_darg(m.jt + (ts + 2) * kJobW, T, invT);
-                        const double L = log_ni(Fc) * kInvLn10, dL = dFc * __drcp_rn(Fc) * kInvLn10;
+                        const double L = log_ni(Fc) * kInvLn10, dL = dFc * rcp_f(Fc) * kInvLn10;
                         const double At = log_ni(Pr) * kInvLn10 - 0.4 - 0.67 * L;
-                        const double Bt = 0.75 - 1.27 * L - 0.14 * At, rB = __drcp_rn(Bt);
-                        const double x = At * rB, rden = __drcp_rn(1.0 + x * x);
+                        const double Bt = 0.75 - 1.27 * L - 0.14 * At, rB = rcp_f(Bt);
+                        const double x = At * rB, rden = rcp_f(1.0 + x * x);
                         F = exp_ni(kLn10 * L * rden);
                         const double dA_T = dlnPr * kInvLn10 - 0.67 * dL, dB_T = -1.27 * dL - 0.14 * dA_T;
                         const double dx_T = (dA_T * Bt - At * dB_T) * rB * rB;
-                        const double dx_P = __drcp_rn(Pr) * kInvLn10 * (Bt + 0.14 * At) * rB * rB;
+                        const double dx_P = rcp_f(Pr) * kInvLn10 * (Bt + 0.14 * At) * rB * rB;
                         const double wF = -L * 2.0 * x * rden * rden;
                         dF_dT = F * kLn10 * (dL * rden + wF * dx_T);
                         dF_dPr = F * kLn10 * wF * dx_P;
                     }
-                    const double op = __drcp_rn(1.0 + Pr);
+                    const double op = rcp_f(1.0 + Pr);
                     c = Pr * op * F;
                     dc_dT = Pr * dlnPr * op * op * F + Pr * op * dF_dT;
                     dc_dM = (op * op * F + Pr * op * dF_dPr) * k0k;
@@ -398,7 +479,7 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
     warp_sum2(hw, ccp);
     warp_sum2(cpw, cdcp);
     __syncwarp();
-    const double rccp = __drcp_rn(ccp);
+    const double rccp = rcp_f(ccp);
     const double Tdot = -T * hw * rccp;
     // columns: assemble the rows of J in place (row k+1 <- species k, descending; row 0 <- temperature)
     if (lane < N) {
@@ -479,7 +560,7 @@ __device__ __noinline__ int lu_warp_pair(double *Ar, double *Ai, int LD, int N, 
         const int p = half_argmax(act ? fabs(akr) + fabs(aki) : -1.0, hm, h);
         const double *pr_ = Pr_ + (p < 0 ? 0 : p) * LD, *pi_ = Pi_ + (p < 0 ? 0 : p) * LD;
         const double pr = pr_[k], pi = pi_[k];
-        const double den = __drcp_rn(pr * pr + pi * pi);
+        const double den = rcp_f(pr * pr + pi * pi);
         if (__any_sync(0xffffffffu, p < 0 || !isfinite(den))) return k + 1;
         const double qr = pr * den, qi = -pi * den;       // 1 / pivot
         if (r == 0) perm[16 * h + k] = p;
