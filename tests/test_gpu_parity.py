@@ -143,3 +143,52 @@ def test_edge_cases(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
     assert np.array_equal(binding.stats_to_numpy(st)["status"], st_ref["status"])
     with pytest.raises(binding.ChemError):
         binding.chem_integrate(m, P, -1.0, RTOL, ATOL, torch.from_numpy(y0).cuda())
+
+
+def test_full_size_config1_sampled_against_oracle(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
+    """BASELINE.json configs[1] at full size (1,048,576 states) in the launch configuration bench.py times (plain
+    chem_integrate, auto kernel): a random sample of states is recomputed by the oracle one by one; properties that
+    hold at any size are checked on ALL states."""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    cfg = synth.CONFIGS[1]
+    y0 = synth.make_states(mech_h2co, cfg["n_states"], cfg["dist"], synth.STATE_SEED)
+    y_dev = torch.from_numpy(y0).cuda()
+    y1 = binding.chem_integrate(gpu_mechs["h2co"], P, cfg["t_end"], RTOL, ATOL, y_dev).cpu().numpy()
+    assert np.all(np.isfinite(y1))
+    # all states: element mass fractions are linear invariants of the method; mass fractions stay in [-atol-ish, 1]
+    W = mech_h2co["mol_weight"]
+    comp = mech_h2co["elem_comp"].astype(np.float64)
+
+    def elem(y):
+        Y = np.concatenate([y[:, 1:], 1.0 - y[:, 1:].sum(axis=1, keepdims=True)], axis=1)
+        return (Y / W) @ comp
+    assert np.abs(elem(y1) - elem(y0)).max() < 1e-12
+    assert y1[:, 1:].min() > -1e-7 and y1[:, 1:].max() < 1.0 + 1e-9
+    assert np.all(y1[:, 0] > 500.0) and np.all(y1[:, 0] < 4000.0)
+    # sample: 2048 random states + the ragged tail of the last CTA
+    rng = np.random.default_rng(123)
+    idx = np.unique(np.concatenate([rng.choice(cfg["n_states"], 2048, replace=False), np.arange(cfg["n_states"] - 9, cfg["n_states"])]))
+    y_ref, st_ref, _ = orc_mechs["h2co"].integrate(y0[idx], P, cfg["t_end"], RTOL, ATOL)
+    assert np.all(st_ref["status"] == 0)
+    assert np.all(np.abs(y1[idx] - y_ref) <= 1e-9 + 1e-6 * np.abs(y_ref))
+    # statistics of the same launch configuration with the counters on
+    _, st = binding.chem_integrate_ex(gpu_mechs["h2co"], P, cfg["t_end"], RTOL, ATOL, y_dev)
+    st = binding.stats_to_numpy(st)
+    assert np.all(st["status"] == 0)
+    assert (st["naccpt"][idx] == st_ref["naccpt"]).mean() >= 0.99
+    assert (st["nstep"][idx] == st_ref["nstep"]).mean() >= 0.99
+
+
+def test_full_size_gri_sampled_against_oracle(torch_cuda, gpu_mechs, orc_mechs, mech_gri):
+    """configs[3] shape (gri, dt = 1e-6) on a 16,384-state slice of the full batch, sampled against the oracle"""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    cfg = synth.CONFIGS[3]
+    n = 16384
+    y0 = synth.make_states(mech_gri, n, cfg["dist"], synth.STATE_SEED)
+    y1 = binding.chem_integrate(gpu_mechs["gri"], P, cfg["t_end"], RTOL, ATOL, torch.from_numpy(y0).cuda()).cpu().numpy()
+    assert np.all(np.isfinite(y1))
+    idx = np.random.default_rng(5).choice(n, 96, replace=False)
+    y_ref, st_ref, _ = orc_mechs["gri"].integrate(y0[idx], P, cfg["t_end"], RTOL, ATOL)
+    assert np.all(np.abs(y1[idx] - y_ref) <= 1e-9 + 1e-6 * np.abs(y_ref))
