@@ -427,6 +427,210 @@ __device__ __noinline__ int lu_complex(int N, double *Ar, double *Ai, int *ip)
     return 0;
 }
 
+// ------------------------------------------------------------------------------------- LU without row moves (N <= 64)
+// Rows never move: lane l of EVERY warp tracks rows l and l + 32 (rowk = elimination step at which the row was the
+// pivot row, -1 before), warp w updates columns j = w (mod NW).  One barrier per elimination step.  After the
+// factorisation row i with rowk = m holds its multipliers in columns j < m and U_{m,j} in columns j >= m;
+// perm[k] = pivot row of step k, rd[k] = 1 / U_kk.  Multipliers of column k are written back one step late (by the
+// warp that owns the column) so that no warp can still be reading the column.
+struct Lu2Aux {
+    int *perm, *rowk;   // [N] each
+    double *rdr, *rdi;  // [N]; rdi unused for the real matrix
+};
+
+__device__ __forceinline__ double rcp_nr(double x)   // 1/x for normal x: MUFU seed + two Newton steps
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+
+// exact arg-max over a warp of (key >= 0 or -1 for inactive, row index); lowest lane wins exact ties
+__device__ __forceinline__ int warp_argmax_row(double v, int row)
+{
+    const bool act = v >= 0.0;
+    const unsigned hi = act ? (unsigned)__double2hiint(v) : 0u;
+    const unsigned m = __reduce_max_sync(0xffffffffu, hi);
+    unsigned cand = __ballot_sync(0xffffffffu, act && hi == m);
+    if (__popc(cand) != 1) {
+        const unsigned lo = (act && hi == m) ? (unsigned)__double2loint(v) : 0u;
+        const unsigned m2 = __reduce_max_sync(0xffffffffu, lo);
+        cand = __ballot_sync(0xffffffffu, act && hi == m && lo == m2);
+        if (m == 0u && m2 == 0u) return -1;
+    }
+    if (cand == 0u) return -1;
+    return __shfl_sync(0xffffffffu, row, __ffs(cand) - 1);
+}
+
+template <int G>
+__device__ __noinline__ int lu2_real(int N, double *A, const Lu2Aux &x)
+{
+    const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
+    constexpr int NW = Grp<G>::NW;
+    const int i0 = wl, i1 = wl + 32;
+    int k0 = (i0 < N) ? -1 : 1 << 30, k1 = (i1 < N) ? -1 : 1 << 30;   // rowk of my two rows (huge = no such row)
+    double l0 = 0.0, l1 = 0.0;
+    for (int k = 0; k < N; k++) {
+        // delayed write-back of the multipliers of column k-1 by its owner warp
+        if (k > 0 && wp == (k - 1) % NW) {
+            if (k0 < 0) A[i0 + (k - 1) * N] = l0;
+            if (k1 < 0) A[i1 + (k - 1) * N] = l1;
+        }
+        const double a0 = (k0 < 0) ? A[i0 + k * N] : 0.0, a1 = (k1 < 0) ? A[i1 + k * N] : 0.0;
+        const double v0 = (k0 < 0) ? fabs(a0) : -1.0, v1 = (k1 < 0) ? fabs(a1) : -1.0;
+        const int p = warp_argmax_row(v1 > v0 ? v1 : v0, v1 > v0 ? i1 : i0);
+        const double pv = (p >= 0) ? A[p + k * N] : 0.0;
+        if (p < 0 || !isfinite(pv)) return k + 1;
+        const double rp = rcp_nr(pv);
+        if (i0 == p) k0 = k;
+        if (i1 == p) k1 = k;
+        if (lane == 0) { x.perm[k] = p; x.rdr[k] = rp; x.rowk[p] = k; }
+        l0 = (k0 < 0) ? a0 * rp : 0.0;
+        l1 = (k1 < 0) ? a1 * rp : 0.0;
+        for (int j = k + 1 + ((wp - (k + 1)) % NW + NW) % NW; j < N; j += NW) {
+            const double u = A[p + j * N];
+            if (k0 < 0) A[i0 + j * N] = fma(-l0, u, A[i0 + j * N]);
+            if (k1 < 0) A[i1 + j * N] = fma(-l1, u, A[i1 + j * N]);
+        }
+        Grp<G>::sync();
+    }
+    return 0;
+}
+
+template <int G>
+__device__ __noinline__ int lu2_complex(int N, double *Ar, double *Ai, const Lu2Aux &x)
+{
+    const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
+    constexpr int NW = Grp<G>::NW;
+    const int i0 = wl, i1 = wl + 32;
+    int k0 = (i0 < N) ? -1 : 1 << 30, k1 = (i1 < N) ? -1 : 1 << 30;
+    double l0r = 0.0, l0i = 0.0, l1r = 0.0, l1i = 0.0;
+    for (int k = 0; k < N; k++) {
+        if (k > 0 && wp == (k - 1) % NW) {
+            if (k0 < 0) { Ar[i0 + (k - 1) * N] = l0r; Ai[i0 + (k - 1) * N] = l0i; }
+            if (k1 < 0) { Ar[i1 + (k - 1) * N] = l1r; Ai[i1 + (k - 1) * N] = l1i; }
+        }
+        const double a0r = (k0 < 0) ? Ar[i0 + k * N] : 0.0, a0i = (k0 < 0) ? Ai[i0 + k * N] : 0.0;
+        const double a1r = (k1 < 0) ? Ar[i1 + k * N] : 0.0, a1i = (k1 < 0) ? Ai[i1 + k * N] : 0.0;
+        const double v0 = (k0 < 0) ? fabs(a0r) + fabs(a0i) : -1.0, v1 = (k1 < 0) ? fabs(a1r) + fabs(a1i) : -1.0;
+        const int p = warp_argmax_row(v1 > v0 ? v1 : v0, v1 > v0 ? i1 : i0);
+        const double pr = (p >= 0) ? Ar[p + k * N] : 0.0, pi = (p >= 0) ? Ai[p + k * N] : 0.0;
+        const double den = rcp_nr(pr * pr + pi * pi);
+        if (p < 0 || !isfinite(den)) return k + 1;
+        const double qr = pr * den, qi = -pi * den;       // 1 / pivot
+        if (i0 == p) k0 = k;
+        if (i1 == p) k1 = k;
+        if (lane == 0) { x.perm[k] = p; x.rdr[k] = qr; x.rdi[k] = qi; x.rowk[p] = k; }
+        l0r = (k0 < 0) ? a0r * qr - a0i * qi : 0.0; l0i = (k0 < 0) ? a0r * qi + a0i * qr : 0.0;
+        l1r = (k1 < 0) ? a1r * qr - a1i * qi : 0.0; l1i = (k1 < 0) ? a1r * qi + a1i * qr : 0.0;
+        for (int j = k + 1 + ((wp - (k + 1)) % NW + NW) % NW; j < N; j += NW) {
+            const double ur = Ar[p + j * N], ui = Ai[p + j * N];
+            if (k0 < 0) {
+                Ar[i0 + j * N] = fma(-l0r, ur, fma(l0i, ui, Ar[i0 + j * N]));
+                Ai[i0 + j * N] = fma(-l0r, ui, fma(-l0i, ur, Ai[i0 + j * N]));
+            }
+            if (k1 < 0) {
+                Ar[i1 + j * N] = fma(-l1r, ur, fma(l1i, ui, Ar[i1 + j * N]));
+                Ai[i1 + j * N] = fma(-l1r, ui, fma(-l1i, ur, Ai[i1 + j * N]));
+            }
+        }
+        Grp<G>::sync();
+    }
+    return 0;
+}
+
+// Solves with the lu2 factors by ONE warp: b (shared, length N, original row order) is overwritten by x.
+__device__ __forceinline__ void solve2_real_warp(int N, const double *A, const Lu2Aux &x, double *b, int wl)
+{
+    const int i0 = wl, i1 = wl + 32;
+    const int k0 = (i0 < N) ? x.rowk[i0] : -1, k1 = (i1 < N) ? x.rowk[i1] : -1;   // -1: no such row (never updated)
+    double b0 = (i0 < N) ? b[i0] : 0.0, b1 = (i1 < N) ? b[i1] : 0.0;
+#pragma unroll 1
+    for (int k = 0; k < N - 1; k++) {
+        const int p = x.perm[k];
+        const double bk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31);
+        if (k0 > k) b0 = fma(-A[i0 + k * N], bk, b0);
+        if (k1 > k) b1 = fma(-A[i1 + k * N], bk, b1);
+    }
+    __syncwarp();
+#pragma unroll 1
+    for (int k = N - 1; k >= 0; k--) {
+        const int p = x.perm[k];
+        const double xk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31) * x.rdr[k];
+        if (k0 >= 0 && k0 < k) b0 = fma(-A[i0 + k * N], xk, b0);
+        if (k1 >= 0 && k1 < k) b1 = fma(-A[i1 + k * N], xk, b1);
+        if (wl == 0) b[k] = xk;
+    }
+    __syncwarp();
+}
+__device__ __forceinline__ void solve2_complex_warp(int N, const double *Ar, const double *Ai, const Lu2Aux &x, double *br,
+                                                    double *bi, int wl)
+{
+    const int i0 = wl, i1 = wl + 32;
+    const int k0 = (i0 < N) ? x.rowk[i0] : -1, k1 = (i1 < N) ? x.rowk[i1] : -1;
+    double b0r = (i0 < N) ? br[i0] : 0.0, b0i = (i0 < N) ? bi[i0] : 0.0;
+    double b1r = (i1 < N) ? br[i1] : 0.0, b1i = (i1 < N) ? bi[i1] : 0.0;
+#pragma unroll 1
+    for (int k = 0; k < N - 1; k++) {
+        const int p = x.perm[k];
+        const double xr = __shfl_sync(0xffffffffu, (p & 32) ? b1r : b0r, p & 31);
+        const double xi = __shfl_sync(0xffffffffu, (p & 32) ? b1i : b0i, p & 31);
+        if (k0 > k) {
+            const double lr = Ar[i0 + k * N], li = Ai[i0 + k * N];
+            b0r = fma(-lr, xr, fma(li, xi, b0r));
+            b0i = fma(-lr, xi, fma(-li, xr, b0i));
+        }
+        if (k1 > k) {
+            const double lr = Ar[i1 + k * N], li = Ai[i1 + k * N];
+            b1r = fma(-lr, xr, fma(li, xi, b1r));
+            b1i = fma(-lr, xi, fma(-li, xr, b1i));
+        }
+    }
+    __syncwarp();
+#pragma unroll 1
+    for (int k = N - 1; k >= 0; k--) {
+        const int p = x.perm[k];
+        const double vr = __shfl_sync(0xffffffffu, (p & 32) ? b1r : b0r, p & 31);
+        const double vi = __shfl_sync(0xffffffffu, (p & 32) ? b1i : b0i, p & 31);
+        const double qr = x.rdr[k], qi = x.rdi[k];
+        const double xr = vr * qr - vi * qi, xi = vr * qi + vi * qr;
+        if (k0 >= 0 && k0 < k) {
+            const double ur = Ar[i0 + k * N], ui = Ai[i0 + k * N];
+            b0r = fma(-ur, xr, fma(ui, xi, b0r));
+            b0i = fma(-ur, xi, fma(-ui, xr, b0i));
+        }
+        if (k1 >= 0 && k1 < k) {
+            const double ur = Ar[i1 + k * N], ui = Ai[i1 + k * N];
+            b1r = fma(-ur, xr, fma(ui, xi, b1r));
+            b1i = fma(-ur, xi, fma(-ui, xr, b1i));
+        }
+        if (wl == 0) { br[k] = xr; bi[k] = xi; }
+    }
+    __syncwarp();
+}
+template <int G>
+__device__ __noinline__ void solve2_pair(int N, const double *E1, const Lu2Aux &x1, double *z1, const double *E2r,
+                                         const double *E2i, const Lu2Aux &x2, double *z2, double *z3)
+{
+    if (G == 32) {
+        solve2_real_warp(N, E1, x1, z1, Grp<G>::wlane());
+        solve2_complex_warp(N, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
+    } else {
+        if (Grp<G>::warp() == 0) solve2_real_warp(N, E1, x1, z1, Grp<G>::wlane());
+        else if (Grp<G>::warp() == 1) solve2_complex_warp(N, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
+    }
+    Grp<G>::sync();
+}
+template <int G>
+__device__ __noinline__ void solve2_real(int N, const double *E1, const Lu2Aux &x1, double *b)
+{
+    if (Grp<G>::warp() == 0) solve2_real_warp(N, E1, x1, b, Grp<G>::wlane());
+    Grp<G>::sync();
+}
+
 // Solves by ONE warp (lanes wl = 0..31) on shared vectors; P b first, then L, then U (column sweeps).
 __device__ __forceinline__ void solve_real_warp(int N, const double *A, const int *ip, double *b, int wl)
 {

@@ -32,6 +32,7 @@ struct Work {
     double *y, *f0, *scal, *z1, *z2, *z3, *w1, *w2, *w3, *c1, *c2, *c3, *ys, *a1, *a2, *a3;  // [N] each
     double *Jm, *E1, *E2r, *E2i;                                                             // [N*N] each
     int *ip1, *ip2;                                                                          // [N]
+    Lu2Aux x1, x2;                                                                           // lu2 bookkeeping (N <= 64)
     ChemScratch cs;
 };
 
@@ -39,7 +40,7 @@ __host__ __device__ inline size_t work_doubles(int N, int NR, int NW)
 {
     const size_t e2 = (size_t)2 * N * N > (size_t)8 * NR ? (size_t)2 * N * N : (size_t)8 * NR;
     // 16 vectors + 6 chem vectors + q + Jm + E1 + E2 region + red + 2 int vectors (N ints each -> N doubles total)
-    return (size_t)22 * N + NR + (size_t)2 * N * N + e2 + 2 * NW + N + 2;
+    return (size_t)22 * N + NR + (size_t)2 * N * N + e2 + 2 * NW + N + 2 + 3 * N + N + 2;   // + rd1, rd2r, rd2i, rowk1/2
 }
 
 __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW)
@@ -61,8 +62,12 @@ __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW)
     w.E2r = r; w.E2i = r + (size_t)N * N;
     w.cs.dq = r; w.cs.dqdT = r + (size_t)6 * NR; w.cs.tb = r + (size_t)7 * NR;   // alive only inside jacobian()
     w.cs.red = take(2 * NW);
-    w.ip1 = reinterpret_cast<int *>(take((N + 1) / 2 + 1));
+    w.ip1 = reinterpret_cast<int *>(take(N + 2));                  // 2 N ints
     w.ip2 = w.ip1 + N;
+    w.x1.perm = w.ip1; w.x2.perm = w.ip2;
+    w.x1.rdr = take(N); w.x1.rdi = nullptr; w.x2.rdr = take(N); w.x2.rdi = take(N);
+    w.x1.rowk = reinterpret_cast<int *>(take(N + 2));
+    w.x2.rowk = w.x1.rowk + N;
     return w;
 }
 
@@ -138,8 +143,13 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
                 }
             int ier = Grp<G>::any(nonfinite, w.cs.red);   // includes the barrier after the stores
             if (G == 32) __syncwarp();
-            if (!ier) ier = lu_real<G>(N, w.E1, w.ip1);
-            if (!ier) ier = lu_complex<G>(N, w.E2r, w.E2i, w.ip2);
+            if (N <= 64) {
+                if (!ier) ier = lu2_real<G>(N, w.E1, w.x1);
+                if (!ier) ier = lu2_complex<G>(N, w.E2r, w.E2i, w.x2);
+            } else {
+                if (!ier) ier = lu_real<G>(N, w.E1, w.ip1);
+                if (!ier) ier = lu_complex<G>(N, w.E2r, w.E2i, w.ip2);
+            }
             Grp<G>::sync();
             st.ndec++;
             if (ier) {
@@ -198,7 +208,8 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
                 w.z3[i] = TI31 * a1 + TI32 * a2 + TI33 * a3 - f3 * ALPHN - f2 * BETAN;
             }
             Grp<G>::sync();
-            solve_pair<G>(N, w.E1, w.ip1, w.z1, w.E2r, w.E2i, w.ip2, w.z2, w.z3);
+            if (N <= 64) solve2_pair<G>(N, w.E1, w.x1, w.z1, w.E2r, w.E2i, w.x2, w.z2, w.z3);
+            else solve_pair<G>(N, w.E1, w.ip1, w.z1, w.E2r, w.E2i, w.ip2, w.z2, w.z3);
             st.nsol++;
             NEWT++;
             double dy = 0.0, dummy = 0.0;
@@ -256,7 +267,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
                 w.a1[i] = f2 + w.f0[i];
             }
             Grp<G>::sync();
-            solve_real<G>(N, w.E1, w.ip1, w.a1);
+            if (N <= 64) solve2_real<G>(N, w.E1, w.x1, w.a1); else solve_real<G>(N, w.E1, w.ip1, w.a1);
             double e = 0.0, dummy = 0.0;
             for (int i = lane; i < N; i += G) { const double r = w.a1[i] / w.scal[i]; e += r * r; }
             Grp<G>::sum2(e, dummy, w.cs.red);
@@ -268,7 +279,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
                 st.nfcn++;
                 for (int i = lane; i < N; i += G) w.a1[i] = w.a3[i] + w.a2[i];
                 Grp<G>::sync();
-                solve_real<G>(N, w.E1, w.ip1, w.a1);
+                if (N <= 64) solve2_real<G>(N, w.E1, w.x1, w.a1); else solve_real<G>(N, w.E1, w.ip1, w.a1);
                 e = 0.0; dummy = 0.0;
                 for (int i = lane; i < N; i += G) { const double r = w.a1[i] / w.scal[i]; e += r * r; }
                 Grp<G>::sum2(e, dummy, w.cs.red);
