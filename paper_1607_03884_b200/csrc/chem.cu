@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
@@ -81,25 +82,34 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     std::vector<double> lnA(nr), b(nr), Ta(nr), lnA0(nr, 0.0), b0(nr, 0.0), Ta0(nr, 0.0), dnu(nr), troe(4 * nr, 1.0), eff_dv;
     std::vector<std::vector<std::pair<int, double>>> inc(ns);
     long n_slots_used = 0, n_eff = 0, n_fall = 0, n_troe = 0, n_tb = 0;
+    // Table order: reactions sorted by type (elementary, three-body, Lindemann, Troe; stable), so that the lanes of a
+    // warp that evaluate 32 consecutive reactions follow the same branch (falloff work is not paid by every warp).
+    std::vector<int> order(nr);
     for (int i = 0; i < nr; i++) {
-        const int ty = d->rxn_type[i];
+        if (d->rxn_type[i] < 0 || d->rxn_type[i] > 3) return fail(CHEM_E_ARG, "reaction %d: unknown type %d", i, d->rxn_type[i]);
+        order[i] = i;
+    }
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return d->rxn_type[x] < d->rxn_type[y]; });
+    for (int i = 0; i < nr; i++) {
+        const int si = order[i];              // source reaction of table slot i
+        const int ty = d->rxn_type[si];
         if (ty < 0 || ty > 3) return fail(CHEM_E_ARG, "reaction %d: unknown type %d", i, ty);
         rtype[i] = ty;
-        if (!(d->arr_A[i] > 0.0)) return fail(CHEM_E_ARG, "reaction %d: A must be positive", i);
-        lnA[i] = std::log(d->arr_A[i]);
-        b[i] = d->arr_b[i];
-        Ta[i] = d->arr_Ea[i] / kRcal;
+        if (!(d->arr_A[si] > 0.0)) return fail(CHEM_E_ARG, "reaction %d: A must be positive", i);
+        lnA[i] = std::log(d->arr_A[si]);
+        b[i] = d->arr_b[si];
+        Ta[i] = d->arr_Ea[si] / kRcal;
         if (ty >= 2) {
-            if (!d->low_A || !d->low_b || !d->low_Ea || !(d->low_A[i] > 0.0))
+            if (!d->low_A || !d->low_b || !d->low_Ea || !(d->low_A[si] > 0.0))
                 return fail(CHEM_E_ARG, "reaction %d: falloff needs a positive low-pressure A", i);
-            lnA0[i] = std::log(d->low_A[i]);
-            b0[i] = d->low_b[i];
-            Ta0[i] = d->low_Ea[i] / kRcal;
+            lnA0[i] = std::log(d->low_A[si]);
+            b0[i] = d->low_b[si];
+            Ta0[i] = d->low_Ea[si] / kRcal;
             n_fall++;
         }
         if (ty == 3) {
             if (!d->troe) return fail(CHEM_E_ARG, "reaction %d: Troe parameters missing", i);
-            for (int c = 0; c < 4; c++) troe[c * nr + i] = d->troe[4 * i + c];
+            for (int c = 0; c < 4; c++) troe[c * nr + i] = d->troe[4 * si + c];
             if (troe[nr + i] == 0.0 || troe[2 * nr + i] == 0.0) return fail(CHEM_E_ARG, "reaction %d: Troe T*** or T* is zero", i);
             n_troe++;
         }
@@ -108,10 +118,10 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
         double dn = 0.0;
         for (int side = 0; side < 2; side++) {
             const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr, *sp = side ? d->prod_sp : d->reac_sp, *nu = side ? d->prod_nu : d->reac_nu;
-            const int n = ptr[i + 1] - ptr[i];
+            const int n = ptr[si + 1] - ptr[si];
             if (n < 1 || n > 3) return fail(CHEM_E_UNSUPPORTED, "reaction %d: %d species on one side (1..3 supported)", i, n);
             for (int p = 0; p < n; p++) {
-                const int k = sp[ptr[i] + p], v = nu[ptr[i] + p];
+                const int k = sp[ptr[si] + p], v = nu[ptr[si] + p];
                 if (k < 0 || k >= ns) return fail(CHEM_E_ARG, "reaction %d: species index %d out of range", i, k);
                 if (v < 1 || v > 3) return fail(CHEM_E_UNSUPPORTED, "reaction %d: stoichiometric coefficient %d (1..3 supported)", i, v);
                 slot_sp[(side * 3 + p) * nr + i] = k;
@@ -125,8 +135,8 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
         for (int k = 0; k < ns; k++)
             if (net[k] != 0.0) inc[k].push_back({i, net[k]});
         if (ty != 0) {
-            if (d->eff_ptr[i + 1] < d->eff_ptr[i]) return fail(CHEM_E_ARG, "eff_ptr not monotone");
-            for (int p = d->eff_ptr[i]; p < d->eff_ptr[i + 1]; p++) {
+            if (d->eff_ptr[si + 1] < d->eff_ptr[si]) return fail(CHEM_E_ARG, "eff_ptr not monotone");
+            for (int p = d->eff_ptr[si]; p < d->eff_ptr[si + 1]; p++) {
                 if (!d->eff_sp || !d->eff_val) return fail(CHEM_E_ARG, "efficiency arrays missing");
                 const int k = d->eff_sp[p];
                 if (k < 0 || k >= ns) return fail(CHEM_E_ARG, "reaction %d: efficiency species out of range", i);
