@@ -156,6 +156,80 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     if (eff_sp.empty()) { eff_sp.push_back(0); eff_dv.push_back(0.0); }
     if (inc_rx.empty()) { inc_rx.push_back(0); inc_nu.push_back(0.0); }
 
+    // ---- exp-job tables for the stage-batched source term of the group kernels (chem_cta.cuh); same idea as
+    // chem_fast.inl: k_f, k_r (ln K_c folded in from the NASA coefficients), k_0/k_inf and the three Troe terms are all
+    // exp(c0 + c1 lnT + c2/T + c3 T + c4 T^2 + c5 T^3 + c6 T^4).  Job order: [0,nr) k_f, [nr,2nr) k_r, then extras.
+    // Eligible when: one common T_mid, <= 63 species, at most three concentration factors per side, 0 < alpha < 1.
+    std::vector<double> job_lo, job_hi;
+    std::vector<int> rdesc(8 * nr, 0);
+    int n_fo = 0, n_jobs = 0, jobs_ok = (ns <= 63);
+    for (int k = 1; k < ns; k++) jobs_ok &= (tmid[k] == tmid[0]);
+    if (jobs_ok) {
+        n_jobs = 2 * nr;
+        for (int i = 0; i < nr; i++) n_jobs += (rtype[i] >= 2) + 3 * (rtype[i] == 3);
+        job_lo.assign((size_t)n_jobs * 8, 0.0);
+        job_hi.assign((size_t)n_jobs * 8, 0.0);
+        const double lnPR = std::log(kPatm / kRerg);
+        int next_extra = 2 * nr;
+        for (int i = 0; i < nr && jobs_ok; i++) {
+            int f[6] = {63, 63, 63, 63, 63, 63};
+            for (int side = 0; side < 2; side++) {
+                int sl = 3 * side;
+                for (int p = 0; p < 3; p++)
+                    for (int rep = 0; rep < slot_nu[(3 * side + p) * nr + i]; rep++) {
+                        if (sl >= 3 * side + 3) { jobs_ok = 0; break; }
+                        f[sl++] = slot_sp[(3 * side + p) * nr + i];
+                    }
+            }
+            rdesc[8 * i + 0] = f[0] | (f[1] << 8) | (f[2] << 16);
+            rdesc[8 * i + 1] = f[3] | (f[4] << 8) | (f[5] << 16);
+            rdesc[8 * i + 2] = rtype[i];
+            rdesc[8 * i + 5] = eff_ptr[i];
+            rdesc[8 * i + 6] = eff_ptr[i + 1];
+            for (int r = 0; r < 2; r++) {
+                std::vector<double> &job = r ? job_hi : job_lo;
+                const std::vector<double> &na = r ? hi : lo;     // coefficient-major [7][ns]
+                double *kf = &job[(size_t)i * 8], *kr = &job[(size_t)(nr + i) * 8];
+                kf[0] = lnA[i]; kf[1] = b[i]; kf[2] = -Ta[i];
+                double g[7] = {0, 0, 0, 0, 0, 0, 0};
+                for (int sl = 0; sl < 6; sl++) {
+                    const double v = (sl < 3 ? -1.0 : 1.0) * slot_nu[sl * nr + i];
+                    const int k = slot_sp[sl * nr + i];
+                    if (v == 0.0) continue;
+                    g[0] += v * (na[0 * ns + k] - na[6 * ns + k]);
+                    g[1] += v * (-na[0 * ns + k]);
+                    g[2] += v * na[5 * ns + k];
+                    g[3] += v * (-na[1 * ns + k] / 2.0);
+                    g[4] += v * (-na[2 * ns + k] / 6.0);
+                    g[5] += v * (-na[3 * ns + k] / 12.0);
+                    g[6] += v * (-na[4 * ns + k] / 20.0);
+                }
+                kr[0] = lnA[i] - dnu[i] * lnPR + g[0];
+                kr[1] = b[i] + dnu[i] + g[1];
+                kr[2] = -Ta[i] + g[2];
+                kr[3] = g[3]; kr[4] = g[4]; kr[5] = g[5]; kr[6] = g[6];
+                if (rtype[i] >= 2) {
+                    double *c = &job[(size_t)next_extra * 8];
+                    c[0] = lnA0[i] - lnA[i]; c[1] = b0[i] - b[i]; c[2] = -(Ta0[i] - Ta[i]);
+                }
+                if (rtype[i] == 3) {
+                    const double al = troe[i], T3 = troe[nr + i], T1 = troe[2 * nr + i], T2 = troe[3 * nr + i];
+                    if (!(al > 0.0 && al < 1.0)) { jobs_ok = 0; break; }
+                    double *c = &job[(size_t)(next_extra + 1) * 8];
+                    c[0] = std::log(1.0 - al); c[3] = -1.0 / T3;
+                    c[8] = std::log(al); c[8 + 3] = -1.0 / T1;
+                    c[16 + 2] = -T2;
+                }
+            }
+            if (rtype[i] >= 2) {
+                rdesc[8 * i + 3] = next_extra;          // k0/kinf job; Troe terms follow at +1..+3
+                rdesc[8 * i + 4] = n_fo++;              // falloff ordinal
+                next_extra += 1 + 3 * (rtype[i] == 3);
+            }
+        }
+    }
+    if (!jobs_ok) { job_lo.assign(8, 0.0); job_hi.assign(8, 0.0); n_jobs = 0; n_fo = 0; }
+
     int dev = 0, n_sm = 0, optin = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
@@ -174,9 +248,10 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     add(lnA.data(), nr * 8); add(b.data(), nr * 8); add(Ta.data(), nr * 8); add(lnA0.data(), nr * 8); add(b0.data(), nr * 8);
     add(Ta0.data(), nr * 8); add(dnu.data(), nr * 8); add(troe.data(), 4 * nr * 8);
     add(eff_dv.data(), eff_dv.size() * 8); add(inc_nu.data(), inc_nu.size() * 8);
+    add(job_lo.data(), job_lo.size() * 8); add(job_hi.data(), job_hi.size() * 8);
     add(rtype.data(), nr * 4); add(slot_sp.data(), 6 * nr * 4); add(slot_nu.data(), 6 * nr * 4);
     add(eff_ptr.data(), (nr + 1) * 4); add(eff_sp.data(), eff_sp.size() * 4);
-    add(inc_ptr.data(), (ns + 1) * 4); add(inc_rx.data(), inc_rx.size() * 4);
+    add(inc_ptr.data(), (ns + 1) * 4); add(inc_rx.data(), inc_rx.size() * 4); add(rdesc.data(), rdesc.size() * 4);
     std::vector<char> host(total, 0);
     for (size_t a = 0; a < parts.size(); a++) std::memcpy(host.data() + offs[a], parts[a].first, parts[a].second);
 
@@ -202,8 +277,9 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     t.n_sp = ns; t.n_rx = nr;
     t.W = D(); t.invW = D(); t.nasa_lo = D(); t.nasa_hi = D(); t.tmid = D();
     t.lnA = D(); t.b = D(); t.Ta = D(); t.lnA0 = D(); t.b0 = D(); t.Ta0 = D(); t.dnu = D(); t.troe = D();
-    t.eff_dv = D(); t.inc_nu = D();
-    t.rtype = I(); t.slot_sp = I(); t.slot_nu = I(); t.eff_ptr = I(); t.eff_sp = I(); t.inc_ptr = I(); t.inc_rx = I();
+    t.eff_dv = D(); t.inc_nu = D(); t.job_lo = D(); t.job_hi = D();
+    t.rtype = I(); t.slot_sp = I(); t.slot_nu = I(); t.eff_ptr = I(); t.eff_sp = I(); t.inc_ptr = I(); t.inc_rx = I(); t.rdesc = I();
+    t.n_jobs = n_jobs; t.n_fo = n_fo; t.tmid0 = tmid[0];
     m->n_sm = n_sm;
     m->max_smem_optin = optin;
 

@@ -1,0 +1,186 @@
+// chem_cta.cuh -- stage-batched source term for the group kernels (G = 32 or 128 threads per state), built on the
+// exp-job tables of the mechanism compiler (chem.cu): the three Radau stage states of one Newton iteration are
+// evaluated in one pass, every rate constant is one exp of a 7-term form in T, the Troe broadening
+// factors of all (falloff reaction, stage) pairs are computed side by side by separate threads.
+// Same mathematics as rhs<G>() (R1-R5).
+#pragma once
+#include "chem_device.cuh"
+
+namespace chem {
+
+// extra shared scratch of the batched source term (doubles): ys2, ys3, C3[3][64], X0[3][8], X[3][n_fo][4], q3[3][NR], red6[6 NW]
+__host__ __device__ inline size_t cta_extra_doubles(int N, int NR, int n_fo, int NW)
+{
+    // (C3 shares the six chemistry vectors of the Jacobian routine, q3 extends its q: see carve())
+    return (size_t)2 * N + (6 * N < 192 ? 192 - 6 * N : 0) + 24 + (size_t)12 * (n_fo > 0 ? n_fo : 1) + (size_t)2 * NR + 6 * NW + 2;
+}
+
+struct CtaScratch {
+    double *ys2, *ys3;   // stage states 2, 3 (stage 1 is Work::ys)
+    double *C3;          // [3][64], C3[s][63] = 1 (unity factor)
+    double *X0;          // [3][8]: T, lnT, 1/T, rho, 1/rho, Ctot
+    double *X;           // [3][n_fo][4]: Fcent, Pr, rnet, reaction index
+    double *q3;          // [3][NR]
+    double *red6;        // [6][NW]
+};
+
+__device__ __forceinline__ double cta_rcp(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+
+// block all-reduce of six sums (deterministic: fixed butterfly, then warps in order)
+template <int G>
+__device__ __forceinline__ void sum6(double (&v)[6], double *red6)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int c = 0; c < 6; c++) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+    if (G > 32) {
+        __syncthreads();
+        if (Grp<G>::wlane() == 0)
+#pragma unroll
+            for (int c = 0; c < 6; c++) red6[c * Grp<G>::NW + Grp<G>::warp()] = v[c];
+        __syncthreads();
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+            double a = 0.0;
+#pragma unroll
+            for (int wv = 0; wv < Grp<G>::NW; wv++) a += red6[c * Grp<G>::NW + wv];
+            v[c] = a;
+        }
+    }
+}
+
+__device__ __forceinline__ double job_val(const double *c, double T, double lnT, double invT)
+{
+    const double2 c01 = __ldg(reinterpret_cast<const double2 *>(c)), c23 = __ldg(reinterpret_cast<const double2 *>(c) + 1);
+    const double2 c45 = __ldg(reinterpret_cast<const double2 *>(c) + 2), c67 = __ldg(reinterpret_cast<const double2 *>(c) + 3);
+    return exp(c01.x + c01.y * lnT + c23.x * invT + T * (c23.y + T * (c45.x + T * (c45.y + T * c67.x))));
+}
+
+// Inputs: stage states ys[0..2] (shared, length N); outputs f[0..2] (shared, length N).  nstage = 1 or 3.
+template <int G>
+__device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, const CtaScratch &x, double P, int nstage,
+                                      const double *ys0, double *f0, double *f1, double *f2)
+{
+    const int N = t.n_sp, NR = t.n_rx, nfo = t.n_fo;
+    const int lane = Grp<G>::lane();
+    const double *ys[3] = {ys0, x.ys2, x.ys3};
+    double *fo[3] = {f0, f1, f2};
+    // ---- mixture: closure, Wbar, rho, concentrations
+    double v[6] = {0, 0, 0, 0, 0, 0};
+    for (int k = lane; k < N - 1; k += G) {
+        const double iw = __ldg(&t.invW[k]);
+#pragma unroll
+        for (int s = 0; s < 3; s++)
+            if (s < nstage) { const double Yk = ys[s][k + 1]; v[2 * s] += Yk; v[2 * s + 1] += Yk * iw; }
+    }
+    sum6<G>(v, x.red6);
+    if (lane < nstage) {
+        const int s = lane;
+        const double T = (s == 0 ? ys0 : (s == 1 ? x.ys2 : x.ys3))[0];
+        const double vY = s == 0 ? v[0] : (s == 1 ? v[2] : v[4]), vW = s == 0 ? v[1] : (s == 1 ? v[3] : v[5]);
+        const double YN = 1.0 - vY;
+        const double sW = vW + YN * __ldg(&t.invW[N - 1]);
+        const double invT = 1.0 / T, rho = P / (kRerg * T * sW);
+        double *o = x.X0 + 8 * s;
+        o[0] = T; o[1] = log(T); o[2] = invT; o[3] = rho; o[4] = kRerg * T * sW / P; o[5] = P * invT * (1.0 / kRerg);
+        x.C3[64 * s + N - 1] = rho * YN * __ldg(&t.invW[N - 1]);
+        x.C3[64 * s + 63] = 1.0;
+    }
+    Grp<G>::sync();
+    for (int k = lane; k < N - 1; k += G) {
+        const double iw = __ldg(&t.invW[k]);
+#pragma unroll
+        for (int s = 0; s < 3; s++)
+            if (s < nstage) x.C3[64 * s + k] = x.X0[8 * s + 3] * ys[s][k + 1] * iw;
+    }
+    Grp<G>::sync();
+    // ---- rates of progress: each thread owns reactions lane, lane + G, ...; all exps of a reaction in its thread
+    for (int i = lane; i < NR; i += G) {
+        const int4 d0 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i);       // f012, f345, type, extra job
+        const int4 d1 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i + 1);   // falloff ordinal, eff_lo, eff_hi
+        const int type = d0.z;
+#pragma unroll 1
+        for (int s = 0; s < nstage; s++) {
+            const double T = x.X0[8 * s], lnT = x.X0[8 * s + 1], invT = x.X0[8 * s + 2];
+            const double *jt = (T <= t.tmid0) ? t.job_lo : t.job_hi;
+            const double *C = x.C3 + 64 * s;
+            const double kf = job_val(jt + (size_t)i * 8, T, lnT, invT), kr = job_val(jt + (size_t)(NR + i) * 8, T, lnT, invT);
+            const double Rf = kf * (C[d0.x & 255] * C[(d0.x >> 8) & 255] * C[(d0.x >> 16) & 255]);
+            const double Rr = kr * (C[d0.y & 255] * C[(d0.y >> 8) & 255] * C[(d0.y >> 16) & 255]);
+            const double rnet = Rf - Rr;
+            double c = 1.0;
+            if (type != 0) {
+                double M = x.X0[8 * s + 5];
+                for (int p = d1.y; p < d1.z; p++) M += __ldg(&t.eff_dv[p]) * C[__ldg(&t.eff_sp[p])];
+                c = M;
+                if (type >= 2) {
+                    const double Pr = job_val(jt + (size_t)d0.w * 8, T, lnT, invT) * M;
+                    double Fc = 1.0;
+                    if (type == 3)
+                        Fc = job_val(jt + (size_t)(d0.w + 1) * 8, T, lnT, invT) + job_val(jt + (size_t)(d0.w + 2) * 8, T, lnT, invT) +
+                             job_val(jt + (size_t)(d0.w + 3) * 8, T, lnT, invT);
+                    double *o = x.X + (size_t)(s * nfo + d1.x) * 4;
+                    o[0] = Fc; o[1] = Pr; o[2] = rnet; o[3] = (double)i;
+                }
+            }
+            if (type < 2) x.q3[s * NR + i] = c * rnet;
+        }
+    }
+    Grp<G>::sync();
+    // ---- falloff pairs (reaction, stage): c = Pr/(1+Pr) F, one thread each (R5)
+    for (int p = lane; p < nstage * nfo; p += G) {
+        const double *o = x.X + (size_t)p * 4;
+        const double Fc = o[0], Pr = o[1];
+        const double L = log10(Fc);
+        const double At = log10(Pr) - 0.4 - 0.67 * L;
+        const double xx = At * cta_rcp(0.75 - 1.27 * L - 0.14 * At);
+        const double F = exp10(L * cta_rcp(1.0 + xx * xx));
+        const int s = p / nfo;
+        x.q3[s * NR + (int)o[3]] = Pr * cta_rcp(1.0 + Pr) * F * o[2];
+    }
+    Grp<G>::sync();
+    // ---- species production rates, temperature equation
+    double r6[6] = {0, 0, 0, 0, 0, 0};
+    for (int k = lane; k < N; k += G) {
+        double w[3] = {0.0, 0.0, 0.0};
+        for (int p = __ldg(&t.inc_ptr[k]); p < __ldg(&t.inc_ptr[k + 1]); p++) {
+            const double nu = __ldg(&t.inc_nu[p]);
+            const int i = __ldg(&t.inc_rx[p]);
+#pragma unroll
+            for (int s = 0; s < 3; s++)
+                if (s < nstage) w[s] += nu * x.q3[s * NR + i];
+        }
+        const double Wk = __ldg(&t.W[k]);
+#pragma unroll
+        for (int s = 0; s < 3; s++)
+            if (s < nstage) {
+                const double T = x.X0[8 * s], invT = x.X0[8 * s + 2];
+                const double *a = (T <= t.tmid0) ? t.nasa_lo : t.nasa_hi;
+                const double a0 = __ldg(&a[k]), a1 = __ldg(&a[N + k]), a2 = __ldg(&a[2 * N + k]), a3 = __ldg(&a[3 * N + k]);
+                const double a4 = __ldg(&a[4 * N + k]), a5 = __ldg(&a[5 * N + k]);
+                const double cpR = a0 + T * (a1 + T * (a2 + T * (a3 + T * a4)));
+                const double hRT = a0 + T * (a1 * 0.5 + T * (a2 * (1.0 / 3.0) + T * (a3 * 0.25 + T * (a4 * 0.2)))) + a5 * invT;
+                r6[2 * s] += hRT * w[s];
+                r6[2 * s + 1] += x.C3[64 * s + k] * cpR;
+                if (k < N - 1) fo[s][k + 1] = Wk * w[s] * x.X0[8 * s + 4];
+            }
+    }
+    sum6<G>(r6, x.red6);
+    if (lane < nstage) {
+        const double hw = lane == 0 ? r6[0] : (lane == 1 ? r6[2] : r6[4]), ccp = lane == 0 ? r6[1] : (lane == 1 ? r6[3] : r6[5]);
+        (lane == 0 ? f0 : (lane == 1 ? f1 : f2))[0] = -x.X0[8 * lane] * hw / ccp;
+    }
+    Grp<G>::sync();
+    (void)cs;
+}
+
+}  // namespace chem

@@ -34,6 +34,11 @@ struct Tables {
     const double *eff_dv;             // alpha - 1
     const int *inc_ptr, *inc_rx;      // CSR over species: reactions the species takes part in
     const double *inc_nu;             // net stoichiometric coefficient nu'' - nu'
+    // exp-job form of the rate constants (chem_cta.cuh); n_jobs == 0: not available for this mechanism
+    const double *job_lo, *job_hi;    // [n_jobs][8]: k_f [0,n_rx), k_r [n_rx,2 n_rx), then k_0/k_inf and Troe terms
+    const int *rdesc;                 // [n_rx][8]: factors 0-2 (8 bits each, 63 = unity), factors 3-5, type, extra job, falloff ordinal, eff_lo, eff_hi, 0
+    int n_jobs, n_fo;
+    double tmid0;
 };
 
 // ---------------------------------------------------------------------------------------------

@@ -37,8 +37,8 @@ __global__ void __launch_bounds__(kBlock) integrate_kernel(Tables t, int n_state
     extern __shared__ double smem[];
     __shared__ int bcast;
     const int N = t.n_sp, NR = t.n_rx;
-    const size_t wd = work_doubles(N, NR, Grp<G>::NW);
-    Work w = carve(smem + (size_t)group_in_block<G>() * wd, N, NR, Grp<G>::NW);
+    const size_t wd = work_doubles(N, NR, Grp<G>::NW, t.n_fo);
+    Work w = carve(smem + (size_t)group_in_block<G>() * wd, N, NR, Grp<G>::NW, t.n_fo);
     const int lane = Grp<G>::lane();
     for (;;) {
         const int q = next_state<G>(counter, &bcast);
@@ -104,8 +104,8 @@ __global__ void __launch_bounds__(kBlock) eval_kernel(Tables t, int n_states, do
 {
     extern __shared__ double smem[];
     const int N = t.n_sp, NR = t.n_rx;
-    const size_t wd = work_doubles(N, NR, Grp<G>::NW);
-    Work w = carve(smem + (size_t)group_in_block<G>() * wd, N, NR, Grp<G>::NW);
+    const size_t wd = work_doubles(N, NR, Grp<G>::NW, t.n_fo);
+    Work w = carve(smem + (size_t)group_in_block<G>() * wd, N, NR, Grp<G>::NW, t.n_fo);
     const int lane = Grp<G>::lane();
     const int gpb = kBlock / G;
     for (int s = blockIdx.x * gpb + group_in_block<G>(); s < n_states; s += gridDim.x * gpb) {

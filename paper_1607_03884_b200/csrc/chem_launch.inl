@@ -21,7 +21,7 @@ int configure(K kernel, const chem_mech *m, size_t smem, int *ctas_per_sm)
 template <int G, bool JAC>
 int launch_eval(const chem_mech *m, int n, double P, const double *y, double *out, cudaStream_t st)
 {
-    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32) * sizeof(double) * (kBlock / G);
+    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (kBlock / G);
     int occ = 0;
     int rc = configure(eval_kernel<G, JAC>, m, smem, &occ);
     if (rc) return rc;
@@ -38,7 +38,7 @@ template <int G>
 int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
                      const chem_opts *o, chem_stats *stats, cudaStream_t st)
 {
-    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32) * sizeof(double) * (kBlock / G);
+    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (kBlock / G);
     int occ = 0;
     int rc = configure(integrate_kernel<G>, m, smem, &occ);
     if (rc) return rc;

@@ -6,7 +6,7 @@
 // [31] = Hairer & Wanner vol. II; the controller is the RADAU5 scheme described there, restated here
 // as a small state machine.  DESIGN.md R7..R12 list the constants and the order of the tests.
 #pragma once
-#include "chem_device.cuh"
+#include "chem_cta.cuh"
 
 namespace chem {
 
@@ -34,16 +34,17 @@ struct Work {
     int *ip1, *ip2;                                                                          // [N]
     Lu2Aux x1, x2;                                                                           // lu2 bookkeeping (N <= 64)
     ChemScratch cs;
+    CtaScratch cx;                                                                           // stage-batched source term
 };
 
-__host__ __device__ inline size_t work_doubles(int N, int NR, int NW)
+__host__ __device__ inline size_t work_doubles(int N, int NR, int NW, int n_fo = 0)
 {
     const size_t e2 = (size_t)2 * N * N > (size_t)8 * NR ? (size_t)2 * N * N : (size_t)8 * NR;
     // 16 vectors + 6 chem vectors + q + Jm + E1 + E2 region + red + 2 int vectors (N ints each -> N doubles total)
-    return (size_t)22 * N + NR + (size_t)2 * N * N + e2 + 2 * NW + N + 2 + 3 * N + N + 2;   // + rd1, rd2r, rd2i, rowk1/2
+    return (size_t)22 * N + NR + (size_t)2 * N * N + e2 + 2 * NW + N + 2 + 3 * N + N + 2 + cta_extra_doubles(N, NR, n_fo, NW);   // + rd1, rd2r, rd2i, rowk1/2, batched-rhs scratch
 }
 
-__device__ __forceinline__ Work carve(double *base, int N, int NR, int NW)
+__device__ __forceinline__ Work carve(double *base, int N, int NR, int NW, int n_fo = 0)
 {
     Work w;
     double *p = base;
@@ -54,7 +55,11 @@ __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW)
     w.c1 = take(N); w.c2 = take(N); w.c3 = take(N);
     w.ys = take(N); w.a1 = take(N); w.a2 = take(N); w.a3 = take(N);
     w.cs.C = take(N); w.cs.g = take(N); w.cs.hRT = take(N); w.cs.cpR = take(N); w.cs.dcpR = take(N); w.cs.wdot = take(N);
+    if (6 * N < 192) take(192 - 6 * N);
+    w.cx.C3 = w.cs.C;                 // [3][64]: the batched source term and the Jacobian routine never run concurrently
     w.cs.q = take(NR);
+    take((size_t)2 * NR);
+    w.cx.q3 = w.cs.q;                 // [3][NR]
     w.Jm = take((size_t)N * N);
     w.E1 = take((size_t)N * N);
     const size_t e2 = (size_t)2 * N * N > (size_t)8 * NR ? (size_t)2 * N * N : (size_t)8 * NR;
@@ -68,6 +73,10 @@ __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW)
     w.x1.rdr = take(N); w.x1.rdi = nullptr; w.x2.rdr = take(N); w.x2.rdi = take(N);
     w.x1.rowk = reinterpret_cast<int *>(take(N + 2));
     w.x2.rowk = w.x1.rowk + N;
+    w.cx.ys2 = take(N); w.cx.ys3 = take(N);
+    w.cx.X0 = take(24);
+    w.cx.X = take((size_t)12 * (n_fo > 0 ? n_fo : 1));
+    w.cx.red6 = take(6 * NW + 2);
     return w;
 }
 
@@ -118,7 +127,8 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
     int NSING = 0;
     for (int i = lane; i < N; i += G) w.scal[i] = ATOL + RTOL * fabs(w.y[i]);
     Grp<G>::sync();
-    rhs<G>(t, w.cs, P, w.y, w.f0);
+    const bool jobs = t.n_jobs > 0;
+    if (jobs) cta_rhs3<G>(t, w.cs, w.cx, P, 1, w.y, w.f0, w.a2, w.a3); else rhs<G>(t, w.cs, P, w.y, w.f0);
     st.nfcn++;
 
     enum { DO_JAC, DO_FACT, DO_STEP };
@@ -190,15 +200,24 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
         int outcome = 0;   // 0 converged, 1 shrink-and-retry with H already set, 2 unexpected rejection (H *= 0.5)
         for (;;) {
             if (NEWT >= NIT) { outcome = 2; break; }
-            for (int i = lane; i < N; i += G) w.ys[i] = w.y[i] + w.z1[i];
-            Grp<G>::sync();
-            rhs<G>(t, w.cs, P, w.ys, w.a1);
-            for (int i = lane; i < N; i += G) w.ys[i] = w.y[i] + w.z2[i];
-            Grp<G>::sync();
-            rhs<G>(t, w.cs, P, w.ys, w.a2);
-            for (int i = lane; i < N; i += G) w.ys[i] = w.y[i] + w.z3[i];
-            Grp<G>::sync();
-            rhs<G>(t, w.cs, P, w.ys, w.a3);
+            if (jobs) {
+                for (int i = lane; i < N; i += G) {
+                    const double yi = w.y[i];
+                    w.ys[i] = yi + w.z1[i]; w.cx.ys2[i] = yi + w.z2[i]; w.cx.ys3[i] = yi + w.z3[i];
+                }
+                Grp<G>::sync();
+                cta_rhs3<G>(t, w.cs, w.cx, P, 3, w.ys, w.a1, w.a2, w.a3);
+            } else {
+                for (int i = lane; i < N; i += G) w.ys[i] = w.y[i] + w.z1[i];
+                Grp<G>::sync();
+                rhs<G>(t, w.cs, P, w.ys, w.a1);
+                for (int i = lane; i < N; i += G) w.ys[i] = w.y[i] + w.z2[i];
+                Grp<G>::sync();
+                rhs<G>(t, w.cs, P, w.ys, w.a2);
+                for (int i = lane; i < N; i += G) w.ys[i] = w.y[i] + w.z3[i];
+                Grp<G>::sync();
+                rhs<G>(t, w.cs, P, w.ys, w.a3);
+            }
             st.nfcn += 3;
             for (int i = lane; i < N; i += G) {
                 const double a1 = w.a1[i], a2 = w.a2[i], a3 = w.a3[i];
@@ -275,7 +294,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
             if (ERR >= 1.0 && (FIRST || REJECT)) {
                 for (int i = lane; i < N; i += G) w.ys[i] = w.y[i] + w.a1[i];
                 Grp<G>::sync();
-                rhs<G>(t, w.cs, P, w.ys, w.a3);
+                if (jobs) cta_rhs3<G>(t, w.cs, w.cx, P, 1, w.ys, w.a3, w.z1, w.z2); else rhs<G>(t, w.cs, P, w.ys, w.a3);
                 st.nfcn++;
                 for (int i = lane; i < N; i += G) w.a1[i] = w.a3[i] + w.a2[i];
                 Grp<G>::sync();
@@ -322,7 +341,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
             Grp<G>::sync();
             CALJAC = false;
             if (LAST) return;
-            rhs<G>(t, w.cs, P, w.y, w.f0);
+            if (jobs) cta_rhs3<G>(t, w.cs, w.cx, P, 1, w.y, w.f0, w.a2, w.a3); else rhs<G>(t, w.cs, P, w.y, w.f0);
             st.nfcn++;
             HNEW = fmin(fabs(HNEW), XEND);
             if (REJECT) HNEW = fmin(HNEW, fabs(H));
