@@ -470,24 +470,28 @@ __device__ __forceinline__ int warp_argmax_row(double v, int row)
     return __shfl_sync(0xffffffffu, row, __ffs(cand) - 1);
 }
 
+// A is column-major with leading dimension LD = N + 1: row index N is a dummy row that absorbs the updates of
+// row slots that do not exist (lanes with l + 32 >= N), so the trailing update needs no branches; rows that were
+// pivot rows already carry a zero multiplier.
 template <int G>
-__device__ __noinline__ int lu2_real(int N, double *A, const Lu2Aux &x)
+__device__ __noinline__ int lu2_real(int N, int LD, double *A, const Lu2Aux &x)
 {
     const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
     constexpr int NW = Grp<G>::NW;
     const int i0 = wl, i1 = wl + 32;
+    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;             // storage rows (N = dummy)
     int k0 = (i0 < N) ? -1 : 1 << 30, k1 = (i1 < N) ? -1 : 1 << 30;   // rowk of my two rows (huge = no such row)
     double l0 = 0.0, l1 = 0.0;
     for (int k = 0; k < N; k++) {
         // delayed write-back of the multipliers of column k-1 by its owner warp
         if (k > 0 && wp == (k - 1) % NW) {
-            if (k0 < 0) A[i0 + (k - 1) * N] = l0;
-            if (k1 < 0) A[i1 + (k - 1) * N] = l1;
+            if (k0 < 0) A[i0 + (k - 1) * LD] = l0;
+            if (k1 < 0) A[i1 + (k - 1) * LD] = l1;
         }
-        const double a0 = (k0 < 0) ? A[i0 + k * N] : 0.0, a1 = (k1 < 0) ? A[i1 + k * N] : 0.0;
+        const double a0 = (k0 < 0) ? A[i0 + k * LD] : 0.0, a1 = (k1 < 0) ? A[i1 + k * LD] : 0.0;
         const double v0 = (k0 < 0) ? fabs(a0) : -1.0, v1 = (k1 < 0) ? fabs(a1) : -1.0;
         const int p = warp_argmax_row(v1 > v0 ? v1 : v0, v1 > v0 ? i1 : i0);
-        const double pv = (p >= 0) ? A[p + k * N] : 0.0;
+        const double pv = (p >= 0) ? A[p + k * LD] : 0.0;
         if (p < 0 || !isfinite(pv)) return k + 1;
         const double rp = rcp_nr(pv);
         if (i0 == p) k0 = k;
@@ -495,10 +499,13 @@ __device__ __noinline__ int lu2_real(int N, double *A, const Lu2Aux &x)
         if (lane == 0) { x.perm[k] = p; x.rdr[k] = rp; x.rowk[p] = k; }
         l0 = (k0 < 0) ? a0 * rp : 0.0;
         l1 = (k1 < 0) ? a1 * rp : 0.0;
-        for (int j = k + 1 + ((wp - (k + 1)) % NW + NW) % NW; j < N; j += NW) {
-            const double u = A[p + j * N];
-            if (k0 < 0) A[i0 + j * N] = fma(-l0, u, A[i0 + j * N]);
-            if (k1 < 0) A[i1 + j * N] = fma(-l1, u, A[i1 + j * N]);
+        const int j0 = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
+        double *c = A + j0 * LD;
+#pragma unroll 2
+        for (int j = j0; j < N; j += NW, c += NW * LD) {
+            const double u = c[p];
+            c[r0] = fma(-l0, u, c[r0]);
+            c[r1] = fma(-l1, u, c[r1]);
         }
         Grp<G>::sync();
     }
@@ -506,23 +513,24 @@ __device__ __noinline__ int lu2_real(int N, double *A, const Lu2Aux &x)
 }
 
 template <int G>
-__device__ __noinline__ int lu2_complex(int N, double *Ar, double *Ai, const Lu2Aux &x)
+__device__ __noinline__ int lu2_complex(int N, int LD, double *Ar, double *Ai, const Lu2Aux &x)
 {
     const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
     constexpr int NW = Grp<G>::NW;
     const int i0 = wl, i1 = wl + 32;
+    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;
     int k0 = (i0 < N) ? -1 : 1 << 30, k1 = (i1 < N) ? -1 : 1 << 30;
     double l0r = 0.0, l0i = 0.0, l1r = 0.0, l1i = 0.0;
     for (int k = 0; k < N; k++) {
         if (k > 0 && wp == (k - 1) % NW) {
-            if (k0 < 0) { Ar[i0 + (k - 1) * N] = l0r; Ai[i0 + (k - 1) * N] = l0i; }
-            if (k1 < 0) { Ar[i1 + (k - 1) * N] = l1r; Ai[i1 + (k - 1) * N] = l1i; }
+            if (k0 < 0) { Ar[i0 + (k - 1) * LD] = l0r; Ai[i0 + (k - 1) * LD] = l0i; }
+            if (k1 < 0) { Ar[i1 + (k - 1) * LD] = l1r; Ai[i1 + (k - 1) * LD] = l1i; }
         }
-        const double a0r = (k0 < 0) ? Ar[i0 + k * N] : 0.0, a0i = (k0 < 0) ? Ai[i0 + k * N] : 0.0;
-        const double a1r = (k1 < 0) ? Ar[i1 + k * N] : 0.0, a1i = (k1 < 0) ? Ai[i1 + k * N] : 0.0;
+        const double a0r = (k0 < 0) ? Ar[i0 + k * LD] : 0.0, a0i = (k0 < 0) ? Ai[i0 + k * LD] : 0.0;
+        const double a1r = (k1 < 0) ? Ar[i1 + k * LD] : 0.0, a1i = (k1 < 0) ? Ai[i1 + k * LD] : 0.0;
         const double v0 = (k0 < 0) ? fabs(a0r) + fabs(a0i) : -1.0, v1 = (k1 < 0) ? fabs(a1r) + fabs(a1i) : -1.0;
         const int p = warp_argmax_row(v1 > v0 ? v1 : v0, v1 > v0 ? i1 : i0);
-        const double pr = (p >= 0) ? Ar[p + k * N] : 0.0, pi = (p >= 0) ? Ai[p + k * N] : 0.0;
+        const double pr = (p >= 0) ? Ar[p + k * LD] : 0.0, pi = (p >= 0) ? Ai[p + k * LD] : 0.0;
         const double den = rcp_nr(pr * pr + pi * pi);
         if (p < 0 || !isfinite(den)) return k + 1;
         const double qr = pr * den, qi = -pi * den;       // 1 / pivot
@@ -531,16 +539,16 @@ __device__ __noinline__ int lu2_complex(int N, double *Ar, double *Ai, const Lu2
         if (lane == 0) { x.perm[k] = p; x.rdr[k] = qr; x.rdi[k] = qi; x.rowk[p] = k; }
         l0r = (k0 < 0) ? a0r * qr - a0i * qi : 0.0; l0i = (k0 < 0) ? a0r * qi + a0i * qr : 0.0;
         l1r = (k1 < 0) ? a1r * qr - a1i * qi : 0.0; l1i = (k1 < 0) ? a1r * qi + a1i * qr : 0.0;
-        for (int j = k + 1 + ((wp - (k + 1)) % NW + NW) % NW; j < N; j += NW) {
-            const double ur = Ar[p + j * N], ui = Ai[p + j * N];
-            if (k0 < 0) {
-                Ar[i0 + j * N] = fma(-l0r, ur, fma(l0i, ui, Ar[i0 + j * N]));
-                Ai[i0 + j * N] = fma(-l0r, ui, fma(-l0i, ur, Ai[i0 + j * N]));
-            }
-            if (k1 < 0) {
-                Ar[i1 + j * N] = fma(-l1r, ur, fma(l1i, ui, Ar[i1 + j * N]));
-                Ai[i1 + j * N] = fma(-l1r, ui, fma(-l1i, ur, Ai[i1 + j * N]));
-            }
+        const int j0 = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
+        double *cr = Ar + j0 * LD, *ci = Ai + j0 * LD;
+#pragma unroll 2
+        for (int j = j0; j < N; j += NW, cr += NW * LD, ci += NW * LD) {
+            const double ur = cr[p], ui = ci[p];
+            const double x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
+            cr[r0] = fma(-l0r, ur, fma(l0i, ui, x0r));
+            ci[r0] = fma(-l0r, ui, fma(-l0i, ur, x0i));
+            cr[r1] = fma(-l1r, ur, fma(l1i, ui, x1r));
+            ci[r1] = fma(-l1r, ui, fma(-l1i, ur, x1i));
         }
         Grp<G>::sync();
     }
@@ -548,7 +556,7 @@ __device__ __noinline__ int lu2_complex(int N, double *Ar, double *Ai, const Lu2
 }
 
 // Solves with the lu2 factors by ONE warp: b (shared, length N, original row order) is overwritten by x.
-__device__ __forceinline__ void solve2_real_warp(int N, const double *A, const Lu2Aux &x, double *b, int wl)
+__device__ __forceinline__ void solve2_real_warp(int N, int LD, const double *A, const Lu2Aux &x, double *b, int wl)
 {
     const int i0 = wl, i1 = wl + 32;
     const int k0 = (i0 < N) ? x.rowk[i0] : -1, k1 = (i1 < N) ? x.rowk[i1] : -1;   // -1: no such row (never updated)
@@ -557,21 +565,21 @@ __device__ __forceinline__ void solve2_real_warp(int N, const double *A, const L
     for (int k = 0; k < N - 1; k++) {
         const int p = x.perm[k];
         const double bk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31);
-        if (k0 > k) b0 = fma(-A[i0 + k * N], bk, b0);
-        if (k1 > k) b1 = fma(-A[i1 + k * N], bk, b1);
+        if (k0 > k) b0 = fma(-A[i0 + k * LD], bk, b0);
+        if (k1 > k) b1 = fma(-A[i1 + k * LD], bk, b1);
     }
     __syncwarp();
 #pragma unroll 1
     for (int k = N - 1; k >= 0; k--) {
         const int p = x.perm[k];
         const double xk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31) * x.rdr[k];
-        if (k0 >= 0 && k0 < k) b0 = fma(-A[i0 + k * N], xk, b0);
-        if (k1 >= 0 && k1 < k) b1 = fma(-A[i1 + k * N], xk, b1);
+        if (k0 >= 0 && k0 < k) b0 = fma(-A[i0 + k * LD], xk, b0);
+        if (k1 >= 0 && k1 < k) b1 = fma(-A[i1 + k * LD], xk, b1);
         if (wl == 0) b[k] = xk;
     }
     __syncwarp();
 }
-__device__ __forceinline__ void solve2_complex_warp(int N, const double *Ar, const double *Ai, const Lu2Aux &x, double *br,
+__device__ __forceinline__ void solve2_complex_warp(int N, int LD, const double *Ar, const double *Ai, const Lu2Aux &x, double *br,
                                                     double *bi, int wl)
 {
     const int i0 = wl, i1 = wl + 32;
@@ -584,12 +592,12 @@ __device__ __forceinline__ void solve2_complex_warp(int N, const double *Ar, con
         const double xr = __shfl_sync(0xffffffffu, (p & 32) ? b1r : b0r, p & 31);
         const double xi = __shfl_sync(0xffffffffu, (p & 32) ? b1i : b0i, p & 31);
         if (k0 > k) {
-            const double lr = Ar[i0 + k * N], li = Ai[i0 + k * N];
+            const double lr = Ar[i0 + k * LD], li = Ai[i0 + k * LD];
             b0r = fma(-lr, xr, fma(li, xi, b0r));
             b0i = fma(-lr, xi, fma(-li, xr, b0i));
         }
         if (k1 > k) {
-            const double lr = Ar[i1 + k * N], li = Ai[i1 + k * N];
+            const double lr = Ar[i1 + k * LD], li = Ai[i1 + k * LD];
             b1r = fma(-lr, xr, fma(li, xi, b1r));
             b1i = fma(-lr, xi, fma(-li, xr, b1i));
         }
@@ -603,12 +611,12 @@ __device__ __forceinline__ void solve2_complex_warp(int N, const double *Ar, con
         const double qr = x.rdr[k], qi = x.rdi[k];
         const double xr = vr * qr - vi * qi, xi = vr * qi + vi * qr;
         if (k0 >= 0 && k0 < k) {
-            const double ur = Ar[i0 + k * N], ui = Ai[i0 + k * N];
+            const double ur = Ar[i0 + k * LD], ui = Ai[i0 + k * LD];
             b0r = fma(-ur, xr, fma(ui, xi, b0r));
             b0i = fma(-ur, xi, fma(-ui, xr, b0i));
         }
         if (k1 >= 0 && k1 < k) {
-            const double ur = Ar[i1 + k * N], ui = Ai[i1 + k * N];
+            const double ur = Ar[i1 + k * LD], ui = Ai[i1 + k * LD];
             b1r = fma(-ur, xr, fma(ui, xi, b1r));
             b1i = fma(-ur, xi, fma(-ui, xr, b1i));
         }
@@ -617,22 +625,22 @@ __device__ __forceinline__ void solve2_complex_warp(int N, const double *Ar, con
     __syncwarp();
 }
 template <int G>
-__device__ __noinline__ void solve2_pair(int N, const double *E1, const Lu2Aux &x1, double *z1, const double *E2r,
+__device__ __noinline__ void solve2_pair(int N, int LD, const double *E1, const Lu2Aux &x1, double *z1, const double *E2r,
                                          const double *E2i, const Lu2Aux &x2, double *z2, double *z3)
 {
     if (G == 32) {
-        solve2_real_warp(N, E1, x1, z1, Grp<G>::wlane());
-        solve2_complex_warp(N, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
+        solve2_real_warp(N, LD, E1, x1, z1, Grp<G>::wlane());
+        solve2_complex_warp(N, LD, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
     } else {
-        if (Grp<G>::warp() == 0) solve2_real_warp(N, E1, x1, z1, Grp<G>::wlane());
-        else if (Grp<G>::warp() == 1) solve2_complex_warp(N, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
+        if (Grp<G>::warp() == 0) solve2_real_warp(N, LD, E1, x1, z1, Grp<G>::wlane());
+        else if (Grp<G>::warp() == 1) solve2_complex_warp(N, LD, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
     }
     Grp<G>::sync();
 }
 template <int G>
-__device__ __noinline__ void solve2_real(int N, const double *E1, const Lu2Aux &x1, double *b)
+__device__ __noinline__ void solve2_real(int N, int LD, const double *E1, const Lu2Aux &x1, double *b)
 {
-    if (Grp<G>::warp() == 0) solve2_real_warp(N, E1, x1, b, Grp<G>::wlane());
+    if (Grp<G>::warp() == 0) solve2_real_warp(N, LD, E1, x1, b, Grp<G>::wlane());
     Grp<G>::sync();
 }
 

@@ -2,13 +2,15 @@
 
 namespace {
 
-constexpr int kBlock = 128;   // threads per CTA for every kernel here
+constexpr int kBlock = 128;   // threads per CTA of the warp-group kernels (G = 32); a CTA-group kernel has G threads
+template <int G>
+__host__ __device__ constexpr int block_of() { return G > kBlock ? G : kBlock; }
 
 // Group <-> CTA mapping: G == 32 -> four warp-groups per CTA, G == 128 -> the CTA is the group.
 template <int G>
 __device__ __forceinline__ int group_in_block() { return G == 32 ? (int)(threadIdx.x >> 5) : 0; }
 template <int G>
-constexpr int groups_per_block() { return kBlock / G; }
+constexpr int groups_per_block() { return block_of<G>() / G; }
 
 // Next state index from the work queue (PAPER.md L194 names load imbalance between IVPs; groups that
 // finish early pull new states).  Uniform across the group.
@@ -29,7 +31,7 @@ __device__ __forceinline__ int next_state(int *counter, int *bcast)
 }
 
 template <int G>
-__global__ void __launch_bounds__(kBlock) integrate_kernel(Tables t, int n_states, double P, const double *P_per_state,
+__global__ void __launch_bounds__(block_of<G>(), G > kBlock ? 2 : 1) integrate_kernel(Tables t, int n_states, double P, const double *P_per_state,
                                                            RadauParams prm, const double *__restrict__ y_in,
                                                            double *__restrict__ y_out, chem_stats *stats, int *counter,
                                                            const int *order)
@@ -99,7 +101,7 @@ __global__ void __launch_bounds__(kWarpBlock, 2) integrate_warp_kernel(Tables t,
 
 // Source term / Jacobian for a batch (static round-robin over groups).
 template <int G, bool JAC>
-__global__ void __launch_bounds__(kBlock) eval_kernel(Tables t, int n_states, double P, const double *__restrict__ y,
+__global__ void __launch_bounds__(block_of<G>()) eval_kernel(Tables t, int n_states, double P, const double *__restrict__ y,
                                                       double *__restrict__ out)
 {
     extern __shared__ double smem[];
@@ -107,7 +109,7 @@ __global__ void __launch_bounds__(kBlock) eval_kernel(Tables t, int n_states, do
     const size_t wd = work_doubles(N, NR, Grp<G>::NW, t.n_fo);
     Work w = carve(smem + (size_t)group_in_block<G>() * wd, N, NR, Grp<G>::NW, t.n_fo);
     const int lane = Grp<G>::lane();
-    const int gpb = kBlock / G;
+    const int gpb = block_of<G>() / G;
     for (int s = blockIdx.x * gpb + group_in_block<G>(); s < n_states; s += gridDim.x * gpb) {
         for (int i = lane; i < N; i += G) w.y[i] = y[(size_t)s * N + i];
         Grp<G>::sync();

@@ -3,16 +3,16 @@
 namespace {
 
 // group size: a warp per state up to 32 unknowns, a CTA per state above
-inline int group_size(const chem_mech *m) { return m->t.n_sp <= 32 ? 32 : 128; }
+inline int group_size(const chem_mech *m) { return m->t.n_sp <= 32 ? 32 : 256; }
 
 template <typename K>
-int configure(K kernel, const chem_mech *m, size_t smem, int *ctas_per_sm)
+int configure(K kernel, const chem_mech *m, size_t smem, int *ctas_per_sm, int block = kBlock)
 {
     if (smem > (size_t)m->max_smem_optin)
         return fail(CHEM_E_UNSUPPORTED, "mechanism needs %zu B of shared memory per CTA, device offers %d", smem, m->max_smem_optin);
     CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, kBlock, smem));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, block, smem));
     if (occ < 1) return fail(CHEM_E_UNSUPPORTED, "kernel does not fit on an SM");
     *ctas_per_sm = occ;
     return CHEM_OK;
@@ -21,14 +21,14 @@ int configure(K kernel, const chem_mech *m, size_t smem, int *ctas_per_sm)
 template <int G, bool JAC>
 int launch_eval(const chem_mech *m, int n, double P, const double *y, double *out, cudaStream_t st)
 {
-    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (kBlock / G);
+    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (block_of<G>() / G);
     int occ = 0;
-    int rc = configure(eval_kernel<G, JAC>, m, smem, &occ);
+    int rc = configure(eval_kernel<G, JAC>, m, smem, &occ, block_of<G>());
     if (rc) return rc;
-    const int gpb = kBlock / G;
+    const int gpb = block_of<G>() / G;
     int grid = (n + gpb - 1) / gpb;
     if (grid > m->n_sm * occ) grid = m->n_sm * occ;
-    eval_kernel<G, JAC><<<grid, kBlock, smem, st>>>(m->t, n, P, y, out);
+    eval_kernel<G, JAC><<<grid, block_of<G>(), smem, st>>>(m->t, n, P, y, out);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return CHEM_OK;
@@ -38,15 +38,15 @@ template <int G>
 int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
                      const chem_opts *o, chem_stats *stats, cudaStream_t st)
 {
-    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (kBlock / G);
+    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (block_of<G>() / G);
     int occ = 0;
-    int rc = configure(integrate_kernel<G>, m, smem, &occ);
+    int rc = configure(integrate_kernel<G>, m, smem, &occ, block_of<G>());
     if (rc) return rc;
-    const int gpb = kBlock / G;
+    const int gpb = block_of<G>() / G;
     int grid = (n + gpb - 1) / gpb;
     if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, groups pull work from the queue
     CUDA_TRY(cudaMemsetAsync(m->counter, 0, sizeof(int), st));
-    integrate_kernel<G><<<grid, kBlock, smem, st>>>(m->t, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats,
+    integrate_kernel<G><<<grid, block_of<G>(), smem, st>>>(m->t, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats,
                                                     m->counter, nullptr);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
@@ -82,7 +82,7 @@ extern "C" int chem_rhs(const chem_mech *m, int32_t n, double P, const double *y
     if (!m || n < 0 || (n > 0 && (!y || !f))) return fail(CHEM_E_ARG, "bad argument");
     if (n == 0) return CHEM_OK;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    return group_size(m) == 32 ? launch_eval<32, false>(m, n, P, y, f, st) : launch_eval<128, false>(m, n, P, y, f, st);
+    return group_size(m) == 32 ? launch_eval<32, false>(m, n, P, y, f, st) : launch_eval<256, false>(m, n, P, y, f, st);
 }
 
 extern "C" int chem_jacobian(const chem_mech *m, int32_t n, double P, const double *y, double *J, void *stream)
@@ -90,7 +90,7 @@ extern "C" int chem_jacobian(const chem_mech *m, int32_t n, double P, const doub
     if (!m || n < 0 || (n > 0 && (!y || !J))) return fail(CHEM_E_ARG, "bad argument");
     if (n == 0) return CHEM_OK;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    return group_size(m) == 32 ? launch_eval<32, true>(m, n, P, y, J, st) : launch_eval<128, true>(m, n, P, y, J, st);
+    return group_size(m) == 32 ? launch_eval<32, true>(m, n, P, y, J, st) : launch_eval<256, true>(m, n, P, y, J, st);
 }
 
 extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const double *A, const double *b, double *x,
@@ -130,7 +130,7 @@ extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double
     if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "register-resident warp kernel not available for this mechanism");
     if (kernel != 1 && warp_path_available(m)) return launch_integrate_warp(m, n, P, prm, y_in, y_out, o, stats, st);
     return group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, st)
-                               : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, st);
+                               : launch_integrate<256>(m, n, P, prm, y_in, y_out, o, stats, st);
 }
 
 extern "C" int chem_integrate(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,

@@ -39,9 +39,9 @@ struct Work {
 
 __host__ __device__ inline size_t work_doubles(int N, int NR, int NW, int n_fo = 0)
 {
-    const size_t e2 = (size_t)2 * N * N > (size_t)8 * NR ? (size_t)2 * N * N : (size_t)8 * NR;
+    const size_t e2 = (size_t)2 * N * (N + 1) > (size_t)8 * NR ? (size_t)2 * N * (N + 1) : (size_t)8 * NR;
     // 16 vectors + 6 chem vectors + q + Jm + E1 + E2 region + red + 2 int vectors (N ints each -> N doubles total)
-    return (size_t)22 * N + NR + (size_t)2 * N * N + e2 + 2 * NW + N + 2 + 3 * N + N + 2 + cta_extra_doubles(N, NR, n_fo, NW);   // + rd1, rd2r, rd2i, rowk1/2, batched-rhs scratch
+    return (size_t)22 * N + NR + (size_t)2 * N * N + N + e2 + 2 * NW + N + 2 + 3 * N + N + 2 + cta_extra_doubles(N, NR, n_fo, NW);   // + rd1, rd2r, rd2i, rowk1/2, batched-rhs scratch
 }
 
 __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW, int n_fo = 0)
@@ -61,10 +61,10 @@ __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW, int n
     take((size_t)2 * NR);
     w.cx.q3 = w.cs.q;                 // [3][NR]
     w.Jm = take((size_t)N * N);
-    w.E1 = take((size_t)N * N);
-    const size_t e2 = (size_t)2 * N * N > (size_t)8 * NR ? (size_t)2 * N * N : (size_t)8 * NR;
+    w.E1 = take((size_t)N * (N + 1));
+    const size_t e2 = (size_t)2 * N * (N + 1) > (size_t)8 * NR ? (size_t)2 * N * (N + 1) : (size_t)8 * NR;
     double *r = take(e2);
-    w.E2r = r; w.E2i = r + (size_t)N * N;
+    w.E2r = r; w.E2i = r + (size_t)N * (N + 1);
     w.cs.dq = r; w.cs.dqdT = r + (size_t)6 * NR; w.cs.tb = r + (size_t)7 * NR;   // alive only inside jacobian()
     w.cs.red = take(2 * NW);
     w.ip1 = reinterpret_cast<int *>(take(N + 2));                  // 2 N ints
@@ -108,6 +108,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
     const double FNEWT = fmax(10.0 * UROUND / RTOL, fmin(0.03, sqrt(RTOL)));
     const double XEND = prm.t_end;
     const double CFAC = SAFE * (1 + 2 * NIT);
+    const int LD = (N <= 64) ? N + 1 : N;      // lu2 keeps a dummy row (chem_device.cuh)
 
     st.status = 0; st.nstep = 0; st.naccpt = 0; st.nrejct = 0; st.nfcn = 0; st.njac = 0; st.ndec = 0; st.nsol = 0;
     st.nnewt_fail = 0; st.h_last = 0.0;
@@ -147,15 +148,15 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
                 for (int i = Grp<G>::wlane(); i < N; i += 32) {
                     const double v = -w.Jm[i * N + j];
                     nonfinite |= !isfinite(v);
-                    w.E1[i + j * N] = (i == j) ? v + FAC1 : v;
-                    w.E2r[i + j * N] = (i == j) ? v + ALPHN : v;
-                    w.E2i[i + j * N] = (i == j) ? BETAN : 0.0;
+                    w.E1[i + j * LD] = (i == j) ? v + FAC1 : v;
+                    w.E2r[i + j * LD] = (i == j) ? v + ALPHN : v;
+                    w.E2i[i + j * LD] = (i == j) ? BETAN : 0.0;
                 }
             int ier = Grp<G>::any(nonfinite, w.cs.red);   // includes the barrier after the stores
             if (G == 32) __syncwarp();
             if (N <= 64) {
-                if (!ier) ier = lu2_real<G>(N, w.E1, w.x1);
-                if (!ier) ier = lu2_complex<G>(N, w.E2r, w.E2i, w.x2);
+                if (!ier) ier = lu2_real<G>(N, LD, w.E1, w.x1);
+                if (!ier) ier = lu2_complex<G>(N, LD, w.E2r, w.E2i, w.x2);
             } else {
                 if (!ier) ier = lu_real<G>(N, w.E1, w.ip1);
                 if (!ier) ier = lu_complex<G>(N, w.E2r, w.E2i, w.ip2);
@@ -227,7 +228,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
                 w.z3[i] = TI31 * a1 + TI32 * a2 + TI33 * a3 - f3 * ALPHN - f2 * BETAN;
             }
             Grp<G>::sync();
-            if (N <= 64) solve2_pair<G>(N, w.E1, w.x1, w.z1, w.E2r, w.E2i, w.x2, w.z2, w.z3);
+            if (N <= 64) solve2_pair<G>(N, LD, w.E1, w.x1, w.z1, w.E2r, w.E2i, w.x2, w.z2, w.z3);
             else solve_pair<G>(N, w.E1, w.ip1, w.z1, w.E2r, w.E2i, w.ip2, w.z2, w.z3);
             st.nsol++;
             NEWT++;
@@ -286,7 +287,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
                 w.a1[i] = f2 + w.f0[i];
             }
             Grp<G>::sync();
-            if (N <= 64) solve2_real<G>(N, w.E1, w.x1, w.a1); else solve_real<G>(N, w.E1, w.ip1, w.a1);
+            if (N <= 64) solve2_real<G>(N, LD, w.E1, w.x1, w.a1); else solve_real<G>(N, w.E1, w.ip1, w.a1);
             double e = 0.0, dummy = 0.0;
             for (int i = lane; i < N; i += G) { const double r = w.a1[i] / w.scal[i]; e += r * r; }
             Grp<G>::sum2(e, dummy, w.cs.red);
@@ -298,7 +299,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
                 st.nfcn++;
                 for (int i = lane; i < N; i += G) w.a1[i] = w.a3[i] + w.a2[i];
                 Grp<G>::sync();
-                if (N <= 64) solve2_real<G>(N, w.E1, w.x1, w.a1); else solve_real<G>(N, w.E1, w.ip1, w.a1);
+                if (N <= 64) solve2_real<G>(N, LD, w.E1, w.x1, w.a1); else solve_real<G>(N, w.E1, w.ip1, w.a1);
                 e = 0.0; dummy = 0.0;
                 for (int i = lane; i < N; i += G) { const double r = w.a1[i] / w.scal[i]; e += r * r; }
                 Grp<G>::sum2(e, dummy, w.cs.red);
