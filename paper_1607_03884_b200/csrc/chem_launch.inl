@@ -3,7 +3,7 @@
 namespace {
 
 // group size: a warp per state up to 32 unknowns, a CTA per state above
-inline int group_size(const chem_mech *m) { return m->t.n_sp <= 32 ? 32 : 256; }
+inline int group_size(const chem_mech *m) { return m->t.n_sp <= 32 ? 32 : 128; }
 
 template <typename K>
 int configure(K kernel, const chem_mech *m, size_t smem, int *ctas_per_sm, int block = kBlock)
@@ -82,7 +82,7 @@ extern "C" int chem_rhs(const chem_mech *m, int32_t n, double P, const double *y
     if (!m || n < 0 || (n > 0 && (!y || !f))) return fail(CHEM_E_ARG, "bad argument");
     if (n == 0) return CHEM_OK;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    return group_size(m) == 32 ? launch_eval<32, false>(m, n, P, y, f, st) : launch_eval<256, false>(m, n, P, y, f, st);
+    return group_size(m) == 32 ? launch_eval<32, false>(m, n, P, y, f, st) : launch_eval<128, false>(m, n, P, y, f, st);
 }
 
 extern "C" int chem_jacobian(const chem_mech *m, int32_t n, double P, const double *y, double *J, void *stream)
@@ -90,7 +90,7 @@ extern "C" int chem_jacobian(const chem_mech *m, int32_t n, double P, const doub
     if (!m || n < 0 || (n > 0 && (!y || !J))) return fail(CHEM_E_ARG, "bad argument");
     if (n == 0) return CHEM_OK;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    return group_size(m) == 32 ? launch_eval<32, true>(m, n, P, y, J, st) : launch_eval<256, true>(m, n, P, y, J, st);
+    return group_size(m) == 32 ? launch_eval<32, true>(m, n, P, y, J, st) : launch_eval<128, true>(m, n, P, y, J, st);
 }
 
 extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const double *A, const double *b, double *x,
@@ -130,7 +130,7 @@ extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double
     if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "register-resident warp kernel not available for this mechanism");
     if (kernel != 1 && warp_path_available(m)) return launch_integrate_warp(m, n, P, prm, y_in, y_out, o, stats, st);
     return group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, st)
-                               : launch_integrate<256>(m, n, P, prm, y_in, y_out, o, stats, st);
+                               : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, st);
 }
 
 extern "C" int chem_integrate(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
