@@ -87,9 +87,11 @@ typedef struct chem_opts {
     double h0;           /* first internal step size; 0 -> t_end (R9)                      */
     int32_t max_steps;   /* limit on internal step attempts per state; 0 -> 100000                    */
     int32_t newton_max;  /* max simplified-Newton iterations per step; 0 -> 7                         */
-    int32_t kernel;      /* 0 auto; 1 generic shared-memory kernel; 2 register-resident warp kernel   */
-    int32_t reorder;     /* 0 off; 1 process states in order of decreasing predicted cost            */
-    const double *P_per_state; /* device [n_states] or NULL: per-state pressure overriding P        */
+    int32_t kernel;      /* 0 auto; 1 shared-memory group kernel; 2 compact warp-per-state kernel (small mechanisms) */
+    int32_t reorder;     /* 1: start the states in order of decreasing cost_hint ("reordering IVPs"); 0 off */
+    const double *P_per_state;  /* device [n_states] or NULL: per-state pressure overriding P        */
+    const int32_t *cost_hint;   /* device [n_states] or NULL: predicted cost per state, e.g. chem_stats.nstep of the
+                                   previous global step; read only when reorder = 1.  Results do not depend on it. */
 } chem_opts;
 
 /* Per-state result record written by chem_integrate_ex (device array of n_states). */

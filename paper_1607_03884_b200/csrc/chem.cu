@@ -50,6 +50,8 @@ struct chem_mech {
     double flops[5] = {0, 0, 0, 0, 0};
     FastTables fast{};          // register-resident warp path (chem_warp.cuh), if eligible
     void *fast_blob = nullptr;
+    void *order_buf = nullptr;  // scratch of the optional cost ordering (grown on demand)
+    size_t order_bytes = 0;
 };
 
 #include "chem_fast.inl"
@@ -308,6 +310,7 @@ extern "C" void chem_mech_free(chem_mech *m)
     if (m->dev_blob) cudaFree(m->dev_blob);
     if (m->counter) cudaFree(m->counter);
     if (m->fast_blob) cudaFree(m->fast_blob);
+    if (m->order_buf) cudaFree(m->order_buf);
     delete m;
 }
 

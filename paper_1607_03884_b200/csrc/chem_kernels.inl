@@ -69,7 +69,7 @@ constexpr int kWarpBlock = 256;
 __global__ void __launch_bounds__(kWarpBlock, 2) integrate_warp_kernel(Tables t, FastTables ft, int n_states, double P,
                                                                     const double *P_per_state, RadauParams prm,
                                                                     const double *__restrict__ y_in, double *__restrict__ y_out,
-                                                                    chem_stats *stats, int *counter)
+                                                                    chem_stats *stats, int *counter, const int *order)
 {
     extern __shared__ double smem[];
     for (int i = threadIdx.x; i < ft.blob_doubles; i += kWarpBlock) smem[i] = ft.blob[i];   // stage the tables once per CTA
@@ -84,6 +84,7 @@ __global__ void __launch_bounds__(kWarpBlock, 2) integrate_warp_kernel(Tables t,
         if (lane == 0) q = atomicAdd(counter, 1);
         q = __shfl_sync(0xffffffffu, q, 0);
         if (q >= n_states) break;
+        if (order) q = order[q];
         double y = lane < N ? y_in[(size_t)q * N + lane] : 0.0;
         RadauResult r;
         radau_state_warp(t, smem, ws, ft.tmid, P_per_state ? P_per_state[q] : P, prm, y, r);

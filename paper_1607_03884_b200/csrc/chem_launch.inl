@@ -1,4 +1,5 @@
 // chem_launch.inl -- host launch logic and the compute entry points of include/chem.h.
+#include <cub/device/device_radix_sort.cuh>
 
 namespace {
 
@@ -15,6 +16,37 @@ int configure(K kernel, const chem_mech *m, size_t smem, int *ctas_per_sm, int b
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, block, smem));
     if (occ < 1) return fail(CHEM_E_UNSUPPORTED, "kernel does not fit on an SM");
     *ctas_per_sm = occ;
+    return CHEM_OK;
+}
+
+
+// Optional cost ordering (chem_opts.reorder, "reordering IVPs to increase similarity"): with a work queue
+// the order only decides WHEN a state starts; starting the expensive ones first shortens the tail of the launch.
+__global__ void iota_kernel(int n, int *v)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) v[i] = i;
+}
+int build_order(const chem_mech *m, int n, const int32_t *cost, int **order_out, cudaStream_t st)
+{
+    chem_mech *mm = const_cast<chem_mech *>(m);
+    size_t tmp_bytes = 0;
+    cub::DeviceRadixSort::SortPairsDescending(nullptr, tmp_bytes, cost, (int32_t *)nullptr, (int *)nullptr, (int *)nullptr, n, 0, 32, st);
+    const size_t need = (size_t)3 * n * sizeof(int) + tmp_bytes + 256;
+    if (need > mm->order_bytes) {
+        if (mm->order_buf) cudaFree(mm->order_buf);
+        mm->order_buf = nullptr; mm->order_bytes = 0;
+        CUDA_TRY(cudaMalloc(&mm->order_buf, need));
+        mm->order_bytes = need;
+    }
+    int *idx = static_cast<int *>(mm->order_buf), *ord = idx + n;
+    int32_t *keys_out = reinterpret_cast<int32_t *>(ord + n);
+    void *tmp = reinterpret_cast<char *>(mm->order_buf) + (((size_t)3 * n * sizeof(int) + 255) & ~size_t(255));
+    iota_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, idx);
+    g_launches++;
+    CUDA_TRY(cub::DeviceRadixSort::SortPairsDescending(tmp, tmp_bytes, cost, keys_out, idx, ord, n, 0, 32, st));
+    g_launches += 3;   // cub: histogram + onesweep passes (not counted exactly)
+    *order_out = ord;
     return CHEM_OK;
 }
 
@@ -46,8 +78,10 @@ int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm
     int grid = (n + gpb - 1) / gpb;
     if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, groups pull work from the queue
     CUDA_TRY(cudaMemsetAsync(m->counter, 0, sizeof(int), st));
+    int *order = nullptr;
+    if (o && o->reorder && o->cost_hint) { rc = build_order(m, n, o->cost_hint, &order, st); if (rc) return rc; }
     integrate_kernel<G><<<grid, block_of<G>(), smem, st>>>(m->t, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats,
-                                                    m->counter, nullptr);
+                                                    m->counter, order);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return CHEM_OK;
@@ -66,8 +100,10 @@ int launch_integrate_warp(const chem_mech *m, int n, double P, const RadauParams
     int grid = (n + wpb - 1) / wpb;
     if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, warps pull states from the queue
     CUDA_TRY(cudaMemsetAsync(m->counter, 0, sizeof(int), st));
+    int *order = nullptr;
+    if (o && o->reorder && o->cost_hint) { const int rc = build_order(m, n, o->cost_hint, &order, st); if (rc) return rc; }
     integrate_warp_kernel<<<grid, kWarpBlock, smem, st>>>(m->t, m->fast, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out,
-                                                          stats, m->counter);
+                                                          stats, m->counter, order);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return CHEM_OK;

@@ -192,3 +192,18 @@ def test_full_size_gri_sampled_against_oracle(torch_cuda, gpu_mechs, orc_mechs, 
     idx = np.random.default_rng(5).choice(n, 96, replace=False)
     y_ref, st_ref, _ = orc_mechs["gri"].integrate(y0[idx], P, cfg["t_end"], RTOL, ATOL)
     assert np.all(np.abs(y1[idx] - y_ref) <= 1e-9 + 1e-6 * np.abs(y_ref))
+
+
+@pytest.mark.parametrize("kind,n", [("h2co", 5000), ("gri", 300)])
+def test_cost_ordering_does_not_change_results(kind, n, torch_cuda, gpu_mechs, request):
+    """chem_opts.reorder only changes WHEN a state is started: results are bit-identical"""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = descs(request)[kind]
+    y0 = torch.from_numpy(synth.make_states(mech, n, "ignition", 77)).cuda()
+    y_a, st_a = binding.chem_integrate_ex(gpu_mechs[kind], P, 1e-5, RTOL, ATOL, y0)
+    nstep = torch.from_numpy(binding.stats_to_numpy(st_a)["nstep"].copy()).cuda()
+    y_b, st_b = binding.chem_integrate_ex(gpu_mechs[kind], P, 1e-5, RTOL, ATOL, y0, reorder=1, cost_hint=nstep)
+    torch.cuda.synchronize()
+    assert torch.equal(y_a, y_b)
+    assert np.array_equal(binding.stats_to_numpy(st_a), binding.stats_to_numpy(st_b))
