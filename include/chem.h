@@ -92,6 +92,9 @@ typedef struct chem_opts {
     const double *P_per_state;  /* device [n_states] or NULL: per-state pressure overriding P        */
     const int32_t *cost_hint;   /* device [n_states] or NULL: predicted cost per state, e.g. chem_stats.nstep of the
                                    previous global step; read only when reorder = 1.  Results do not depend on it. */
+    int32_t fd_jacobian; /* 1: first-order finite-difference Jacobian "based on that of CVODE" (Sec. 3.4;
+                            DESIGN.md R13) instead of the analytical one; costs N extra source terms per Jacobian */
+    int32_t reserved;
 } chem_opts;
 
 /* Per-state result record written by chem_integrate_ex (device array of n_states). */

@@ -437,6 +437,7 @@ typedef struct {
     int newton_max;     /* NIT:  0 -> 7                                                          */
     double h0;          /* first step size; 0 -> t_end                                           */
     int fixed_steps;    /* >0: take exactly this many equal steps, no error control */
+    int fd_jacobian;    /* 1: first-order finite-difference Jacobian "based on that of CVODE" (R13) */
 } orc_radau_opts;
 
 typedef struct {
@@ -539,7 +540,25 @@ void orc_radau5(int n, orc_fcn fcn, orc_jac jac, void *ctx, double *y, double t_
     int fixed_done = 0;
 
 compute_jacobian:                                   /* label 10 */
-    jac(n, y, FJAC, ctx); st->njac++;
+    if (opt && opt->fd_jacobian) {
+        /* CVODE's dense difference quotient (R13): column j = (f(y + inc_j e_j) - f(y)) / inc_j,
+           inc_j = max(sqrt(u) |y_j|, minInc / ewt_j), ewt_j = 1/scal_j,
+           minInc = 1000 |h| u n ||f(y)||_wrms (1 if the norm is zero); f(y) = Y0 is current at this point. */
+        double fnorm = 0.0;
+        for (int i = 0; i < n; i++) fnorm += (Y0[i] / SCAL[i]) * (Y0[i] / SCAL[i]);
+        fnorm = sqrt(fnorm / n);
+        const double minInc = (fnorm != 0.0) ? 1000.0 * fabs(H) * UROUND * n * fnorm : 1.0;
+        for (int j = 0; j < n; j++) {
+            const double inc = fmax(sqrt(UROUND) * fabs(y[j]), minInc * SCAL[j]);
+            for (int i = 0; i < n; i++) TMP[i] = y[i];
+            TMP[j] += inc;
+            fcn(n, TMP, A1, ctx); st->nfcn++;
+            for (int i = 0; i < n; i++) FJAC[i * n + j] = (A1[i] - Y0[i]) / inc;
+        }
+    } else {
+        jac(n, y, FJAC, ctx);
+    }
+    st->njac++;
     CALJAC = 1;
 factorize:                                          /* label 20 */
     {

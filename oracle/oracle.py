@@ -41,7 +41,8 @@ class _Mech(C.Structure):
 
 
 class RadauOpts(C.Structure):
-    _fields_ = [("max_steps", C.c_int), ("newton_max", C.c_int), ("h0", C.c_double), ("fixed_steps", C.c_int)]
+    _fields_ = [("max_steps", C.c_int), ("newton_max", C.c_int), ("h0", C.c_double), ("fixed_steps", C.c_int),
+                ("fd_jacobian", C.c_int)]
 
 
 class RadauStats(C.Structure):
@@ -137,20 +138,20 @@ class Mechanism:
 
     # -- batched integration -----------------------------------------------------
     def integrate(self, y_in, P: float, t_end: float, rtol: float, atol: float, n_threads: int = 0,
-                  h0: float = 0.0, max_steps: int = 0, fixed_steps: int = 0):
+                  h0: float = 0.0, max_steps: int = 0, fixed_steps: int = 0, fd_jacobian: int = 0):
         y_in = np.ascontiguousarray(y_in, dtype=np.float64)
         n = y_in.shape[0]
         assert y_in.shape[1] == self.n_sp
         y_out = np.empty_like(y_in)
         stats = np.zeros(n, dtype=STATS_DTYPE)
-        opt = RadauOpts(max_steps, 0, h0, fixed_steps)
+        opt = RadauOpts(max_steps, 0, h0, fixed_steps, fd_jacobian)
         used = lib().orc_integrate(C.byref(self.c), n, C.c_double(P), C.c_double(t_end), C.c_double(rtol),
                                    C.c_double(atol), _d(y_in), _d(y_out), C.byref(opt),
                                    stats.ctypes.data_as(C.c_void_p), n_threads)
         return y_out, stats, used
 
 
-def radau5(f, jac, y0, t_end, rtol, atol, h0=0.0, max_steps=0, fixed_steps=0, newton_max=0):
+def radau5(f, jac, y0, t_end, rtol, atol, h0=0.0, max_steps=0, fixed_steps=0, newton_max=0, fd_jacobian=0):
     """Generic Radau IIA driver on a Python right-hand side f(y) and Jacobian jac(y) (row-major)."""
     y = np.array(y0, dtype=np.float64)
     n = y.size
@@ -163,7 +164,7 @@ def radau5(f, jac, y0, t_end, rtol, atol, h0=0.0, max_steps=0, fixed_steps=0, ne
         yy = np.ctypeslib.as_array(yp, shape=(n_,))
         np.ctypeslib.as_array(Jp, shape=(n_ * n_,))[:] = np.asarray(jac(yy), dtype=np.float64).reshape(-1)
 
-    opt = RadauOpts(max_steps, newton_max, h0, fixed_steps)
+    opt = RadauOpts(max_steps, newton_max, h0, fixed_steps, fd_jacobian)
     st = RadauStats()
     lib().orc_radau5(n, FCN(_f), JAC(_j), None, _d(y), C.c_double(t_end), C.c_double(rtol), C.c_double(atol),
                      C.byref(opt), C.byref(st))

@@ -83,6 +83,7 @@ __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW, int n
 struct RadauParams {
     double t_end, rtol, atol, h0;
     int max_steps, newton_max;
+    int fd_jacobian, pad_;          // 1: CVODE-style difference-quotient Jacobian (R13)
     double rtol_t, atol_t, fnewt;   // RADAU5's transformed tolerances and Newton stopping level (R8), set on the host
 };
 
@@ -136,7 +137,35 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
     int next = DO_JAC;
     for (;;) {
         if (next == DO_JAC) {
-            jacobian<G>(t, w.cs, P, w.y, w.Jm);
+            if (prm.fd_jacobian) {
+                // column j = (f(y + inc_j e_j) - f(y)) / inc_j, inc_j = max(sqrt(u) |y_j|, minInc scal_j),
+                // minInc = 1000 |h| u N ||f(y)||_wrms (1 if zero); f(y) = f0 is current here (R13)
+                double fn = 0.0, dummy = 0.0;
+                for (int i = lane; i < N; i += G) { const double r = w.f0[i] / w.scal[i]; fn += r * r; }
+                Grp<G>::sum2(fn, dummy, w.cs.red);
+                const double fnorm = sqrt(fn / N);
+                const double minInc = (fnorm != 0.0) ? 1000.0 * fabs(H) * UROUND * N * fnorm : 1.0;
+                const int step = jobs ? 3 : 1;
+                for (int j0 = 0; j0 < N; j0 += step) {
+                    for (int i = lane; i < N; i += G) {
+                        const double yi = w.y[i], inc = fmax(1.4901161193847656e-08 * fabs(yi), minInc * w.scal[i]);
+                        w.ys[i] = (i == j0) ? yi + inc : yi;
+                        if (jobs) { w.cx.ys2[i] = (i == j0 + 1) ? yi + inc : yi; w.cx.ys3[i] = (i == j0 + 2) ? yi + inc : yi; }
+                    }
+                    Grp<G>::sync();
+                    if (jobs) cta_rhs3<G>(t, w.cs, w.cx, P, 3, w.ys, w.a1, w.a2, w.a3); else rhs<G>(t, w.cs, P, w.ys, w.a1);
+                    for (int c = 0; c < step && j0 + c < N; c++) {
+                        const int j = j0 + c;
+                        const double *fc = (c == 0) ? w.a1 : (c == 1 ? w.a2 : w.a3);
+                        const double inc = fmax(1.4901161193847656e-08 * fabs(w.y[j]), minInc * w.scal[j]);
+                        for (int i = lane; i < N; i += G) w.Jm[i * N + j] = (fc[i] - w.f0[i]) / inc;
+                        st.nfcn++;
+                    }
+                    Grp<G>::sync();
+                }
+            } else {
+                jacobian<G>(t, w.cs, P, w.y, w.Jm);
+            }
             st.njac++;
             CALJAC = true;
             next = DO_FACT;

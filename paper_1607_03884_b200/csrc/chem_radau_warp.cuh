@@ -78,7 +78,30 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     int next = DO_JAC;
     for (;;) {
         if (next == DO_JAC) {
-            warp_jacobian(tab, ws, tmid, P, invP, y, M.Jm, M.Ar, M.vec);
+            if (prm.fd_jacobian) {
+                // CVODE-style difference quotient, three columns per source-term call (R13)
+                const double scal = ATOL + RTOL * fabs(y);
+                double fn = 0.0;
+                if (mine) { const double r = f0 * iscal; fn = r * r; }
+                const double fnorm = sqrt_s(warp_sum(fn) * invN);
+                const double minInc = (fnorm != 0.0) ? 1000.0 * fabs(H) * UROUND * N * fnorm : 1.0;
+                const double inc = fmax(1.4901161193847656e-08 * fabs(y), minInc * scal);
+                for (int j0 = 0; j0 < N; j0 += 3) {
+                    const D3 fs = warp_rhs3(tab, ws, tmid, P, invP,
+                                            D3{lane == j0 ? y + inc : y, lane == j0 + 1 ? y + inc : y, lane == j0 + 2 ? y + inc : y}, 3);
+#pragma unroll
+                    for (int c = 0; c < 3; c++) {
+                        const int j = j0 + c;
+                        const double incj = __shfl_sync(0xffffffffu, inc, j < N ? j : 0);
+                        const double fc = c == 0 ? fs.a : (c == 1 ? fs.b : fs.c);
+                        if (mine && j < N) M.Jm[lane * N + j] = (fc - f0) / incj;
+                        if (j < N) st.nfcn++;
+                    }
+                }
+                __syncwarp();
+            } else {
+                warp_jacobian(tab, ws, tmid, P, invP, y, M.Jm, M.Ar, M.vec);
+            }
             st.njac++;
             CALJAC = true;
             next = DO_FACT;

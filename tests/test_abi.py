@@ -25,7 +25,7 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 
 def test_struct_layouts_match_header():
-    assert ctypes.sizeof(binding.chem_opts) == 40
+    assert ctypes.sizeof(binding.chem_opts) == 48
     assert binding.STATS_DTYPE.itemsize == 48
     assert ctypes.sizeof(binding.chem_mech_desc) == 8 + 21 * 8
 

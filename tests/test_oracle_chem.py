@@ -325,3 +325,26 @@ def test_configs_integrate_without_failures(mech_h2co, mech_gri):
         y1, st, _ = orc.Mechanism(mech).integrate(y0, P_ATM, t_end, synth.RTOL, synth.ATOL)
         assert np.all(st["status"] == 0)
         assert np.all(np.isfinite(y1)) and y1[:, 1:].min() > -1e-7
+
+
+def test_finite_difference_jacobian_option(mech_h2co):
+    """PAPER.md L82 / Sec. 3.4: first-order FD Jacobian 'based on that of CVODE' (R13).  It costs N extra
+    source terms per Jacobian and must give the same answer within the integration tolerance."""
+    M = orc.Mechanism(mech_h2co)
+    y0 = synth.make_states(mech_h2co, 256, "ignition", 5)
+    ya, sa, _ = M.integrate(y0, P_ATM, 1e-4, 1e-6, 1e-10)
+    yf, sf, _ = M.integrate(y0, P_ATM, 1e-4, 1e-6, 1e-10, fd_jacobian=1)
+    assert np.all(sf["status"] == 0)
+    same = sa["nstep"] == sf["nstep"]
+    assert same.mean() > 0.9
+    # with identical step sequences the only extra work is N source terms per Jacobian evaluation
+    mask = same & (sa["njac"] == sf["njac"]) & (sa["nsol"] == sf["nsol"]) & (sa["naccpt"] == sf["naccpt"])
+    assert mask.mean() > 0.8
+    assert ((sf["nfcn"] - sa["nfcn"])[mask] == (13 * sf["njac"])[mask]).mean() > 0.97
+    Emax, _ = orc.error_metric(yf, ya, 1e-6, 1e-10)
+    assert Emax < 500.0
+    # on a linear problem the difference quotient is exact up to rounding: same result as the analytic Jacobian
+    A = np.array([[-3.0, 1.0], [2.0, -400.0]])
+    y1, s1 = orc.radau5(lambda y: A @ y, lambda y: A, [1.0, 2.0], 1.0, 1e-6, 1e-10)
+    y2, s2 = orc.radau5(lambda y: A @ y, lambda y: 0 * A, [1.0, 2.0], 1.0, 1e-6, 1e-10, fd_jacobian=1)
+    assert np.allclose(y1, y2, rtol=1e-7, atol=1e-12) and s1["naccpt"] == s2["naccpt"]
