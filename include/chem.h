@@ -15,7 +15,7 @@
  *   - LU factorisation of the Jacobian-based matrices on the device:
  *     PAPER.md L86.
  *   - per-IVP internal step counts d_i (divergence measure, Eq. 3): L190.
- * DESIGN.md lists every reading (R1..R12) where the paper is silent.
+ * DESIGN.md lists every reading (R1..R13) where the paper is silent.
  *
  * Conventions
  *   - units: cm, mol, s, K, g/mol, dyn/cm^2 (1 atm = 1.01325e6), Ea in cal/mol.
