@@ -94,7 +94,8 @@ typedef struct chem_opts {
                                    previous global step; read only when reorder = 1.  Results do not depend on it. */
     int32_t fd_jacobian; /* 1: first-order finite-difference Jacobian "based on that of CVODE" (Sec. 3.4;
                             DESIGN.md R13) instead of the analytical one; costs N extra source terms per Jacobian */
-    int32_t reserved;
+    int32_t fixed_steps; /* > 0: take exactly this many equal internal steps without error control (the solver-verification
+                            experiment of PAPER.md L106-L128, Fig. 2); 0: adaptive (default) */
 } chem_opts;
 
 /* Per-state result record written by chem_integrate_ex (device array of n_states). */

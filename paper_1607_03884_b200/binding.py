@@ -35,7 +35,7 @@ class chem_mech_desc(C.Structure):
 class chem_opts(C.Structure):
     _fields_ = [("h0", C.c_double), ("max_steps", C.c_int32), ("newton_max", C.c_int32),
                 ("kernel", C.c_int32), ("reorder", C.c_int32), ("P_per_state", C.c_void_p), ("cost_hint", C.c_void_p),
-                ("fd_jacobian", C.c_int32), ("reserved", C.c_int32)]
+                ("fd_jacobian", C.c_int32), ("fixed_steps", C.c_int32)]
 
 
 STATS_DTYPE = np.dtype([("status", "i4"), ("nstep", "i4"), ("naccpt", "i4"), ("nrejct", "i4"), ("nfcn", "i4"),
@@ -172,13 +172,14 @@ def chem_lu_solve(A, b, stream=None):
     return (torch.view_as_complex(x) if cplx else x), info[:batch]
 
 
-def _opts(h0=0.0, max_steps=0, newton_max=0, kernel=0, reorder=0, P_per_state=None, cost_hint=None, fd_jacobian=0):
+def _opts(h0=0.0, max_steps=0, newton_max=0, kernel=0, reorder=0, P_per_state=None, cost_hint=None, fd_jacobian=0, fixed_steps=0):
     """cost_hint: int32 CUDA tensor [n_states] (e.g. nstep of the previous global step); used when reorder=1"""
     o = chem_opts()
     o.h0, o.max_steps, o.newton_max, o.kernel, o.reorder = h0, max_steps, newton_max, kernel, reorder
     o.P_per_state = P_per_state.data_ptr() if P_per_state is not None else None
     o.cost_hint = cost_hint.data_ptr() if cost_hint is not None else None
     o.fd_jacobian = fd_jacobian
+    o.fixed_steps = fixed_steps
     return o
 
 

@@ -159,7 +159,7 @@ extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double
     prm.max_steps = o ? o->max_steps : 0;
     prm.newton_max = o ? o->newton_max : 0;
     prm.fd_jacobian = o ? o->fd_jacobian : 0;
-    prm.pad_ = 0;
+    prm.fixed_steps = o ? o->fixed_steps : 0;
     prm.rtol_t = 0.1 * std::pow(rtol, 2.0 / 3.0);
     prm.atol_t = prm.rtol_t * (atol / rtol);
     prm.fnewt = std::fmax(10.0 * 2.220446049250313e-16 / prm.rtol_t, std::fmin(0.03, std::sqrt(prm.rtol_t)));

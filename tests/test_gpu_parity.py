@@ -236,3 +236,44 @@ def test_finite_difference_jacobian_matches_oracle(kind, n, kernels, torch_cuda,
         assert Emax < 100.0, Emax
         assert (st["nfcn"] == st_ref["nfcn"]).mean() >= 0.85
         assert (st["njac"] == st_ref["njac"]).mean() >= 0.97
+
+
+@pytest.mark.parametrize("kind,n,kernels", [("h2co", 600, (1, 2)), ("gri", 60, (0,))])
+def test_fixed_step_mode_matches_oracle(kind, n, kernels, torch_cuda, gpu_mechs, orc_mechs, request):
+    """solver-verification mode of PAPER.md L106-L128: a given number of equal internal steps, no error control"""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = descs(request)[kind]
+    y0 = synth.make_states(mech, n, "uniform", 41)
+    for steps in (1, 4, 16):
+        y_ref, st_ref, _ = orc_mechs[kind].integrate(y0, P, 1e-6, RTOL, ATOL, fixed_steps=steps)
+        for kernel in kernels:
+            y, st = binding.chem_integrate_ex(gpu_mechs[kind], P, 1e-6, RTOL, ATOL, torch.from_numpy(y0).cuda(),
+                                              kernel=kernel, fixed_steps=steps)
+            st = binding.stats_to_numpy(st)
+            fin = np.all(np.isfinite(y_ref), axis=1)          # one giant step may legitimately blow up on both sides
+            assert fin.mean() > 0.9
+            assert np.array_equal(st["naccpt"][fin], st_ref["naccpt"][fin]) and np.all(st["naccpt"][fin] == steps)
+            y = y.cpu().numpy()
+            ok = np.all(np.abs(y[fin] - y_ref[fin]) <= 1e-9 + 1e-6 * np.abs(y_ref[fin]), axis=1)
+            assert ok.mean() >= 0.99, (steps, kernel, ok.mean())
+
+
+def test_fixed_step_convergence_like_fig2(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
+    """Fig. 2 of the paper on synthetic states: |E| (Eq. 2) against a tight-tolerance truth falls steeply with the
+    number of internal steps (about four orders of magnitude from 1 to 10 steps for Radau IIA)"""
+    from oracle import oracle as orc
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    y0 = synth.make_states(mech_h2co, 1000, "uniform", 43)
+    truth, st_t, _ = orc_mechs["h2co"].integrate(y0, P, 1e-6, 1e-12, 1e-18)
+    assert np.all(st_t["status"] == 0)
+    E = []
+    for steps in (1, 10, 100):
+        y, _ = binding.chem_integrate_ex(gpu_mechs["h2co"], P, 1e-6, RTOL, ATOL, torch.from_numpy(y0).cuda(), fixed_steps=steps)
+        y = y.cpu().numpy()
+        fin = np.all(np.isfinite(y), axis=1)
+        Emax, Ei = orc.error_metric(y[fin], truth[fin], RTOL, ATOL)
+        E.append(Emax)
+    # oracle values on these states: |E| = 3.7e4, 0.46, 0.22 for 1, 10, 100 steps (then the Newton tolerance floor)
+    assert E[1] < 1e-3 * E[0] and E[2] < 10.0 * E[1] and E[2] < 1.0, E
