@@ -277,3 +277,72 @@ def test_fixed_step_convergence_like_fig2(torch_cuda, gpu_mechs, orc_mechs, mech
         E.append(Emax)
     # oracle values on these states: |E| = 3.7e4, 0.46, 0.22 for 1, 10, 100 steps (then the Newton tolerance floor)
     assert E[1] < 1e-3 * E[0] and E[2] < 10.0 * E[1] and E[2] < 1.0, E
+
+
+def _tiny(rxn_type, **kw):
+    from tests.test_oracle_chem import tiny_mech
+    nasa = np.array([[3.5, 1e-3, 0, 0, 0, 2000.0, 4.0], [4.0, 5e-4, 1e-7, 0, 0, -3000.0, 6.0],
+                     [4.5, 2e-3, -2e-7, 0, 0, -9000.0, 5.0], [2.5, 0, 0, 0, 0, 0.0, 5.0]])
+    return tiny_mech(rxn_type=rxn_type, A=1.0e9, b=0.7, Ea=8000.0, low=(3.0e13, -0.5, 3000.0),
+                     troe=(0.6, 150.0, 1800.0, 4000.0), eff=((0, 3.0), (2, 0.4)), reac=((0, 1), (1, 1)), prod=((2, 1),),
+                     W=(10.0, 18.0, 28.0, 40.0), nasa=nasa, **kw)
+
+
+@pytest.mark.parametrize("rxn_type", [0, 1, 2, 3])
+def test_tiny_mechanisms_every_reaction_type(rxn_type, torch_cuda):
+    """degenerate sizes (4 species, 1 reaction) and the Lindemann type, which the synthetic mechanisms do not contain:
+    source term, Jacobian and integration through both kernels against the oracle"""
+    from oracle import oracle as orc
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = _tiny(rxn_type)
+    gm, om = binding.chem_mech_load(mech), orc.Mechanism(mech)
+    rng = np.random.default_rng(rxn_type)
+    n = 70
+    Y = rng.uniform(0.05, 0.4, (n, 4))
+    Y /= Y.sum(axis=1, keepdims=True)
+    y0 = np.concatenate([rng.uniform(900.0, 1900.0, (n, 1)), Y[:, :3]], axis=1)
+    yd = torch.from_numpy(y0).cuda()
+    f, f_ref = binding.chem_rhs(gm, P, yd).cpu().numpy(), om.rhs(P, y0)
+    assert np.all(np.abs(f - f_ref) <= 1e-10 * np.abs(f_ref).max(axis=1, keepdims=True) + 1e-300)
+    J, J_ref = binding.chem_jacobian(gm, P, yd).cpu().numpy(), om.jacobian(P, y0)
+    assert np.all(np.abs(J - J_ref) <= 1e-9 * np.abs(J_ref).max(axis=1, keepdims=True) + 1e-300)
+    y_ref, st_ref, _ = om.integrate(y0, P, 1e-3, RTOL, ATOL)
+    for kernel in (1, 2):
+        y, st = binding.chem_integrate_ex(gm, P, 1e-3, RTOL, ATOL, yd, kernel=kernel)
+        compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+
+
+def test_mechanism_outside_the_fast_paths(torch_cuda, orc_mechs, mech_h2co):
+    """species with different NASA switch temperatures: neither the warp path nor the exp-job source term applies, the
+    reaction-by-reaction group kernel must give the same answers"""
+    from oracle import oracle as orc
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = dict(mech_h2co)
+    mech["nasa_tmid"] = mech_h2co["nasa_tmid"].copy()
+    mech["nasa_tmid"][3] = 1200.0
+    gm, om = binding.chem_mech_load(mech), orc.Mechanism(mech)
+    y0 = synth.make_states(mech_h2co, 700, "ignition", 51)
+    with pytest.raises(binding.ChemError):
+        binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, torch.from_numpy(y0).cuda(), kernel=2)
+    y_ref, st_ref, _ = om.integrate(y0, P, 1e-5, RTOL, ATOL)
+    y, st = binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, torch.from_numpy(y0).cuda())
+    compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+
+
+def test_single_state_and_per_state_pressure(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    y0 = synth.make_states(mech_h2co, 33, "uniform", 61)
+    y_ref, st_ref, _ = orc_mechs["h2co"].integrate(y0[:1], P, 1e-6, RTOL, ATOL)
+    y, st = binding.chem_integrate_ex(gpu_mechs["h2co"], P, 1e-6, RTOL, ATOL, torch.from_numpy(y0[:1]).cuda())
+    compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+    # per-state pressure: each state at its own P equals separate calls at that P
+    Ps = np.linspace(0.5, 5.0, 33) * P
+    y, _ = binding.chem_integrate_ex(gpu_mechs["h2co"], P, 1e-6, RTOL, ATOL, torch.from_numpy(y0).cuda(),
+                                     P_per_state=torch.from_numpy(Ps).cuda())
+    y = y.cpu().numpy()
+    for s in (0, 16, 32):
+        yr, _, _ = orc_mechs["h2co"].integrate(y0[s:s + 1], float(Ps[s]), 1e-6, RTOL, ATOL)
+        assert np.all(np.abs(y[s] - yr[0]) <= 1e-9 + 1e-6 * np.abs(yr[0]))
