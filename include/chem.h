@@ -142,7 +142,10 @@ int chem_integrate_ex(const chem_mech *mech, int32_t n_states, double P, double 
                       const double *y_in, double *y_out, const chem_opts *opts, chem_stats *stats, void *stream);
 
 /* End-to-end form with HOST buffers (the paper's timings include the transfers):
- * copies y_in to the device, integrates, copies y_out (and stats if not NULL) back, synchronises. */
+ * copies y_in to the device, integrates, copies y_out (and stats if not NULL) back, synchronises.  Large batches are
+ * processed in chunks on two internal streams so that copies overlap kernels (pinned host memory makes the copies
+ * asynchronous); the device staging buffer is cached in the mechanism object.  `reorder` is ignored here.
+ * Not thread-safe per mechanism object. */
 int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
                         const double *y_in_host, double *y_out_host, const chem_opts *opts, chem_stats *stats_host);
 

@@ -52,6 +52,10 @@ struct chem_mech {
     void *fast_blob = nullptr;
     void *order_buf = nullptr;  // scratch of the optional cost ordering (grown on demand)
     size_t order_bytes = 0;
+    // host-buffer entry point: cached device staging buffer and two streams for chunked copy/compute overlap
+    void *host_buf = nullptr;
+    size_t host_bytes = 0;
+    cudaStream_t hs[2] = {nullptr, nullptr};
 };
 
 #include "chem_fast.inl"
@@ -311,6 +315,9 @@ extern "C" void chem_mech_free(chem_mech *m)
     if (m->counter) cudaFree(m->counter);
     if (m->fast_blob) cudaFree(m->fast_blob);
     if (m->order_buf) cudaFree(m->order_buf);
+    if (m->host_buf) cudaFree(m->host_buf);
+    for (int i = 0; i < 2; i++)
+        if (m->hs[i]) cudaStreamDestroy(m->hs[i]);
     delete m;
 }
 

@@ -68,7 +68,7 @@ int launch_eval(const chem_mech *m, int n, double P, const double *y, double *ou
 
 template <int G>
 int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
-                     const chem_opts *o, chem_stats *stats, cudaStream_t st)
+                     const chem_opts *o, chem_stats *stats, cudaStream_t st, int slot)
 {
     const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (block_of<G>() / G);
     int occ = 0;
@@ -77,18 +77,19 @@ int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm
     const int gpb = block_of<G>() / G;
     int grid = (n + gpb - 1) / gpb;
     if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, groups pull work from the queue
-    CUDA_TRY(cudaMemsetAsync(m->counter, 0, sizeof(int), st));
+    int *counter = m->counter + slot;     // one work-queue head per concurrently running launch
+    CUDA_TRY(cudaMemsetAsync(counter, 0, sizeof(int), st));
     int *order = nullptr;
     if (o && o->reorder && o->cost_hint) { rc = build_order(m, n, o->cost_hint, &order, st); if (rc) return rc; }
     integrate_kernel<G><<<grid, block_of<G>(), smem, st>>>(m->t, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats,
-                                                    m->counter, order);
+                                                    counter, order);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return CHEM_OK;
 }
 
 int launch_integrate_warp(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
-                          const chem_opts *o, chem_stats *stats, cudaStream_t st)
+                          const chem_opts *o, chem_stats *stats, cudaStream_t st, int slot)
 {
     const int wpb = kWarpBlock / 32;
     const size_t smem = ((size_t)m->fast.blob_doubles + (size_t)wpb * warp_ws_doubles(m->t.n_sp, m->t.n_rx)) * sizeof(double);
@@ -99,11 +100,12 @@ int launch_integrate_warp(const chem_mech *m, int n, double P, const RadauParams
     if (occ < 1) return fail(CHEM_E_UNSUPPORTED, "warp kernel does not fit on an SM");
     int grid = (n + wpb - 1) / wpb;
     if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, warps pull states from the queue
-    CUDA_TRY(cudaMemsetAsync(m->counter, 0, sizeof(int), st));
+    int *counter = m->counter + slot;
+    CUDA_TRY(cudaMemsetAsync(counter, 0, sizeof(int), st));
     int *order = nullptr;
     if (o && o->reorder && o->cost_hint) { const int rc = build_order(m, n, o->cost_hint, &order, st); if (rc) return rc; }
     integrate_warp_kernel<<<grid, kWarpBlock, smem, st>>>(m->t, m->fast, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out,
-                                                          stats, m->counter, order);
+                                                          stats, counter, order);
     g_launches++;
     CUDA_TRY(cudaGetLastError());
     return CHEM_OK;
@@ -147,8 +149,9 @@ extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const
     return CHEM_OK;
 }
 
-extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
-                                 const double *y_in, double *y_out, const chem_opts *o, chem_stats *stats, void *stream)
+namespace {
+int integrate_impl(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol, const double *y_in,
+                   double *y_out, const chem_opts *o, chem_stats *stats, cudaStream_t st, int slot)
 {
     if (!m || n < 0 || (n > 0 && (!y_in || !y_out))) return fail(CHEM_E_ARG, "bad argument");
     if (!(t_end > 0.0) || !(rtol > 0.0) || !(atol > 0.0)) return fail(CHEM_E_ARG, "t_end, rtol and atol must be positive");
@@ -163,12 +166,18 @@ extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double
     prm.rtol_t = 0.1 * std::pow(rtol, 2.0 / 3.0);
     prm.atol_t = prm.rtol_t * (atol / rtol);
     prm.fnewt = std::fmax(10.0 * 2.220446049250313e-16 / prm.rtol_t, std::fmin(0.03, std::sqrt(prm.rtol_t)));
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int kernel = o ? o->kernel : 0;
     if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "register-resident warp kernel not available for this mechanism");
-    if (kernel != 1 && warp_path_available(m)) return launch_integrate_warp(m, n, P, prm, y_in, y_out, o, stats, st);
-    return group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, st)
-                               : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, st);
+    if (kernel != 1 && warp_path_available(m)) return launch_integrate_warp(m, n, P, prm, y_in, y_out, o, stats, st, slot);
+    return group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, st, slot)
+                               : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, st, slot);
+}
+}  // namespace
+
+extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
+                                 const double *y_in, double *y_out, const chem_opts *o, chem_stats *stats, void *stream)
+{
+    return integrate_impl(m, n, P, t_end, rtol, atol, y_in, y_out, o, stats, static_cast<cudaStream_t>(stream), 0);
 }
 
 extern "C" int chem_integrate(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
@@ -182,25 +191,48 @@ extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, doub
 {
     if (!m || n < 0 || (n > 0 && (!y_in_host || !y_out_host))) return fail(CHEM_E_ARG, "bad argument");
     if (n == 0) return CHEM_OK;
-    const size_t bytes = (size_t)n * m->t.n_sp * sizeof(double);
-    double *d_y = nullptr;
-    chem_stats *d_st = nullptr;
-    CUDA_TRY(cudaMalloc(&d_y, bytes));
+    chem_mech *mm = const_cast<chem_mech *>(m);
+    const int N = m->t.n_sp;
+    const size_t ybytes = (size_t)n * N * sizeof(double), sbytes = stats_host ? (size_t)n * sizeof(chem_stats) : 0;
+    if (ybytes + sbytes > mm->host_bytes) {          // cached staging buffer, grown on demand
+        if (mm->host_buf) cudaFree(mm->host_buf);
+        mm->host_buf = nullptr; mm->host_bytes = 0;
+        CUDA_TRY(cudaMalloc(&mm->host_buf, ybytes + sbytes));
+        mm->host_bytes = ybytes + sbytes;
+    }
+    for (int i = 0; i < 2; i++)
+        if (!mm->hs[i]) CUDA_TRY(cudaStreamCreateWithFlags(&mm->hs[i], cudaStreamNonBlocking));
+    double *d_y = static_cast<double *>(mm->host_buf);
+    chem_stats *d_st = stats_host ? reinterpret_cast<chem_stats *>(static_cast<char *>(mm->host_buf) + ybytes) : nullptr;
+    // chunks alternate between two streams so that the copies of one chunk overlap the kernel of the other
+    // (the paper's GPU timings include the transfers); per-state results do not depend on the chunking
+    const int n_chunks = n >= 65536 ? 2 : 1;     // every extra launch adds one tail (slowest states) of ~2 ms
     int rc = CHEM_OK;
-    if (stats_host && cudaMalloc(&d_st, (size_t)n * sizeof(chem_stats)) != cudaSuccess) {
-        cudaFree(d_y);
-        return fail(CHEM_E_CUDA, "cudaMalloc(stats) failed");
+    cudaError_t e = cudaSuccess;
+    for (int c = 0; c < n_chunks && rc == CHEM_OK && e == cudaSuccess; c++) {
+        const int lo = (int)((long long)n * c / n_chunks), hi = (int)((long long)n * (c + 1) / n_chunks);
+        if (hi == lo) continue;
+        cudaStream_t st = mm->hs[c & 1];
+        chem_opts oc;
+        if (o) {
+            oc = *o;
+            if (oc.P_per_state) oc.P_per_state += lo;
+            oc.reorder = 0;          // the ordering scratch is shared by launches; chunks are short anyway
+            oc.cost_hint = nullptr;
+        }
+        const size_t off = (size_t)lo * N, cnt = (size_t)(hi - lo) * N;
+        e = cudaMemcpyAsync(d_y + off, y_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) break;
+        rc = integrate_impl(m, hi - lo, P, t_end, rtol, atol, d_y + off, d_y + off, o ? &oc : nullptr, d_st ? d_st + lo : nullptr, st, 1 + (c & 1));
+        if (rc != CHEM_OK) break;
+        e = cudaMemcpyAsync(y_out_host + off, d_y + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && stats_host)
+            e = cudaMemcpyAsync(stats_host + lo, d_st + lo, (size_t)(hi - lo) * sizeof(chem_stats), cudaMemcpyDeviceToHost, st);
     }
-    cudaError_t e = cudaMemcpyAsync(d_y, y_in_host, bytes, cudaMemcpyHostToDevice, 0);
-    if (e == cudaSuccess) {
-        rc = chem_integrate_ex(m, n, P, t_end, rtol, atol, d_y, d_y, o, d_st, nullptr);
-        if (rc == CHEM_OK) e = cudaMemcpyAsync(y_out_host, d_y, bytes, cudaMemcpyDeviceToHost, 0);
-        if (rc == CHEM_OK && e == cudaSuccess && stats_host)
-            e = cudaMemcpyAsync(stats_host, d_st, (size_t)n * sizeof(chem_stats), cudaMemcpyDeviceToHost, 0);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+    for (int i = 0; i < 2; i++) {
+        const cudaError_t e2 = cudaStreamSynchronize(mm->hs[i]);
+        if (e == cudaSuccess) e = e2;
     }
-    cudaFree(d_y);
-    if (d_st) cudaFree(d_st);
     if (rc != CHEM_OK) return rc;
     if (e != cudaSuccess) return fail(CHEM_E_CUDA, "chem_integrate_host: %s", cudaGetErrorString(e));
     return CHEM_OK;

@@ -375,16 +375,10 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
             }
             Grp<G>::sync();
             CALJAC = false;
-            if (fixed) {                            // fixed-step mode: new Jacobian every step, H unchanged
-                if (++fixed_done >= fixed) return;
-                if (jobs) cta_rhs3<G>(t, w.cs, w.cx, P, 1, w.y, w.f0, w.a2, w.a3); else rhs<G>(t, w.cs, P, w.y, w.f0);
-                st.nfcn++;
-                next = DO_JAC;
-                continue;
-            }
-            if (LAST) return;
+            if (fixed ? (++fixed_done >= fixed) : LAST) return;
             if (jobs) cta_rhs3<G>(t, w.cs, w.cx, P, 1, w.y, w.f0, w.a2, w.a3); else rhs<G>(t, w.cs, P, w.y, w.f0);
             st.nfcn++;
+            if (fixed) { next = DO_JAC; continue; }   // fixed-step mode: new Jacobian every step, H unchanged
             HNEW = fmin(fabs(HNEW), XEND);
             if (REJECT) HNEW = fmin(HNEW, fabs(H));
             REJECT = false;

@@ -34,6 +34,58 @@ __device__ __forceinline__ WarpMats warp_mats(double *ws, int N)
     return m;
 }
 
+// half-warp 0: E1 = gamma/h I - J (imaginary plane zero), half-warp 1: E2 = (alpha + i beta)/h I - J; lane 16 h + r
+// writes row r.  Returns whether this lane saw a non-finite Jacobian entry.
+__device__ __noinline__ bool warp_form_matrices(const double *Jm, double *Ar, double *Ai, int N, int LD, double FAC1,
+                                                double ALPHN, double BETAN)
+{
+    const int lane = threadIdx.x & 31, h = lane >> 4, r16 = lane & 15;
+    bool nonfinite = false;
+    if (r16 < N) {
+        double *ar = Ar + h * N * LD + r16 * LD, *ai = Ai + h * N * LD + r16 * LD;
+        const double dre = h ? ALPHN : FAC1, dim = h ? BETAN : 0.0;
+#pragma unroll 1
+        for (int j = 0; j < N; j++) {
+            const double v = -Jm[r16 * N + j];
+            nonfinite |= !isfinite(v);
+            ar[j] = (j == r16) ? v + dre : v;
+            ai[j] = (j == r16) ? dim : 0.0;
+        }
+    }
+    return nonfinite;
+}
+
+// CVODE-style difference-quotient Jacobian (R13), three columns per source-term call; out of line so that the
+// rarely used variant does not enlarge the controller's instruction footprint.  Returns the number of source terms.
+__device__ __noinline__ int warp_jacobian_fd(const double *tab, double *ws, double tmid, double P, double invP, double y,
+                                             double f0, double scal, double H, int N, double *Jm)
+{
+    const int lane = threadIdx.x & 31;
+    const bool mine = lane < N;
+    const double UROUND = 2.220446049250313e-16;
+    double fn = 0.0;
+    if (mine) { const double r = f0 / scal; fn = r * r; }
+    const double fnorm = sqrt_s(warp_sum(fn) / N);
+    const double minInc = (fnorm != 0.0) ? 1000.0 * fabs(H) * UROUND * N * fnorm : 1.0;
+    const double inc = fmax(1.4901161193847656e-08 * fabs(y), minInc * scal);
+    int nf = 0;
+#pragma unroll 1
+    for (int j0 = 0; j0 < N; j0 += 3) {
+        const D3 fs = warp_rhs3(tab, ws, tmid, P, invP,
+                                D3{lane == j0 ? y + inc : y, lane == j0 + 1 ? y + inc : y, lane == j0 + 2 ? y + inc : y}, 3);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const int j = j0 + c;
+            const double incj = __shfl_sync(0xffffffffu, inc, j < N ? j : 0);
+            const double fc = c == 0 ? fs.a : (c == 1 ? fs.b : fs.c);
+            if (mine && j < N) Jm[lane * N + j] = (fc - f0) / incj;
+            if (j < N) nf++;
+        }
+    }
+    __syncwarp();
+    return nf;
+}
+
 __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws, double tmid, double P,
                                  const RadauParams &prm, double &y, RadauResult &st)
 {
@@ -82,26 +134,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     for (;;) {
         if (next == DO_JAC) {
             if (prm.fd_jacobian) {
-                // CVODE-style difference quotient, three columns per source-term call (R13)
-                const double scal = ATOL + RTOL * fabs(y);
-                double fn = 0.0;
-                if (mine) { const double r = f0 * iscal; fn = r * r; }
-                const double fnorm = sqrt_s(warp_sum(fn) * invN);
-                const double minInc = (fnorm != 0.0) ? 1000.0 * fabs(H) * UROUND * N * fnorm : 1.0;
-                const double inc = fmax(1.4901161193847656e-08 * fabs(y), minInc * scal);
-                for (int j0 = 0; j0 < N; j0 += 3) {
-                    const D3 fs = warp_rhs3(tab, ws, tmid, P, invP,
-                                            D3{lane == j0 ? y + inc : y, lane == j0 + 1 ? y + inc : y, lane == j0 + 2 ? y + inc : y}, 3);
-#pragma unroll
-                    for (int c = 0; c < 3; c++) {
-                        const int j = j0 + c;
-                        const double incj = __shfl_sync(0xffffffffu, inc, j < N ? j : 0);
-                        const double fc = c == 0 ? fs.a : (c == 1 ? fs.b : fs.c);
-                        if (mine && j < N) M.Jm[lane * N + j] = (fc - f0) / incj;
-                        if (j < N) st.nfcn++;
-                    }
-                }
-                __syncwarp();
+                st.nfcn += warp_jacobian_fd(tab, ws, tmid, P, invP, y, f0, ATOL + RTOL * fabs(y), H, N, M.Jm);
             } else {
                 warp_jacobian(tab, ws, tmid, P, invP, y, M.Jm, M.Ar, M.vec);
             }
@@ -112,18 +145,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         if (next == DO_FACT) {
             const double invH = rcp_f(H);
             const double FAC1 = U1 * invH, ALPHN = ALPH * invH, BETAN = BETA * invH;
-            // half-warp 0: E1 = gamma/h I - J (imaginary plane zero), half-warp 1: E2 = (alpha + i beta)/h I - J
-            bool nonfinite = false;
-            if (r16 < N) {
-                double *ar = M.Ar + h * N * LD + r16 * LD, *ai = M.Ai + h * N * LD + r16 * LD;
-                const double dre = h ? ALPHN : FAC1, dim = h ? BETAN : 0.0;
-                for (int j = 0; j < N; j++) {
-                    const double v = -M.Jm[r16 * N + j];
-                    nonfinite |= !isfinite(v);
-                    ar[j] = (j == r16) ? v + dre : v;
-                    ai[j] = (j == r16) ? dim : 0.0;
-                }
-            }
+            const bool nonfinite = warp_form_matrices(M.Jm, M.Ar, M.Ai, N, LD, FAC1, ALPHN, BETAN);
             int ier = __any_sync(0xffffffffu, nonfinite);
             __syncwarp();
             if (!ier) ier = lu_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi);
@@ -271,16 +293,10 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             }
             iscal = rcp_f(ATOL + RTOL * fabs(y));
             CALJAC = false;
-            if (fixed) {                            // fixed-step mode: new Jacobian every step, H unchanged
-                if (++fixed_done >= fixed) return;
-                f0 = warp_rhs3(tab, ws, tmid, P, invP, D3{y, y, y}, 1).a;
-                st.nfcn++;
-                next = DO_JAC;
-                continue;
-            }
-            if (LAST) return;
+            if (fixed ? (++fixed_done >= fixed) : LAST) return;
             f0 = warp_rhs3(tab, ws, tmid, P, invP, D3{y, y, y}, 1).a;
             st.nfcn++;
+            if (fixed) { next = DO_JAC; continue; }   // fixed-step mode: new Jacobian every step, H unchanged
             HNEW = fmin(fabs(HNEW), XEND);
             if (REJECT) HNEW = fmin(HNEW, fabs(H));
             REJECT = false;
