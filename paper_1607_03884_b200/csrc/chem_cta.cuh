@@ -24,16 +24,6 @@ struct CtaScratch {
     double *red6;        // [6][NW]
 };
 
-__device__ __forceinline__ double cta_rcp(double x)
-{
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    return fma(r, e, r);
-}
-
 // block all-reduce of six sums (deterministic: fixed butterfly, then warps in order)
 template <int G>
 __device__ __forceinline__ void sum6(double (&v)[6], double *red6)
@@ -142,10 +132,10 @@ __device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, co
         const double Fc = o[0], Pr = o[1];
         const double L = log10(Fc);
         const double At = log10(Pr) - 0.4 - 0.67 * L;
-        const double xx = At * cta_rcp(0.75 - 1.27 * L - 0.14 * At);
-        const double F = exp10(L * cta_rcp(1.0 + xx * xx));
+        const double xx = At * rcp_nr(0.75 - 1.27 * L - 0.14 * At);
+        const double F = exp10(L * rcp_nr(1.0 + xx * xx));
         const int s = p / nfo;
-        x.q3[s * NR + (int)o[3]] = Pr * cta_rcp(1.0 + Pr) * F * o[2];
+        x.q3[s * NR + (int)o[3]] = Pr * rcp_nr(1.0 + Pr) * F * o[2];
     }
     Grp<G>::sync();
     // ---- species production rates, temperature equation

@@ -77,6 +77,16 @@ struct Grp {
     }
 };
 
+__device__ __forceinline__ double rcp_nr(double x)   // 1/x for normal x: MUFU seed + two Newton steps
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+
 __device__ __forceinline__ double powi(double c, int nu)
 {
     return nu == 0 ? 1.0 : (nu == 1 ? c : (nu == 2 ? c * c : c * c * c));
@@ -442,16 +452,6 @@ struct Lu2Aux {
     int *perm, *rowk;   // [N] each
     double *rdr, *rdi;  // [N]; rdi unused for the real matrix
 };
-
-__device__ __forceinline__ double rcp_nr(double x)   // 1/x for normal x: MUFU seed + two Newton steps
-{
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    return fma(r, e, r);
-}
 
 // exact arg-max over a warp of (key >= 0 or -1 for inactive, row index); lowest lane wins exact ties
 __device__ __forceinline__ int warp_argmax_row(double v, int row)

@@ -1,4 +1,4 @@
-// chem_fast.inl -- mechanism compiler, part 2: the "exp job" tables of the register-resident warp path
+// chem_fast.inl -- mechanism compiler, part 2: the "exp job" tables of the compact warp-per-state path
 // (chem_warp.cuh).  Included by chem.cu after the definition of chem_mech.
 //
 // Every transcendental of a source-term evaluation becomes  exp(c0 + c1 ln T + c2/T + c3 T + .. + c6 T^4):
@@ -34,7 +34,7 @@ int build_fast(const chem_mech_desc *d, chem_mech *m)
     std::vector<double> job[2] = {std::vector<double>(kJobs * kJobW, 0.0), std::vector<double>(kJobs * kJobW, 0.0)};
     std::vector<double> sp[2] = {std::vector<double>(16 * kJobW, 0.0), std::vector<double>(16 * kJobW, 0.0)};
     std::vector<int> slots(32, 0), type(32, -1), jobs(32, 0);
-    // idle jobs evaluate exp(-inf) = 0 harmlessly?  keep them at exp(0) = 1: all-zero rows.
+    // unused job rows stay all-zero: they evaluate exp(0) = 1 and are never read
     for (int k = 0; k < ns; k++)
         for (int r = 0; r < 2; r++) {
             const double *a = (r ? d->nasa_hi : d->nasa_lo) + 7 * k;

@@ -6,11 +6,9 @@ constexpr int kBlock = 128;   // threads per CTA of the warp-group kernels (G = 
 template <int G>
 __host__ __device__ constexpr int block_of() { return G > kBlock ? G : kBlock; }
 
-// Group <-> CTA mapping: G == 32 -> four warp-groups per CTA, G == 128 -> the CTA is the group.
+// Group <-> CTA mapping: G == 32 -> four warp-groups per CTA, G >= 128 -> the CTA is the group.
 template <int G>
 __device__ __forceinline__ int group_in_block() { return G == 32 ? (int)(threadIdx.x >> 5) : 0; }
-template <int G>
-constexpr int groups_per_block() { return block_of<G>() / G; }
 
 // Next state index from the work queue (PAPER.md L194 names load imbalance between IVPs; groups that
 // finish early pull new states).  Uniform across the group.

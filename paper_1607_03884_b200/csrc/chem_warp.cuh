@@ -9,7 +9,7 @@
 //     exp(c0 + c1 ln T + c2/T + c3 T + c4 T^2 + c5 T^3 + c6 T^4)
 // (forward rate, reverse rate with the equilibrium constant folded in, k0/kinf, the three Troe terms), two
 // jobs per lane.  The code is deliberately compact (rolled loops, one out-of-line copy of every routine):
-// the first version of this kernel was bound by instruction-cache misses (profiles/r1_generic_ncu.md).
+// the first version of this kernel was bound by instruction-cache misses (profiles/r1_history.md).
 #pragma once
 #include "chem_radau.cuh"
 
@@ -57,16 +57,8 @@ __constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120
                                  1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
 __constant__ double kAtanhC[11] = {2.0, 2.0 / 3, 2.0 / 5, 2.0 / 7, 2.0 / 9, 2.0 / 11, 2.0 / 13, 2.0 / 15, 2.0 / 17, 2.0 / 19, 2.0 / 21};
 
-// 1/x for normal x: hardware seed (MUFU.RCP64H) + two Newton steps; no denormal / zero / inf handling
-__device__ __forceinline__ double rcp_f(double x)
-{
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    return fma(r, e, r);
-}
+// 1/x for normal x (rcp_nr, chem_device.cuh): hardware seed + two Newton steps; no denormal / zero / inf handling
+__device__ __forceinline__ double rcp_f(double x) { return rcp_nr(x); }
 // a / b with one residual correction (<= 1 ulp for normal operands)
 __device__ __forceinline__ double div_f(double a, double b)
 {
@@ -505,24 +497,6 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
 }
 
 // ---------------------------------------------------------------------------- LU with rows owned by lanes
-// exact argmax over lanes of a non-negative key v (inactive lanes pass -1): highest 32 bits first, low word
-// only on ties; lowest lane wins exact ties.  Returns -1 if the maximum is not > 0.
-__device__ __forceinline__ int warp_argmax(double v)
-{
-    const bool act = v >= 0.0;
-    const unsigned hi = act ? (unsigned)__double2hiint(v) : 0u;
-    const unsigned m = __reduce_max_sync(0xffffffffu, hi);
-    unsigned cand = __ballot_sync(0xffffffffu, act && hi == m);
-    if (__popc(cand) != 1) {
-        const unsigned lo = (act && hi == m) ? (unsigned)__double2loint(v) : 0u;
-        const unsigned m2 = __reduce_max_sync(0xffffffffu, lo);
-        cand = __ballot_sync(0xffffffffu, act && hi == m && lo == m2);
-        if (m == 0u && m2 == 0u) return -1;
-    }
-    if (cand == 0u) return -1;
-    return __ffs(cand) - 1;
-}
-
 // argmax inside one half-warp (mask hm, half h): returns the row 0..15 of the maximum, or -1.
 __device__ __forceinline__ int half_argmax(double v, unsigned hm, int h)
 {
