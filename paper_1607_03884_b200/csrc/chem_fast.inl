@@ -152,7 +152,7 @@ int build_fast(const chem_mech_desc *d, chem_mech *m)
     }
     auto pad2 = [](size_t n) { return (n + 1) & ~size_t(1); };
     const int o_inc_nu = kOffLists, o_eff_dv = o_inc_nu + (int)pad2(inc_nu.size());
-    const int o_inc_rx = o_eff_dv + (int)pad2(eff_dv.size()), o_eff_sp = o_inc_rx + (int)pad2(inc_rx.size()) / 2 + 1;
+    const int o_inc_rx = o_eff_dv + (int)pad2(eff_dv.size()), o_eff_sp = o_inc_rx + (int)pad2(inc_rx.size()) + 2;
     const int total = (int)pad2(o_eff_sp + pad2(eff_sp.size()) / 2 + 1);
     std::vector<double> host(total, 0.0);
     int *hdr = reinterpret_cast<int *>(host.data());
@@ -165,7 +165,11 @@ int build_fast(const chem_mech_desc *d, chem_mech *m)
     std::memcpy(&host[kOffDesc], desc.data(), 32 * 8 * 4);
     if (!inc_nu.empty()) std::memcpy(&host[o_inc_nu], inc_nu.data(), inc_nu.size() * 8);
     if (!eff_dv.empty()) std::memcpy(&host[o_eff_dv], eff_dv.data(), eff_dv.size() * 8);
-    if (!inc_rx.empty()) std::memcpy(&host[o_inc_rx], inc_rx.data(), inc_rx.size() * 4);
+    {   // incidence entries as (reaction, net coefficient) int pairs: one 8-byte load per entry in the kernels
+        std::vector<int> pairs(2 * inc_rx.size());
+        for (size_t e = 0; e < inc_rx.size(); e++) { pairs[2 * e] = inc_rx[e]; pairs[2 * e + 1] = (int)inc_nu[e]; }
+        if (!pairs.empty()) std::memcpy(&host[o_inc_rx], pairs.data(), pairs.size() * 4);
+    }
     if (!eff_sp.empty()) std::memcpy(&host[o_eff_sp], eff_sp.data(), eff_sp.size() * 4);
     CUDA_TRY(cudaMalloc(&m->fast_blob, host.size() * 8));
     CUDA_TRY(cudaMemcpy(m->fast_blob, host.data(), host.size() * 8, cudaMemcpyHostToDevice));

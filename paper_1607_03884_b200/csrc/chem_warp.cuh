@@ -23,7 +23,7 @@ constexpr int kOffSpHi = kOffSpLo + 16 * kJobW, kOffDesc = kOffSpHi + 16 * kJobW
 constexpr int kOffLists = kOffDesc + 128;
 
 // Tables of the fast path: one blob in global memory, staged into shared memory once per CTA.
-// blob[0..7] is a header of ints: {n_sp, n_rx, off_inc_nu, off_inc_rx, off_eff_dv, off_eff_sp, LD, n_falloff} (offsets in doubles).
+// blob[0..7] is a header of ints: {n_sp, n_rx, off_inc_nu, off_inc (int pairs), off_eff_dv, off_eff_sp, LD, n_falloff} (offsets in doubles).
 struct FastTables {
     int enabled;
     int n_sp, n_rx;
@@ -311,14 +311,13 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     for (int s = 0; s < 3; s++) q[32 * s + lane] = type >= 0 ? cm[s] * rnet[s] : 0.0;
     __syncwarp();
     // species production rates (three stages per pass over the incidence list), temperature equation
-    const double *inc_nu = tab + hdr[2];
-    const int *inc_rx = reinterpret_cast<const int *>(tab + hdr[3]);
+    const int2 *inc = reinterpret_cast<const int2 *>(tab + hdr[3]);      // (reaction, net stoichiometric coefficient)
     double w[3] = {0.0, 0.0, 0.0};
 #pragma unroll 1
     for (int p = d1.z; p < d1.w; p++) {
-        const double nu = inc_nu[p];
-        const int i = inc_rx[p];
-        w[0] += nu * q[i]; w[1] += nu * q[32 + i]; w[2] += nu * q[64 + i];
+        const int2 e = inc[p];
+        const double nu = (double)e.y;
+        w[0] += nu * q[e.x]; w[1] += nu * q[32 + e.x]; w[2] += nu * q[64 + e.x];
     }
     double hw[3], ccp[3];
 #pragma unroll
@@ -436,15 +435,14 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
     const double hRT = spc[0] + T * (spc[1] * 0.5 + T * (spc[2] * (1.0 / 3.0) + T * (spc[3] * 0.25 + T * (spc[4] * 0.2)))) + spc[5] * invT;
     double hw = 0.0, ccp = 0.0, cpw = 0.0, cdcp = 0.0;
     if (lane < N) {
-        const double *inc_nu = tab + hdr[2];
-        const int *inc_rx = reinterpret_cast<const int *>(tab + hdr[3]);
+        const int2 *inc = reinterpret_cast<const int2 *>(tab + hdr[3]);
         double *row = Jm + lane * N;
         for (int l = 0; l < N; l++) row[l] = 0.0;
         double wd = 0.0, dwT = 0.0, u = 0.0;
 #pragma unroll 1
         for (int p = d1.z; p < d1.w; p++) {
-            const int i = inc_rx[p];
-            const double nu = inc_nu[p];
+            const int i = inc[p].x;
+            const double nu = (double)inc[p].y;
             const int4 e0 = desc[2 * i], e1 = desc[2 * i + 1];
             wd += nu * q[i];
             dwT += nu * dqdT[i];
