@@ -48,11 +48,21 @@ __device__ __forceinline__ void sum6(double (&v)[6], double *red6)
     }
 }
 
+struct JobRow { double2 c01, c23, c45, c67; };
+__device__ __forceinline__ JobRow job_load(const double *c)
+{
+    JobRow r;
+    r.c01 = __ldg(reinterpret_cast<const double2 *>(c)); r.c23 = __ldg(reinterpret_cast<const double2 *>(c) + 1);
+    r.c45 = __ldg(reinterpret_cast<const double2 *>(c) + 2); r.c67 = __ldg(reinterpret_cast<const double2 *>(c) + 3);
+    return r;
+}
+__device__ __forceinline__ double job_eval(const JobRow &r, double T, double lnT, double invT)
+{
+    return exp(r.c01.x + r.c01.y * lnT + r.c23.x * invT + T * (r.c23.y + T * (r.c45.x + T * (r.c45.y + T * r.c67.x))));
+}
 __device__ __forceinline__ double job_val(const double *c, double T, double lnT, double invT)
 {
-    const double2 c01 = __ldg(reinterpret_cast<const double2 *>(c)), c23 = __ldg(reinterpret_cast<const double2 *>(c) + 1);
-    const double2 c45 = __ldg(reinterpret_cast<const double2 *>(c) + 2), c67 = __ldg(reinterpret_cast<const double2 *>(c) + 3);
-    return exp(c01.x + c01.y * lnT + c23.x * invT + T * (c23.y + T * (c45.x + T * (c45.y + T * c67.x))));
+    return job_eval(job_load(c), T, lnT, invT);
 }
 
 // Inputs: stage states ys[0..2] (shared, length N); outputs f[0..2] (shared, length N).  nstage = 1 or 3.
@@ -98,12 +108,18 @@ __device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, co
         const int4 d0 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i);       // f012, f345, type, extra job
         const int4 d1 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i + 1);   // falloff ordinal, eff_lo, eff_hi
         const int type = d0.z;
+        // the coefficient rows of k_f and k_r are read once for all stages when the stages share a NASA range (the rule;
+        // job tables live in L2: 49 KB per range for the GRI shape)
+        const double *jt0 = (x.X0[0] <= t.tmid0) ? t.job_lo : t.job_hi;
+        const JobRow rf = job_load(jt0 + (size_t)i * 8), rr = job_load(jt0 + (size_t)(NR + i) * 8);
 #pragma unroll 1
         for (int s = 0; s < nstage; s++) {
             const double T = x.X0[8 * s], lnT = x.X0[8 * s + 1], invT = x.X0[8 * s + 2];
             const double *jt = (T <= t.tmid0) ? t.job_lo : t.job_hi;
             const double *C = x.C3 + 64 * s;
-            const double kf = job_val(jt + (size_t)i * 8, T, lnT, invT), kr = job_val(jt + (size_t)(NR + i) * 8, T, lnT, invT);
+            double kf, kr;
+            if (jt == jt0) { kf = job_eval(rf, T, lnT, invT); kr = job_eval(rr, T, lnT, invT); }
+            else { kf = job_val(jt + (size_t)i * 8, T, lnT, invT); kr = job_val(jt + (size_t)(NR + i) * 8, T, lnT, invT); }
             const double Rf = kf * (C[d0.x & 255] * C[(d0.x >> 8) & 255] * C[(d0.x >> 16) & 255]);
             const double Rr = kr * (C[d0.y & 255] * C[(d0.y >> 8) & 255] * C[(d0.y >> 16) & 255]);
             const double rnet = Rf - Rr;
