@@ -180,17 +180,28 @@ def test_full_size_config1_sampled_against_oracle(torch_cuda, gpu_mechs, orc_mec
     assert (st["nstep"][idx] == st_ref["nstep"]).mean() >= 0.99
 
 
-def test_full_size_gri_sampled_against_oracle(torch_cuda, gpu_mechs, orc_mechs, mech_gri):
-    """configs[3] shape (gri, dt = 1e-6) on a 16,384-state slice of the full batch, sampled against the oracle"""
+@pytest.mark.parametrize("ci,n_sample", [(2, 1024), (3, 128), (4, 96)])
+def test_full_size_other_configs_sampled_against_oracle(ci, n_sample, torch_cuda, gpu_mechs, orc_mechs, request):
+    """BASELINE.json configs[2..4] at FULL size through the plain entry point; a random sample (plus the ragged tail) is
+    recomputed by the oracle one by one; element conservation is checked on every state"""
     from paper_1607_03884_b200 import binding
     torch = torch_cuda
-    cfg = synth.CONFIGS[3]
-    n = 16384
-    y0 = synth.make_states(mech_gri, n, cfg["dist"], synth.STATE_SEED)
-    y1 = binding.chem_integrate(gpu_mechs["gri"], P, cfg["t_end"], RTOL, ATOL, torch.from_numpy(y0).cuda()).cpu().numpy()
+    cfg = synth.CONFIGS[ci]
+    mech = descs(request)[cfg["kind"]]
+    y0 = synth.make_states(mech, cfg["n_states"], cfg["dist"], synth.STATE_SEED)
+    y1 = binding.chem_integrate(gpu_mechs[cfg["kind"]], P, cfg["t_end"], RTOL, ATOL, torch.from_numpy(y0).cuda()).cpu().numpy()
     assert np.all(np.isfinite(y1))
-    idx = np.random.default_rng(5).choice(n, 96, replace=False)
-    y_ref, st_ref, _ = orc_mechs["gri"].integrate(y0[idx], P, cfg["t_end"], RTOL, ATOL)
+    W, comp = mech["mol_weight"], mech["elem_comp"].astype(np.float64)
+
+    def elem(y):
+        Y = np.concatenate([y[:, 1:], 1.0 - y[:, 1:].sum(axis=1, keepdims=True)], axis=1)
+        return (Y / W) @ comp
+    assert np.abs(elem(y1) - elem(y0)).max() < 1e-11
+    rng = np.random.default_rng(1000 + ci)
+    idx = np.unique(np.concatenate([rng.choice(cfg["n_states"], n_sample, replace=False),
+                                    np.arange(cfg["n_states"] - 5, cfg["n_states"])]))
+    y_ref, st_ref, _ = orc_mechs[cfg["kind"]].integrate(y0[idx], P, cfg["t_end"], RTOL, ATOL)
+    assert np.all(st_ref["status"] == 0)
     assert np.all(np.abs(y1[idx] - y_ref) <= 1e-9 + 1e-6 * np.abs(y_ref))
 
 
