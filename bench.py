@@ -229,7 +229,8 @@ def main():
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                      "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-                     "kernel": "integrate_kernel", "kernel_ms": 1e3 * kernel_s, "flops_per_launch": flops_per_launch,
+                     "kernel": ("integrate_warp_kernel" if (N <= 16 and args.kernel != 1) else "integrate_kernel<128>"),
+                     "kernel_ms": 1e3 * kernel_s, "flops_per_launch": flops_per_launch,
                      "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
                      "hbm_frac": (2 * n * N * 8 / kernel_s / 1e9) / peaks["hbm_gbs"], "hbm_peak_source": which},
     }
