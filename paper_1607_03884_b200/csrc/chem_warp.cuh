@@ -495,21 +495,24 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
 }
 
 // ---------------------------------------------------------------------------- LU with rows owned by lanes
-// argmax inside one half-warp (mask hm, half h): returns the row 0..15 of the maximum, or -1.
-__device__ __forceinline__ int half_argmax(double v, unsigned hm, int h)
+// Separate arg-max in each half-warp with FULL-mask collectives only (partial-mask reductions take a slow
+// WARPSYNC path): returns the row 0..15 of the maximum of key v (>= 0, or -1 for inactive lanes) within the
+// caller's half h, or -1 if that maximum is not > 0.  Highest word first, low word on ties, lowest row wins exact ties.
+__device__ __forceinline__ int half_argmax(double v, int h)
 {
     const bool act = v >= 0.0;
     const unsigned hi = act ? (unsigned)__double2hiint(v) : 0u;
-    const unsigned m = __reduce_max_sync(hm, hi);
-    unsigned cand = __ballot_sync(hm, act && hi == m) & hm;
-    if (__popc(cand) != 1) {
+    const unsigned m0 = __reduce_max_sync(0xffffffffu, h ? 0u : hi), m1 = __reduce_max_sync(0xffffffffu, h ? hi : 0u);
+    const unsigned m = h ? m1 : m0;
+    unsigned cand = (__ballot_sync(0xffffffffu, act && hi == m) >> (16 * h)) & 0xffffu;
+    if (__any_sync(0xffffffffu, __popc(cand) != 1)) {
         const unsigned lo = (act && hi == m) ? (unsigned)__double2loint(v) : 0u;
-        const unsigned m2 = __reduce_max_sync(hm, lo);
-        cand = __ballot_sync(hm, act && hi == m && lo == m2) & hm;
-        if (m == 0u && m2 == 0u) return -1;
+        const unsigned l0 = __reduce_max_sync(0xffffffffu, h ? 0u : lo), l1 = __reduce_max_sync(0xffffffffu, h ? lo : 0u);
+        const unsigned m2 = h ? l1 : l0;
+        cand = (__ballot_sync(0xffffffffu, act && hi == m && lo == m2) >> (16 * h)) & 0xffffu;
+        if (m == 0u && m2 == 0u) cand = 0u;
     }
-    if (cand == 0u) return -1;
-    return __ffs(cand) - 1 - 16 * h;
+    return cand ? __ffs(cand) - 1 : -1;
 }
 
 // LU of BOTH Radau matrices in one instruction stream: half-warp 0 factors the real matrix E1 (imaginary plane
@@ -521,7 +524,6 @@ __device__ __noinline__ int lu_warp_pair(double *Ar, double *Ai, int LD, int N, 
                                          double &rdi_out)
 {
     const int lane = threadIdx.x & 31, h = lane >> 4, r = lane & 15;
-    const unsigned hm = h ? 0xffff0000u : 0x0000ffffu;
     double *Pr_ = Ar + h * N * LD, *Pi_ = Ai + h * N * LD;
     double *rr = Pr_ + (r < N ? r : 0) * LD, *ri = Pi_ + (r < N ? r : 0) * LD;
     int myk = -1;
@@ -529,7 +531,7 @@ __device__ __noinline__ int lu_warp_pair(double *Ar, double *Ai, int LD, int N, 
     for (int k = 0; k < N; k++) {
         const bool act = (r < N) && (myk < 0);
         const double akr = rr[k], aki = ri[k];
-        const int p = half_argmax(act ? fabs(akr) + fabs(aki) : -1.0, hm, h);
+        const int p = half_argmax(act ? fabs(akr) + fabs(aki) : -1.0, h);
         const double *pr_ = Pr_ + (p < 0 ? 0 : p) * LD, *pi_ = Pi_ + (p < 0 ? 0 : p) * LD;
         const double pr = pr_[k], pi = pi_[k];
         const double den = rcp_f(pr * pr + pi * pi);
