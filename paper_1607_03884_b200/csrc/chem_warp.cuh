@@ -543,11 +543,13 @@ __device__ __noinline__ int lu_warp_pair(double *Ar, double *Ai, int LD, int N, 
             const double lr = akr * qr - aki * qi, li = akr * qi + aki * qr;
             rr[k] = lr;
             ri[k] = li;
-#pragma unroll 2
-            for (int j = k + 1; j < N; j++) {
-                const double ur = pr_[j], ui = pi_[j];
-                rr[j] = fma(-lr, ur, fma(li, ui, rr[j]));
-                ri[j] = fma(-lr, ui, fma(-li, ur, ri[j]));
+            const double *up = pr_ + k + 1, *uq = pi_ + k + 1;
+            double *xp = rr + k + 1, *xq = ri + k + 1;
+#pragma unroll 1
+            for (int n = N - 1 - k; n > 0; n--, up++, uq++, xp++, xq++) {
+                const double ur = *up, ui = *uq;
+                *xp = fma(-lr, ur, fma(li, ui, *xp));
+                *xq = fma(-lr, ui, fma(-li, ur, *xq));
             }
         }
         __syncwarp();
