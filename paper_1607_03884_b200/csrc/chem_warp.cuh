@@ -204,8 +204,8 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
         sY[s] = Yk[s];
         sYW[s] = Yk[s] * invWk;
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll 1
+    for (int o = 16; o > 0; o >>= 1)      // rolled on purpose: code size matters more than the loop overhead here
 #pragma unroll
         for (int s = 0; s < 3; s++) {
             sY[s] += __shfl_xor_sync(0xffffffffu, sY[s], o);
@@ -329,7 +329,7 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
         hw[s] = lane < N ? hRT * w[s] : 0.0;
         ccp[s] = lane < N ? Ck[s] * cpR : 0.0;
     }
-#pragma unroll
+#pragma unroll 1
     for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
         for (int s = 0; s < 3; s++) {
