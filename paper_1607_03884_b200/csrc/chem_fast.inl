@@ -162,7 +162,11 @@ int build_fast(const chem_mech_desc *d, chem_mech *m)
     std::memcpy(&host[kOffJobHi], job[1].data(), kJobs * kJobW * 8);
     std::memcpy(&host[kOffSpLo], sp[0].data(), 16 * kJobW * 8);
     std::memcpy(&host[kOffSpHi], sp[1].data(), 16 * kJobW * 8);
-    std::memcpy(&host[kOffDesc], desc.data(), 32 * 8 * 4);
+    {   // descriptor words as two planes of int4 per lane (conflict-free 16-byte loads)
+        int *dst = reinterpret_cast<int *>(&host[kOffDesc]);
+        for (int l = 0; l < 32; l++)
+            for (int c = 0; c < 8; c++) dst[(c < 4 ? 0 : 128) + 4 * l + (c & 3)] = desc[8 * l + c];
+    }
     if (!inc_nu.empty()) std::memcpy(&host[o_inc_nu], inc_nu.data(), inc_nu.size() * 8);
     if (!eff_dv.empty()) std::memcpy(&host[o_eff_dv], eff_dv.data(), eff_dv.size() * 8);
     {   // incidence entries as (reaction, net coefficient) int pairs: one 8-byte load per entry in the kernels

@@ -15,11 +15,11 @@
 
 namespace chem {
 
-constexpr int kJobW = 8;     // doubles per job row (7 used)
+constexpr int kJobW = 9;     // doubles per job row (7 used; 8 for species rows); ODD: lane-per-row reads are bank-conflict free
 constexpr int kJobs = 64;    // 2 rounds x 32 lanes
 // fixed part of the staged table blob (doubles)
 constexpr int kOffJobLo = 8, kOffJobHi = kOffJobLo + kJobs * kJobW, kOffSpLo = kOffJobHi + kJobs * kJobW;
-constexpr int kOffSpHi = kOffSpLo + 16 * kJobW, kOffDesc = kOffSpHi + 16 * kJobW;   // desc: 32 lanes x 8 ints = 128 doubles
+constexpr int kOffSpHi = kOffSpLo + 16 * kJobW, kOffDesc = kOffSpHi + 16 * kJobW;   // desc: 2 planes x 32 lanes x int4 = 128 doubles
 constexpr int kOffLists = kOffDesc + 128;
 
 // Tables of the fast path: one blob in global memory, staged into shared memory once per CTA.
@@ -189,8 +189,8 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     const int lane = threadIdx.x & 31;
     const int *hdr = reinterpret_cast<const int *>(tab);
     const int N = hdr[0];
-    const int4 d0 = reinterpret_cast<const int4 *>(tab + kOffDesc)[2 * lane];       // factors, troe ordinal, type, jobs
-    const int4 d1 = reinterpret_cast<const int4 *>(tab + kOffDesc)[2 * lane + 1];   // eff_lo, eff_hi, inc_lo, inc_hi
+    const int4 d0 = reinterpret_cast<const int4 *>(tab + kOffDesc)[lane];       // factors, troe ordinal, type, jobs
+    const int4 d1 = reinterpret_cast<const int4 *>(tab + kOffDesc)[32 + lane];   // eff_lo, eff_hi, inc_lo, inc_hi
     double *C = ws + kWsC, *E = ws + kWsE, *q = ws + kWsQ, *X = ws + kWsX;
     const int row = lane < N ? lane : 0;
     double T[3], Yk[3], sY[3], sYW[3];
@@ -362,7 +362,7 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
     const int *hdr = reinterpret_cast<const int *>(tab);
     const int N = hdr[0];
     const int4 *desc = reinterpret_cast<const int4 *>(tab + kOffDesc);
-    const int4 d0 = desc[2 * lane], d1 = desc[2 * lane + 1];
+    const int4 d0 = desc[lane], d1 = desc[32 + lane];
     double *C = ws + kWsC, *E = ws + kWsE, *q = ws + kWsQ;
     double *dq = scr, *dqdT = scr + 192, *tb = scr + 224;
     const double *eff_dv = tab + hdr[4];
@@ -443,7 +443,7 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
         for (int p = d1.z; p < d1.w; p++) {
             const int i = inc[p].x;
             const double nu = (double)inc[p].y;
-            const int4 e0 = desc[2 * i], e1 = desc[2 * i + 1];
+            const int4 e0 = desc[i], e1 = desc[32 + i];
             wd += nu * q[i];
             dwT += nu * dqdT[i];
 #pragma unroll
