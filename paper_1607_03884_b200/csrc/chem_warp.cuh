@@ -437,6 +437,7 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
     if (lane < N) {
         const int2 *inc = reinterpret_cast<const int2 *>(tab + hdr[3]);
         double *row = Jm + lane * N;
+#pragma unroll 1
         for (int l = 0; l < N; l++) row[l] = 0.0;
         double wd = 0.0, dwT = 0.0, u = 0.0;
 #pragma unroll 1
@@ -453,11 +454,14 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
             }
             const double v = nu * tb[i];
             u += v;
+#pragma unroll 1
             for (int pe = e1.x; pe < e1.y; pe++) row[eff_sp[pe]] += v * eff_dv[pe];
         }
         double GC = 0.0;
+#pragma unroll 1
         for (int l = 0; l < N; l++) GC += row[l] * C[l];
         const double GN = row[N - 1] * invWN;
+#pragma unroll 1
         for (int j = N - 1; j >= 1; j--) {
             const double iw = spt[(j - 1) * kJobW + 7];
             row[j] = -m.Wbar * (iw - invWN) * GC + m.rho * (row[j - 1] * iw - GN);
@@ -475,6 +479,7 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
     if (lane < N) {
         const int j = lane;
         double S = 0.0;
+#pragma unroll 1
         for (int k = 0; k < N; k++) S += vec[16 + k] * Jm[k * N + j];
         double dlnrho, drcp;
         if (j == 0) {
@@ -485,6 +490,7 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
             dlnrho = -m.Wbar * (iw - invWN);
             drcp = dlnrho * ccp + m.rho * (vec[32 + j - 1] * iw - vec[32 + N - 1] * invWN);
         }
+#pragma unroll 1
         for (int k = N - 2; k >= 0; k--) {
             const double Wr = spt[k * kJobW + 6] * m.inv_rho;
             Jm[(k + 1) * N + j] = Wr * (Jm[k * N + j] - vec[k] * dlnrho);
