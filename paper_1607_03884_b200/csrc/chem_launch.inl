@@ -166,6 +166,7 @@ int integrate_impl(const chem_mech *m, int32_t n, double P, double t_end, double
     prm.rtol_t = 0.1 * std::pow(rtol, 2.0 / 3.0);
     prm.atol_t = prm.rtol_t * (atol / rtol);
     prm.fnewt = std::fmax(10.0 * 2.220446049250313e-16 / prm.rtol_t, std::fmin(0.03, std::sqrt(prm.rtol_t)));
+    prm.inv_fnewt = 1.0 / prm.fnewt; prm.inv_n = 1.0 / m->t.n_sp; prm.inv_3n = 1.0 / (3 * m->t.n_sp);
     const int kernel = o ? o->kernel : 0;
     if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "register-resident warp kernel not available for this mechanism");
     if (kernel != 1 && warp_path_available(m)) return launch_integrate_warp(m, n, P, prm, y_in, y_out, o, stats, st, slot);

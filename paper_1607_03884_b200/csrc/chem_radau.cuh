@@ -86,6 +86,7 @@ struct RadauParams {
     int fd_jacobian;                // 1: CVODE-style difference-quotient Jacobian (R13)
     int fixed_steps;                // > 0: that many equal steps, no error control
     double rtol_t, atol_t, fnewt;   // RADAU5's transformed tolerances and Newton stopping level (R8), set on the host
+    double inv_fnewt, inv_n, inv_3n; // 1/fnewt, 1/N, 1/(3N): host-side divisions for the warp path
 };
 
 struct RadauResult {

@@ -103,7 +103,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     const int h = lane >> 4, r16 = lane & 15;
     const int LD = M.LD;
     const bool mine = lane < N;
-    const double invN = 1.0 / N, inv3N = 1.0 / (3 * N), invFNEWT = 1.0 / FNEWT;
+    const double invN = prm.inv_n, inv3N = prm.inv_3n, invFNEWT = prm.inv_fnewt;
     const double invP = rcp_f(P);
 
     st.status = 0; st.nstep = 0; st.naccpt = 0; st.nrejct = 0; st.nfcn = 0; st.njac = 0; st.ndec = 0; st.nsol = 0;

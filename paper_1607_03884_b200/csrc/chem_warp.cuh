@@ -46,7 +46,6 @@ __device__ __forceinline__ void warp_sum2(double &a, double &b)
         b += __shfl_xor_sync(0xffffffffu, b, o);
     }
 }
-__device__ __noinline__ double pow_ni(double a, double b) { return pow(a, b); }
 constexpr double kLn10 = 2.302585092994045684, kInvLn10 = 0.4342944819032518277;
 
 // Compact fp64 elementary functions for normal, finite arguments (the rates, temperatures and step-size ratios of
@@ -123,6 +122,9 @@ __device__ __forceinline__ double log_f(double x)
 }
 __device__ __noinline__ double exp_ni(double a) { return exp_f(a); }
 __device__ __noinline__ double log_ni(double a) { return log_f(a); }
+// a^b for normal a > 0 (step-size controller only): exp(b ln a) from the compact routines above, ~|b ln a| ulp;
+// the library pow() is a 270-instruction routine that this instruction-fetch-bound kernel would stream in twice per step
+__device__ __forceinline__ double pow_ni(double a, double b) { return exp_ni(b * log_ni(a)); }
 
 // per-warp scratch layout (doubles), three stage slots each: C[3][32] (C[s][31] = 1 for unused factor slots),
 // E[3][64] exp-job results, q[3][32] rates of progress, X[48] stage parameters and phase-2 jobs; then matrices
