@@ -72,7 +72,7 @@ __device__ __noinline__ int warp_jacobian_fd(const double *tab, double *ws, doub
 #pragma unroll 1
     for (int j0 = 0; j0 < N; j0 += 3) {
         const D3 fs = warp_rhs3(tab, ws, tmid, P, invP,
-                                D3{lane == j0 ? y + inc : y, lane == j0 + 1 ? y + inc : y, lane == j0 + 2 ? y + inc : y}, 3);
+                                D3{lane == j0 ? y + inc : y, lane == j0 + 1 ? y + inc : y, lane == j0 + 2 ? y + inc : y});
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             const int j = j0 + c;
@@ -122,7 +122,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     double FACCON = 1.0, THETA = 0.0, HACC = 0.0, ERRACC = 0.0;
     int NSING = 0;
     double iscal = rcp_f(ATOL + RTOL * fabs(y));     // 1 / scal
-    double f0 = warp_rhs3(tab, ws, tmid, P, invP, D3{y, y, y}, 1).a;
+    double f0 = warp_rhs1(tab, ws, tmid, P, invP, y);
     st.nfcn++;
     double z1 = 0, z2 = 0, z3 = 0, w1 = 0, w2 = 0, w3 = 0, c1 = 0, c2 = 0, c3 = 0;
     // LU factors
@@ -183,7 +183,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         int outcome = 0;
         for (;;) {
             if (NEWT >= NIT) { if (!fixed) outcome = 2; break; }
-            const D3 fs = warp_rhs3(tab, ws, tmid, P, invP, D3{y + z1, y + z2, y + z3}, 3);
+            const D3 fs = warp_rhs3(tab, ws, tmid, P, invP, D3{y + z1, y + z2, y + z3});
             const double a1 = fs.a, a2 = fs.b, a3 = fs.c;
             st.nfcn += 3;
             z1 = TI11 * a1 + TI12 * a2 + TI13 * a3 - w1 * FAC1;
@@ -252,7 +252,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             ERR = fmax(sqrt_s(warp_sum(e) * invN), 1.0e-10);
             if (ERR >= 1.0 && (FIRST || REJECT)) {
                 const double yc = y + cont;
-                const double fr = warp_rhs3(tab, ws, tmid, P, invP, D3{yc, yc, yc}, 1).a;
+                const double fr = warp_rhs1(tab, ws, tmid, P, invP, yc);
                 st.nfcn++;
                 cont = solve_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi, h ? 0.0 : fr + f2, 0.0).x;
                 e = 0.0;
@@ -294,7 +294,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             iscal = rcp_f(ATOL + RTOL * fabs(y));
             CALJAC = false;
             if (fixed ? (++fixed_done >= fixed) : LAST) return;
-            f0 = warp_rhs3(tab, ws, tmid, P, invP, D3{y, y, y}, 1).a;
+            f0 = warp_rhs1(tab, ws, tmid, P, invP, y);
             st.nfcn++;
             if (fixed) { next = DO_JAC; continue; }   // fixed-step mode: new Jacobian every step, H unchanged
             HNEW = fmin(fabs(HNEW), XEND);

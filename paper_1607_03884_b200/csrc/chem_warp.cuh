@@ -186,7 +186,8 @@ struct D3 { double a, b, c; };
 // Batching the stages lets one instruction stream serve 3 x 64 exp jobs, lets single lanes take the serial
 // transcendentals (ln T, reciprocals, the Troe broadening factor of every (reaction, stage) pair) in
 // parallel, and shares every table read.  tab = staged table blob (shared), ws = this warp's scratch (shared).
-__device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid, double P, double invP, D3 y, int nstage)
+template <int NS>
+__device__ __forceinline__ D3 warp_rhs_body(const double *tab, double *ws, double tmid, double P, double invP, D3 y)
 {
     const int lane = threadIdx.x & 31;
     const int *hdr = reinterpret_cast<const int *>(tab);
@@ -195,13 +196,16 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     const int4 d1 = reinterpret_cast<const int4 *>(tab + kOffDesc)[32 + lane];   // eff_lo, eff_hi, inc_lo, inc_hi
     double *C = ws + kWsC, *E = ws + kWsE, *q = ws + kWsQ, *X = ws + kWsX;
     const int row = lane < N ? lane : 0;
-    double T[3], Yk[3], sY[3], sYW[3];
-    T[0] = __shfl_sync(0xffffffffu, y.a, 0); T[1] = __shfl_sync(0xffffffffu, y.b, 0); T[2] = __shfl_sync(0xffffffffu, y.c, 0);
-    Yk[0] = __shfl_down_sync(0xffffffffu, y.a, 1); Yk[1] = __shfl_down_sync(0xffffffffu, y.b, 1);
-    Yk[2] = __shfl_down_sync(0xffffffffu, y.c, 1);
+    double T[NS], Yk[NS], sY[NS], sYW[NS];
+    const double yin[3] = {y.a, y.b, y.c};
+#pragma unroll
+    for (int s = 0; s < NS; s++) {
+        T[s] = __shfl_sync(0xffffffffu, yin[s], 0);
+        Yk[s] = __shfl_down_sync(0xffffffffu, yin[s], 1);
+    }
     const double invWk = tab[kOffSpLo + row * kJobW + 7], invWN = tab[kOffSpLo + (N - 1) * kJobW + 7];
 #pragma unroll
-    for (int s = 0; s < 3; s++) {
+    for (int s = 0; s < NS; s++) {
         if (lane >= N - 1) Yk[s] = 0.0;
         sY[s] = Yk[s];
         sYW[s] = Yk[s] * invWk;
@@ -209,28 +213,30 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
 #pragma unroll 1
     for (int o = 16; o > 0; o >>= 1)      // rolled on purpose: code size matters more than the loop overhead here
 #pragma unroll
-        for (int s = 0; s < 3; s++) {
+        for (int s = 0; s < NS; s++) {
             sY[s] += __shfl_xor_sync(0xffffffffu, sY[s], o);
             sYW[s] += __shfl_xor_sync(0xffffffffu, sYW[s], o);
         }
-    double sW[3];
+    double sW[NS];
 #pragma unroll
-    for (int s = 0; s < 3; s++) {
+    for (int s = 0; s < NS; s++) {
         const double YN = 1.0 - sY[s];                      // closure: last species
         if (lane == N - 1) Yk[s] = YN;
         sW[s] = sYW[s] + YN * invWN;                        // 1 / Wbar
     }
     // serial transcendentals, one lane each: lanes 0-2 take T_s (ln, 1/x), lanes 3-5 take 1/Wbar_s (1/x)
-    const int sl3 = lane % 3;
-    const double Tsel = sl3 == 0 ? T[0] : (sl3 == 1 ? T[1] : T[2]);
-    const double Wsel = sl3 == 0 ? sW[0] : (sl3 == 1 ? sW[1] : sW[2]);
-    const double lnsel = log_f(Tsel);
-    const double rsel = rcp_f((lane >= 3 && lane < 6) ? Wsel : Tsel);
-    double invT[3], rho[3], inv_rho[3], Ck[3];
+    const int sl3 = lane % NS;
+    double Tsel = T[0], Wsel = sW[0];
 #pragma unroll
-    for (int s = 0; s < 3; s++) {
+    for (int s = 1; s < NS; s++)
+        if (sl3 == s) { Tsel = T[s]; Wsel = sW[s]; }
+    const double lnsel = log_f(Tsel);
+    const double rsel = rcp_f((lane >= NS && lane < 2 * NS) ? Wsel : Tsel);
+    double invT[NS], rho[NS], inv_rho[NS], Ck[NS];
+#pragma unroll
+    for (int s = 0; s < NS; s++) {
         invT[s] = __shfl_sync(0xffffffffu, rsel, s);
-        const double Wbar = __shfl_sync(0xffffffffu, rsel, 3 + s);
+        const double Wbar = __shfl_sync(0xffffffffu, rsel, NS + s);
         const double lnT = __shfl_sync(0xffffffffu, lnsel, s);
         rho[s] = P * Wbar * invT[s] * (1.0 / kRerg);
         inv_rho[s] = kRerg * T[s] * sW[s] * invP;
@@ -241,24 +247,21 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     __syncwarp();
     // exp jobs: 3 stages x 2 rounds per lane, one rolled loop
 #pragma unroll 1
-    for (int it = 0; it < 2 * nstage; it++) {     // nstage = 1: the three inputs are copies, stage 0 only
+    for (int it = 0; it < 2 * NS; it++) {
         const int s = it >> 1, r = it & 1;
         const double Ts = X[4 * s], lnT = X[4 * s + 1], iT = X[4 * s + 2];
         const double *c = tab + (Ts <= tmid ? kOffJobLo : kOffJobHi) + (32 * r + lane) * kJobW;
         E[kJobs * s + 32 * r + lane] = exp_f(job_arg(c, Ts, lnT, iT));
     }
     __syncwarp();
-    if (nstage == 1) {                                // replicate stage 0 (same state): keeps the rest branch-free
-        E[kJobs + lane] = E[lane]; E[kJobs + 32 + lane] = E[32 + lane];
-        E[2 * kJobs + lane] = E[lane]; E[2 * kJobs + 32 + lane] = E[32 + lane];
-        __syncwarp();
-    }
     // rates of progress of reaction `lane` at the three stages; factors: species indices with multiplicity, 31 = unity
     const int type = d0.z;
-    double rnet[3] = {0.0, 0.0, 0.0}, cm[3] = {1.0, 1.0, 1.0};
+    double rnet[NS], cm[NS];
+#pragma unroll
+    for (int s = 0; s < NS; s++) { rnet[s] = 0.0; cm[s] = 1.0; }
     if (type >= 0) {
 #pragma unroll
-        for (int s = 0; s < 3; s++) {
+        for (int s = 0; s < NS; s++) {
             const double *Cs = C + 32 * s, *Es = E + kJobs * s;
             const double Rf = Es[lane] * (Cs[d0.x & 31] * Cs[(d0.x >> 5) & 31] * Cs[(d0.x >> 10) & 31]);
             const double Rr = Es[32 + lane] * (Cs[(d0.x >> 15) & 31] * Cs[(d0.x >> 20) & 31] * Cs[(d0.x >> 25) & 31]);
@@ -268,18 +271,19 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
             const double *eff_dv = tab + hdr[4];
             const int *eff_sp = reinterpret_cast<const int *>(tab + hdr[5]);
 #pragma unroll
-            for (int s = 0; s < 3; s++) cm[s] = P * invT[s] * (1.0 / kRerg);
+            for (int s = 0; s < NS; s++) cm[s] = P * invT[s] * (1.0 / kRerg);
 #pragma unroll 1
             for (int p = d1.x; p < d1.y; p++) {
                 const double dv = eff_dv[p];
                 const int sp = eff_sp[p];
-                cm[0] += dv * C[sp]; cm[1] += dv * C[32 + sp]; cm[2] += dv * C[64 + sp];
+                #pragma unroll
+                for (int s = 0; s < NS; s++) cm[s] += dv * C[32 * s + sp];
             }
             if (type >= 2) {
                 // hand (Fcent, Pr) of every (reaction, stage) pair to the phase-2 lanes; Lindemann: Fcent = 1
-                const int slot = 12 + 6 * d0.y;
+                const int slot = 12 + 2 * NS * d0.y;
 #pragma unroll
-                for (int s = 0; s < 3; s++) {
+                for (int s = 0; s < NS; s++) {
                     const double *Es = E + kJobs * s;
                     const int ts = (d0.w >> 8) & 255;
                     X[slot + 2 * s] = type == 3 ? Es[ts] + Es[ts + 1] + Es[ts + 2] : 1.0;
@@ -292,7 +296,7 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     // phase 2: lane pair (2p, 2p+1) serves falloff pair p = (ordinal, stage): c = Pr/(1+Pr) F  (R5)
     {
         const int nfo = hdr[7];                                   // number of falloff reactions
-        const bool live = lane < 6 * nfo;
+        const bool live = lane < 2 * NS * nfo;
         const double v = live ? X[12 + lane] : 1.0;
         const double lg = log_f(v) * kInvLn10;                      // even lane: log10 Fcent, odd lane: log10 Pr
         const double lPr = __shfl_down_sync(0xffffffffu, lg, 1);
@@ -306,24 +310,28 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     }
     __syncwarp();
     if (type >= 2) {
-        const int slot = 12 + 6 * d0.y;
-        cm[0] = X[slot]; cm[1] = X[slot + 2]; cm[2] = X[slot + 4];
+        const int slot = 12 + 2 * NS * d0.y;
+        #pragma unroll
+        for (int s = 0; s < NS; s++) cm[s] = X[slot + 2 * s];
     }
 #pragma unroll
-    for (int s = 0; s < 3; s++) q[32 * s + lane] = type >= 0 ? cm[s] * rnet[s] : 0.0;
+    for (int s = 0; s < NS; s++) q[32 * s + lane] = type >= 0 ? cm[s] * rnet[s] : 0.0;
     __syncwarp();
     // species production rates (three stages per pass over the incidence list), temperature equation
     const int2 *inc = reinterpret_cast<const int2 *>(tab + hdr[3]);      // (reaction, net stoichiometric coefficient)
-    double w[3] = {0.0, 0.0, 0.0};
+    double w[NS];
+#pragma unroll
+    for (int s = 0; s < NS; s++) w[s] = 0.0;
 #pragma unroll 1
     for (int p = d1.z; p < d1.w; p++) {
         const int2 e = inc[p];
         const double nu = (double)e.y;
-        w[0] += nu * q[e.x]; w[1] += nu * q[32 + e.x]; w[2] += nu * q[64 + e.x];
+        #pragma unroll
+        for (int s = 0; s < NS; s++) w[s] += nu * q[32 * s + e.x];
     }
-    double hw[3], ccp[3];
+    double hw[NS], ccp[NS];
 #pragma unroll
-    for (int s = 0; s < 3; s++) {
+    for (int s = 0; s < NS; s++) {
         const double *spc = tab + (T[s] <= tmid ? kOffSpLo : kOffSpHi) + row * kJobW;
         const double Ts = T[s];
         const double cpR = spc[0] + Ts * (spc[1] + Ts * (spc[2] + Ts * (spc[3] + Ts * spc[4])));
@@ -334,15 +342,19 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
 #pragma unroll 1
     for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
-        for (int s = 0; s < 3; s++) {
+        for (int s = 0; s < NS; s++) {
             hw[s] += __shfl_xor_sync(0xffffffffu, hw[s], o);
             ccp[s] += __shfl_xor_sync(0xffffffffu, ccp[s], o);
         }
     const double Wk = tab[kOffSpLo + row * kJobW + 6];
-    const double rc = rcp_f(sl3 == 0 ? ccp[0] : (sl3 == 1 ? ccp[1] : ccp[2]));
-    double f[3];
+    double csel = ccp[0];
 #pragma unroll
-    for (int s = 0; s < 3; s++) {
+    for (int s = 1; s < NS; s++)
+        if (sl3 == s) csel = ccp[s];
+    const double rc = rcp_f(csel);
+    double f[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int s = 0; s < NS; s++) {
         const double Ydot = Wk * w[s] * inv_rho[s];               // W_k wdot_k / rho in species lane k
         f[s] = __shfl_up_sync(0xffffffffu, Ydot, 1);               // component k+1
         const double rccp = __shfl_sync(0xffffffffu, rc, s);
@@ -352,6 +364,17 @@ __device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid,
     D3 out;
     out.a = f[0]; out.b = f[1]; out.c = f[2];
     return out;
+}
+
+// out-of-line instances: the Newton iterations evaluate three stage points at once, everything else one state
+// (a one-state call runs and fetches about a third of the instructions; the kernel is bound by instruction fetch)
+__device__ __noinline__ D3 warp_rhs3(const double *tab, double *ws, double tmid, double P, double invP, D3 y)
+{
+    return warp_rhs_body<3>(tab, ws, tmid, P, invP, y);
+}
+__device__ __noinline__ double warp_rhs1(const double *tab, double *ws, double tmid, double P, double invP, double y)
+{
+    return warp_rhs_body<1>(tab, ws, tmid, P, invP, D3{y, y, y}).a;
 }
 
 // Analytical Jacobian (R6) for the warp path: Jm[i*N + j] = d f_i / d y_j in shared memory.
