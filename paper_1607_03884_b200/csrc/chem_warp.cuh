@@ -578,9 +578,9 @@ __device__ __noinline__ int lu_warp_pair(double *Ar, double *Ai, int LD, int N, 
             double *xp = rr + k + 1, *xq = ri + k + 1;
 #pragma unroll 1
             for (int n = N - 1 - k; n > 0; n--, up++, uq++, xp++, xq++) {
-                const double ur = *up, ui = *uq;
-                *xp = fma(-lr, ur, fma(li, ui, *xp));
-                *xq = fma(-lr, ui, fma(-li, ur, *xq));
+                const double ur = *up, ui = *uq, xr = *xp, xi = *xq;     // all loads first: one shared-memory round trip
+                *xp = fma(-lr, ur, fma(li, ui, xr));
+                *xq = fma(-lr, ui, fma(-li, ur, xi));
             }
         }
         __syncwarp();
