@@ -126,7 +126,9 @@ int chem_rhs(const chem_mech *mech, int32_t n_states, double P, const double *y,
 /* Analytical Jacobian J[s][i][j] = d f_i / d y_j, device [n_states][N][N] row-major. */
 int chem_jacobian(const chem_mech *mech, int32_t n_states, double P, const double *y, double *J, void *stream);
 
-/* Batched dense LU solve hook (the device LU/solve routines the integrator uses):
+/* Batched dense solve hook (the device routines the integrator uses: for n <= 16 those of the warp-per-state kernel,
+ * a pivoted Gauss-Jordan inverse applied as a matrix-vector product; above that the LU + triangular solves of the
+ * group kernels):
  * solves A_s x_s = b_s for s < batch.  A: device [batch][n][n] row-major (complex: interleaved re,im),
  * b: device [batch][n] (complex: interleaved), x: same shape as b.  info: device [batch], 0 or k+1 of a zero pivot. */
 int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const double *A, const double *b, double *x,

@@ -167,6 +167,40 @@ __global__ void __launch_bounds__(32) lu_solve_kernel(int n, int batch, int is_c
     }
 }
 
+// The same hook for n <= 16 through the warp path's own routines (gj_warp_pair / solve_warp_pair, chem_warp.cuh):
+// one warp per system, both half-warps are given the system (a real one with zero imaginary parts).
+__global__ void __launch_bounds__(32) lu_solve_warp_kernel(int n, int batch, int is_complex, const double *__restrict__ A,
+                                                           const double *__restrict__ b, double *__restrict__ x, int *info)
+{
+    extern __shared__ double smem[];
+    const int LD = n | 1;
+    double2 *Z = reinterpret_cast<double2 *>(smem), *bp = Z + 2 * n * LD;
+    const int lane = threadIdx.x, h = lane >> 4, r = lane & 15;
+    for (int s = blockIdx.x; s < batch; s += gridDim.x) {
+        for (int e = lane; e < n * n; e += 32) {
+            const size_t g = (size_t)s * n * n + e;
+            const double2 v = is_complex ? make_double2(A[2 * g], A[2 * g + 1]) : make_double2(A[g], 0.0);
+            Z[(e / n) * LD + e % n] = v;
+            Z[n * LD + (e / n) * LD + e % n] = v;
+        }
+        __syncwarp();
+        int myk = -1, src = lane;
+        double rdr = 0.0, rdi = 0.0;
+        const int ier = gj_warp_pair(Z, LD, n, myk, src, rdr, rdi);
+        __syncwarp();
+        if (lane == 0) info[s] = ier;
+        if (!ier) {
+            const size_t g = (size_t)s * n + (r < n ? r : 0);
+            const double br = is_complex ? b[2 * g] : b[g], bi = is_complex ? b[2 * g + 1] : 0.0;
+            const double2 v = solve_warp_pair(Z, LD, n, bp, myk, src, rdr, rdi, br, bi);
+            if (h == 0 && r < n) {
+                if (is_complex) { x[2 * g] = v.x; x[2 * g + 1] = v.y; } else x[g] = v.x;
+            }
+        }
+        __syncwarp();
+    }
+}
+
 }  // namespace
 
 #include "chem_launch.inl"

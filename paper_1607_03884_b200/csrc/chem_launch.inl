@@ -136,6 +136,14 @@ extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const
 {
     if (n < 1 || batch < 0 || (batch > 0 && (!A || !b || !x))) return fail(CHEM_E_ARG, "bad argument");
     if (batch == 0) return CHEM_OK;
+    if (n <= 16) {   // the warp path's routines (Gauss-Jordan inverse + matrix-vector solve)
+        const size_t sm = ((size_t)2 * n * (n | 1) + 34) * sizeof(double2);
+        const int g = batch < 65535 ? batch : 65535;
+        lu_solve_warp_kernel<<<g, 32, sm, static_cast<cudaStream_t>(stream)>>>(n, batch, is_complex, A, b, x, info);
+        g_launches++;
+        CUDA_TRY(cudaGetLastError());
+        return CHEM_OK;
+    }
     const size_t smem = ((size_t)2 * n * n + 2 * n) * sizeof(double) + (size_t)n * sizeof(int) + 16;
     int dev = 0, optin = 0;
     CUDA_TRY(cudaGetDevice(&dev));

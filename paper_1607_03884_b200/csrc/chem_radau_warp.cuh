@@ -6,18 +6,19 @@
 
 namespace chem {
 
-// Per-warp scratch (doubles) after the fixed part [C E q X]: Jm[N*N] Ar[2][N*LD] Ai[2][N*LD] (>= 8*32 Jacobian scratch) perm[32 ints] vec[48]
+// Per-warp scratch (doubles) after the fixed part [C E q X]: Jm[N*N, padded even] Z[2][N*LD] complex (>= 8*32 doubles of
+// Jacobian scratch) bp[34] complex vec[48]
 __host__ __device__ inline int warp_ws_doubles(int N, int NR)
 {
     const int LD = N | 1;
     const int e = 4 * N * LD > 8 * 32 ? 4 * N * LD : 8 * 32;
     (void)NR;
-    return kWsMat + N * N + e + 16 + 48;
+    return kWsMat + ((N * N + 1) & ~1) + e + 68 + 48;
 }
 
 struct WarpMats {
-    double *Jm, *Ar, *Ai, *vec;
-    int *perm;
+    double *Jm, *vec;
+    double2 *Z, *bp;
     int N, LD;
 };
 
@@ -26,30 +27,29 @@ __device__ __forceinline__ WarpMats warp_mats(double *ws, int N)
     WarpMats m;
     m.N = N; m.LD = N | 1;
     double *p = ws + kWsMat;
-    m.Jm = p; p += N * N;
-    m.Ar = p; m.Ai = p + 2 * N * m.LD;          // the Jacobian routine borrows Ar.. as its 8*32 scratch
+    m.Jm = p; p += (N * N + 1) & ~1;
+    m.Z = reinterpret_cast<double2 *>(p);          // the Jacobian routine borrows Z as its 8*32 scratch
     p += (4 * N * m.LD > 8 * 32 ? 4 * N * m.LD : 8 * 32);
-    m.perm = reinterpret_cast<int *>(p); p += 16;
+    m.bp = reinterpret_cast<double2 *>(p); p += 68;
     m.vec = p;
     return m;
 }
 
-// half-warp 0: E1 = gamma/h I - J (imaginary plane zero), half-warp 1: E2 = (alpha + i beta)/h I - J; lane 16 h + r
+// half-warp 0: E1 = gamma/h I - J (imaginary parts zero), half-warp 1: E2 = (alpha + i beta)/h I - J; lane 16 h + r
 // writes row r.  Returns whether this lane saw a non-finite Jacobian entry.
-__device__ __noinline__ bool warp_form_matrices(const double *Jm, double *Ar, double *Ai, int N, int LD, double FAC1,
-                                                double ALPHN, double BETAN)
+__device__ __noinline__ bool warp_form_matrices(const double *Jm, double2 *Z, int N, int LD, double FAC1, double ALPHN,
+                                                double BETAN)
 {
     const int lane = threadIdx.x & 31, h = lane >> 4, r16 = lane & 15;
     bool nonfinite = false;
     if (r16 < N) {
-        double *ar = Ar + h * N * LD + r16 * LD, *ai = Ai + h * N * LD + r16 * LD;
+        double2 *z = Z + h * N * LD + r16 * LD;
         const double dre = h ? ALPHN : FAC1, dim = h ? BETAN : 0.0;
 #pragma unroll 1
         for (int j = 0; j < N; j++) {
             const double v = -Jm[r16 * N + j];
             nonfinite |= !isfinite(v);
-            ar[j] = (j == r16) ? v + dre : v;
-            ai[j] = (j == r16) ? dim : 0.0;
+            z[j] = (j == r16) ? make_double2(v + dre, dim) : make_double2(v, 0.0);
         }
     }
     return nonfinite;
@@ -125,8 +125,8 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
     double f0 = warp_rhs1(tab, ws, tmid, P, invP, y);
     st.nfcn++;
     double z1 = 0, z2 = 0, z3 = 0, w1 = 0, w2 = 0, w3 = 0, c1 = 0, c2 = 0, c3 = 0;
-    // LU factors
-    int myk = -1;
+    // factorisation data held in registers
+    int myk = -1, src = lane;
     double rdr = 0, rdi = 0;
 
     enum { DO_JAC, DO_FACT, DO_STEP };
@@ -136,7 +136,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             if (prm.fd_jacobian) {
                 st.nfcn += warp_jacobian_fd(tab, ws, tmid, P, invP, y, f0, ATOL + RTOL * fabs(y), H, N, M.Jm);
             } else {
-                warp_jacobian(tab, ws, tmid, P, invP, y, M.Jm, M.Ar, M.vec);
+                warp_jacobian(tab, ws, tmid, P, invP, y, M.Jm, reinterpret_cast<double *>(M.Z), M.vec);
             }
             st.njac++;
             CALJAC = true;
@@ -145,10 +145,10 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         if (next == DO_FACT) {
             const double invH = rcp_f(H);
             const double FAC1 = U1 * invH, ALPHN = ALPH * invH, BETAN = BETA * invH;
-            const bool nonfinite = warp_form_matrices(M.Jm, M.Ar, M.Ai, N, LD, FAC1, ALPHN, BETAN);
+            const bool nonfinite = warp_form_matrices(M.Jm, M.Z, N, LD, FAC1, ALPHN, BETAN);
             int ier = __any_sync(0xffffffffu, nonfinite);
             __syncwarp();
-            if (!ier) ier = lu_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi);
+            if (!ier) ier = gj_warp_pair(M.Z, LD, N, myk, src, rdr, rdi);
             __syncwarp();
             st.ndec++;
             if (ier) {
@@ -192,7 +192,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             {
                 // lower half solves the real system for z1, upper half the complex system for (z2, z3)
                 const double t2 = __shfl_sync(0xffffffffu, z2, r16), t3 = __shfl_sync(0xffffffffu, z3, r16);
-                const double2 x = solve_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi, h ? t2 : z1, h ? t3 : 0.0);
+                const double2 x = solve_warp_pair(M.Z, LD, N, M.bp, myk, src, rdr, rdi, h ? t2 : z1, h ? t3 : 0.0);
                 z1 = x.x;
                 z2 = __shfl_sync(0xffffffffu, x.x, 16 + r16);
                 z3 = __shfl_sync(0xffffffffu, x.y, 16 + r16);
@@ -247,7 +247,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         double ERR;
         {
             const double f2 = (DD1 * z1 + DD2 * z2 + DD3 * z3) * invH;
-            double cont = solve_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi, h ? 0.0 : f2 + f0, 0.0).x;
+            double cont = solve_warp_pair(M.Z, LD, N, M.bp, myk, src, rdr, rdi, h ? 0.0 : f2 + f0, 0.0).x;
             double e = 0.0;
             if (mine) { const double q = cont * iscal; e = q * q; }
             ERR = fmax(sqrt_s(warp_sum(e) * invN), 1.0e-10);
@@ -255,7 +255,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
                 const double yc = y + cont;
                 const double fr = warp_rhs1(tab, ws, tmid, P, invP, yc);
                 st.nfcn++;
-                cont = solve_warp_pair(M.Ar, M.Ai, LD, N, M.perm, myk, rdr, rdi, h ? 0.0 : fr + f2, 0.0).x;
+                cont = solve_warp_pair(M.Z, LD, N, M.bp, myk, src, rdr, rdi, h ? 0.0 : fr + f2, 0.0).x;
                 e = 0.0;
                 if (mine) { const double q = cont * iscal; e = q * q; }
                 ERR = fmax(sqrt_s(warp_sum(e) * invN), 1.0e-10);

@@ -525,7 +525,7 @@ __device__ __noinline__ void warp_jacobian(const double *tab, double *ws, double
     __syncwarp();
 }
 
-// ---------------------------------------------------------------------------- LU with rows owned by lanes
+// ---------------------------------------------------------------------------- linear algebra with rows owned by lanes
 // Separate arg-max in each half-warp with FULL-mask collectives only (partial-mask reductions take a slow
 // WARPSYNC path): returns the row 0..15 of the maximum of key v (>= 0, or -1 for inactive lanes) within the
 // caller's half h, or -1 if that maximum is not > 0.  Highest word first, low word on ties, lowest row wins exact ties.
@@ -546,85 +546,83 @@ __device__ __forceinline__ int half_argmax(double v, int h)
     return cand ? __ffs(cand) - 1 : -1;
 }
 
-// LU of BOTH Radau matrices in one instruction stream: half-warp 0 factors the real matrix E1 (imaginary plane
-// zero), half-warp 1 the complex matrix E2, both with complex arithmetic ("LU factorization of the
-// Jacobian"; one real and one complex N x N system per step).  Planes: Ar[h][N*LD], Ai[h][N*LD]; row r of half h is
-// owned by lane 16 h + r and never moves.  perm[16 h + k] = pivot row of step k; myk = step at which this lane's
-// row was the pivot row; (rdr, rdi) = 1/U_kk held by that lane.  Partial pivoting on |re| + |im| (R10).
-__device__ __noinline__ int lu_warp_pair(double *Ar, double *Ai, int LD, int N, int *perm, int &myk_out, double &rdr_out,
-                                         double &rdi_out)
+// Gauss-Jordan inversion of BOTH Radau matrices in one instruction stream: half-warp 0 handles the real matrix E1
+// (imaginary parts zero), half-warp 1 the complex matrix E2, both with complex arithmetic ("LU
+// factorization of the Jacobian"; one real and one complex N x N system per step).  The elimination is the one of LU
+// with partial pivoting on |re| + |im| (R10: same pivot sequence), continued above the diagonal, so that each
+// of the ~9 solves per factorisation becomes a matrix-vector product without the 2N-long chain of dependent
+// broadcasts of a triangular solve (the one place where this path departs from the oracle's
+// arithmetic; the group kernels keep LU + triangular solves).  Z[h][N][LD] complex (re, im); row r of half h is owned by lane
+// 16 h + r and never moves.  With p_k the pivot row of step k, the row operations G satisfy G A = D Pi (row p_k of
+// the result is piv_k e_k^T), so A^-1 = Pi^T D^-1 G.  In place: column k of the storage ends as column p_k of G.
+// Outputs: myk = step at which this lane's row was the pivot row, (rdr, rdi) = 1/piv of that row, src = lane owning
+// the pivot row of step r (where component r of a solution is produced).  Returns 0, or k + 1 at a zero/non-finite pivot.
+__device__ __noinline__ int gj_warp_pair(double2 *Z, int LD, int N, int &myk_out, int &src_out, double &rdr_out, double &rdi_out)
 {
     const int lane = threadIdx.x & 31, h = lane >> 4, r = lane & 15;
-    double *Pr_ = Ar + h * N * LD, *Pi_ = Ai + h * N * LD;
-    double *rr = Pr_ + (r < N ? r : 0) * LD, *ri = Pi_ + (r < N ? r : 0) * LD;
-    int myk = -1;
+    double2 *Zh = Z + h * N * LD;
+    double2 *row = Zh + (r < N ? r : 0) * LD;
+    int myk = -1, src = lane;
     double rdr = 0.0, rdi = 0.0;
     for (int k = 0; k < N; k++) {
-        const bool act = (r < N) && (myk < 0);
-        const double akr = rr[k], aki = ri[k];
-        const int p = half_argmax(act ? fabs(akr) + fabs(aki) : -1.0, h);
-        const double *pr_ = Pr_ + (p < 0 ? 0 : p) * LD, *pi_ = Pi_ + (p < 0 ? 0 : p) * LD;
-        const double pr = pr_[k], pi = pi_[k];
-        const double den = rcp_f(pr * pr + pi * pi);
+        const double2 a = row[k];
+        const int p = half_argmax((r < N && myk < 0) ? fabs(a.x) + fabs(a.y) : -1.0, h);
+        const double2 *prow = Zh + (p < 0 ? 0 : p) * LD;
+        const double2 pv = prow[k];
+        const double den = rcp_f(pv.x * pv.x + pv.y * pv.y);
         if (__any_sync(0xffffffffu, p < 0 || !isfinite(den))) return k + 1;
-        const double qr = pr * den, qi = -pi * den;       // 1 / pivot
-        if (r == 0) perm[16 * h + k] = p;
+        const double qr = pv.x * den, qi = -pv.y * den;       // 1 / pivot
+        if (r == k) src = 16 * h + p;
         if (r == p) { myk = k; rdr = qr; rdi = qi; }
-        if (act && r != p) {
-            const double lr = akr * qr - aki * qi, li = akr * qi + aki * qr;
-            rr[k] = lr;
-            ri[k] = li;
-            const double *up = pr_ + k + 1, *uq = pi_ + k + 1;
-            double *xp = rr + k + 1, *xq = ri + k + 1;
+        if (r < N && r != p) {
+            const double lr = a.x * qr - a.y * qi, li = a.x * qi + a.y * qr;
+            const double2 *u = prow;
+            double2 *x = row;
 #pragma unroll 1
-            for (int n = N - 1 - k; n > 0; n--, up++, uq++, xp++, xq++) {
-                const double ur = *up, ui = *uq, xr = *xp, xi = *xq;     // all loads first: one shared-memory round trip
-                *xp = fma(-lr, ur, fma(li, ui, xr));
-                *xq = fma(-lr, ui, fma(-li, ur, xi));
+            for (int n = N; n > 0; n--, u++, x++) {
+                const double2 uu = *u;
+                double2 xx = *x;
+                xx.x = fma(-lr, uu.x, fma(li, uu.y, xx.x));
+                xx.y = fma(-lr, uu.y, fma(-li, uu.x, xx.y));
+                *x = xx;
             }
+            row[k] = make_double2(-lr, -li);                   // column p_k of G (the eliminated entry itself is zero)
         }
         __syncwarp();
+        if (r == p) row[k] = make_double2(1.0, 0.0);           // only its owner reads this row from now on
     }
     myk_out = myk;
+    src_out = src;
     rdr_out = rdr;
     rdi_out = rdi;
     return 0;
 }
 
-// Solve with both factorisations at once: lane 16 h + r passes row r of the right-hand side of system h
-// and receives component r of its solution.
-__device__ __noinline__ double2 solve_warp_pair(const double *Ar, const double *Ai, int LD, int N, const int *perm, int myk,
-                                                double rdr, double rdi, double br, double bi)
+// Solve with both inverses at once: lane 16 h + r passes row r of the right-hand side of system h and receives
+// component r of its solution.  bp: 34 complex scratch entries (b permuted to pivot order, one dump slot per half).
+__device__ __noinline__ double2 solve_warp_pair(const double2 *Z, int LD, int N, double2 *bp, int myk, int src, double rdr,
+                                                double rdi, double br, double bi)
 {
     const int lane = threadIdx.x & 31, h = lane >> 4, r = lane & 15;
-    const int off = h * N * LD + (r < N ? r : 0) * LD;
-    const double *rr = Ar + off, *ri = Ai + off;
-    const int *pm = perm + 16 * h;
-    const int base = 16 * h;
+    const double2 *x = Z + h * N * LD + (r < N ? r : 0) * LD;
+    double2 *bh = bp + 17 * h;
+    bh[myk >= 0 ? myk : 16] = make_double2(br, bi);
+    __syncwarp();
+    double ar = 0.0, ai = 0.0, cr = 0.0, ci = 0.0;
+    const double2 *b = bh;
 #pragma unroll 1
-    for (int k = 0; k < N - 1; k++) {
-        const int p = pm[k] + base;
-        const double xr = __shfl_sync(0xffffffffu, br, p), xi = __shfl_sync(0xffffffffu, bi, p);
-        if (myk > k) {
-            const double lr = rr[k], li = ri[k];
-            br = fma(-lr, xr, fma(li, xi, br));
-            bi = fma(-lr, xi, fma(-li, xr, bi));
-        }
+    for (int n = N; n > 0; n--, b++, x++) {
+        const double2 bb = *b, g = *x;
+        ar = fma(g.x, bb.x, ar);
+        cr = fma(-g.y, bb.y, cr);
+        ai = fma(g.x, bb.y, ai);
+        ci = fma(g.y, bb.x, ci);
     }
-    double sr = 0.0, si = 0.0;
-#pragma unroll 1
-    for (int k = N - 1; k >= 0; k--) {
-        const int p = pm[k] + base;
-        const double vr = br * rdr - bi * rdi, vi = br * rdi + bi * rdr;
-        const double xr = __shfl_sync(0xffffffffu, vr, p), xi = __shfl_sync(0xffffffffu, vi, p);
-        if (myk >= 0 && myk < k) {
-            const double ur = rr[k], ui = ri[k];
-            br = fma(-ur, xr, fma(ui, xi, br));
-            bi = fma(-ur, xi, fma(-ui, xr, bi));
-        }
-        if (r == k) { sr = xr; si = xi; }
-    }
-    return make_double2(sr, si);
+    ar += cr;
+    ai += ci;
+    const double vr = ar * rdr - ai * rdi, vi = ar * rdi + ai * rdr;      // component myk of the solution
+    __syncwarp();
+    return make_double2(__shfl_sync(0xffffffffu, vr, src), __shfl_sync(0xffffffffu, vi, src));
 }
 
 }  // namespace chem

@@ -64,7 +64,7 @@ def test_jacobian_matches_oracle(kind, n, torch_cuda, gpu_mechs, orc_mechs, requ
 
 
 @pytest.mark.parametrize("cplx", [False, True])
-@pytest.mark.parametrize("n", [1, 2, 13, 53])
+@pytest.mark.parametrize("n", [1, 2, 5, 13, 16, 17, 53])    # n <= 16: the warp path's routines, else the group kernels'
 def test_lu_solve_matches_oracle(n, cplx, torch_cuda):
     from oracle import oracle as orc
     from paper_1607_03884_b200 import binding
@@ -85,6 +85,35 @@ def test_lu_solve_matches_oracle(n, cplx, torch_cuda):
             LU, ip, ier = orc.lu_real(A[s])
             ref = orc.lu_solve_real(LU, ip, b[s])
         assert np.allclose(x[s], ref, rtol=1e-9, atol=1e-11 * np.abs(ref).max())
+
+
+@pytest.mark.parametrize("n", [13, 16, 53])
+def test_lu_solve_stiff_newton_matrices(n, torch_cuda):
+    """Matrices of the shape the integrator factors, gamma/h I - J and (alpha + i beta)/h I - J with a stiff J
+    (eigenvalues spread over 12 decades): the residual of the device solve must be at the level of a backward-stable
+    solve of a system with this condition number (the warp path applies an explicit inverse)."""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    rng = np.random.default_rng(7 + n)
+    batch = 24
+    for cplx in (False, True):
+        A = np.empty((batch, n, n), dtype=complex if cplx else float)
+        conds = []
+        for s in range(batch):
+            V = rng.standard_normal((n, n))
+            lam = -10.0 ** rng.uniform(-2, 10, n)
+            J = V @ np.diag(lam) @ np.linalg.inv(V)
+            fac = (3.6378 + (0.0 if not cplx else 3.0j)) / 10.0 ** rng.uniform(-8, -4)
+            A[s] = fac * np.eye(n) - J
+            conds.append(np.linalg.cond(A[s]))
+        b = rng.standard_normal((batch, n)) + (1j * rng.standard_normal((batch, n)) if cplx else 0)
+        x, info = binding.chem_lu_solve(torch.from_numpy(A).cuda(), torch.from_numpy(b).cuda())
+        x, info = x.cpu().numpy(), info.cpu().numpy()
+        assert np.all(info == 0)
+        for s in range(batch):
+            ref = np.linalg.solve(A[s], b[s])
+            err = np.abs(x[s] - ref).max() / np.abs(ref).max()
+            assert err <= 1e-13 * conds[s] + 1e-12, (n, cplx, s, err, conds[s])
 
 
 def compare_integration(y_gpu, st_gpu, y_ref, st_ref):
