@@ -62,9 +62,9 @@ __global__ void __launch_bounds__(block_of<G>(), G > kBlock ? 2 : 1) integrate_k
 }
 
 // Compact warp-per-state integrator (chem_warp.cuh / chem_radau_warp.cuh): 8 warps per CTA.
-constexpr int kWarpBlock = 256;
+constexpr int kWarpBlock = 640;
 
-__global__ void __launch_bounds__(kWarpBlock, 2) integrate_warp_kernel(Tables t, FastTables ft, int n_states, double P,
+__global__ void __launch_bounds__(kWarpBlock, 1) integrate_warp_kernel(Tables t, FastTables ft, int n_states, double P,
                                                                     const double *P_per_state, RadauParams prm,
                                                                     const double *__restrict__ y_in, double *__restrict__ y_out,
                                                                     chem_stats *stats, int *counter, const int *order)

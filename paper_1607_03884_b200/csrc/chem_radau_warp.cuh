@@ -6,14 +6,15 @@
 
 namespace chem {
 
-// Per-warp scratch (doubles) after the fixed part [C E q X]: Jm[N*N, padded even] Z[2][N*LD] complex (>= 8*32 doubles of
-// Jacobian scratch) bp[34] complex vec[48]
+// Per-warp scratch (doubles) after the fixed part [C E q X]: Jm[N*N, padded even], Z[2][N*LD] complex.  The Jacobian
+// routine borrows Z (8*32 doubles of scratch, then vec[48]); the solves borrow q as bp[34] complex (q is dead between
+// source-term calls).
 __host__ __device__ inline int warp_ws_doubles(int N, int NR)
 {
     const int LD = N | 1;
-    const int e = 4 * N * LD > 8 * 32 ? 4 * N * LD : 8 * 32;
+    const int e = 4 * N * LD > 8 * 32 + 48 ? 4 * N * LD : 8 * 32 + 48;
     (void)NR;
-    return kWsMat + ((N * N + 1) & ~1) + e + 68 + 48;
+    return kWsMat + ((N * N + 1) & ~1) + e;
 }
 
 struct WarpMats {
@@ -28,10 +29,9 @@ __device__ __forceinline__ WarpMats warp_mats(double *ws, int N)
     m.N = N; m.LD = N | 1;
     double *p = ws + kWsMat;
     m.Jm = p; p += (N * N + 1) & ~1;
-    m.Z = reinterpret_cast<double2 *>(p);          // the Jacobian routine borrows Z as its 8*32 scratch
-    p += (4 * N * m.LD > 8 * 32 ? 4 * N * m.LD : 8 * 32);
-    m.bp = reinterpret_cast<double2 *>(p); p += 68;
-    m.vec = p;
+    m.Z = reinterpret_cast<double2 *>(p);
+    m.vec = p + 8 * 32;
+    m.bp = reinterpret_cast<double2 *>(ws + kWsQ);
     return m;
 }
 
