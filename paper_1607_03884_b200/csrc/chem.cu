@@ -159,8 +159,49 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
         for (auto &pr : inc[k]) { inc_rx.push_back(pr.first); inc_nu.push_back(pr.second); }
         inc_ptr[k + 1] = (int)inc_rx.size();
     }
+    // ---- balanced schedule of the species-production gather of the stage-batched source term (chem_cta.cuh): species k
+    // gets c_k = 2^m adjacent threads of one warp, each summing an equal share of its incidence list; the shares are
+    // combined by a fixed butterfly (deterministic).  c_k = the power of two above len_k / target, with the smallest
+    // target for which all groups fit into the G threads of a state (G as in group_size(), chem_launch.inl).
+    const int G_gather = ns <= 32 ? 32 : 128;
+    std::vector<int> gat(4 * G_gather, 0), inc2;
+    int gat_steps = -1;                                   // -1: no schedule (more species than threads)
+    if (ns <= G_gather) {
+        auto groups = [&](int target, std::vector<int> *lg) {
+            int tot = 0;
+            for (int k = 0; k < ns; k++) {
+                const int len = inc_ptr[k + 1] - inc_ptr[k], need = (len + target - 1) / target;
+                int m2 = 0;
+                while ((1 << m2) < need && m2 < 5) m2++;
+                if (lg) (*lg)[k] = m2;
+                tot += 1 << m2;
+            }
+            return tot;
+        };
+        int target = 1;
+        while (groups(target, nullptr) > G_gather) target++;
+        std::vector<int> lg(ns, 0), ord(ns);
+        groups(target, &lg);
+        for (int k = 0; k < ns; k++) ord[k] = k;
+        std::stable_sort(ord.begin(), ord.end(), [&](int a, int b2) { return lg[a] > lg[b2]; });   // big groups first: aligned starts
+        for (int t2 = 0; t2 < G_gather; t2++) gat[4 * t2] = -1;
+        int t2 = 0;
+        gat_steps = 0;
+        for (int k : ord) {
+            const int c = 1 << lg[k], len = inc_ptr[k + 1] - inc_ptr[k];
+            for (int j = 0; j < c; j++, t2++) {
+                gat[4 * t2] = k;
+                gat[4 * t2 + 1] = inc_ptr[k] + (int)((long long)len * j / c);
+                gat[4 * t2 + 2] = inc_ptr[k] + (int)((long long)len * (j + 1) / c);
+                gat[4 * t2 + 3] = lg[k];
+            }
+            if (lg[k] > gat_steps) gat_steps = lg[k];
+        }
+    }
+    for (size_t e = 0; e < inc_rx.size(); e++) { inc2.push_back(inc_rx[e]); inc2.push_back((int)inc_nu[e]); }
     if (eff_sp.empty()) { eff_sp.push_back(0); eff_dv.push_back(0.0); }
     if (inc_rx.empty()) { inc_rx.push_back(0); inc_nu.push_back(0.0); }
+    if (inc2.empty()) { inc2.push_back(0); inc2.push_back(0); }
 
     // ---- exp-job tables for the stage-batched source term of the group kernels (chem_cta.cuh); same idea as
     // chem_fast.inl: k_f, k_r (ln K_c folded in from the NASA coefficients), k_0/k_inf and the three Troe terms are all
@@ -258,6 +299,7 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     add(rtype.data(), nr * 4); add(slot_sp.data(), 6 * nr * 4); add(slot_nu.data(), 6 * nr * 4);
     add(eff_ptr.data(), (nr + 1) * 4); add(eff_sp.data(), eff_sp.size() * 4);
     add(inc_ptr.data(), (ns + 1) * 4); add(inc_rx.data(), inc_rx.size() * 4); add(rdesc.data(), rdesc.size() * 4);
+    add(gat.data(), gat.size() * 4); add(inc2.data(), inc2.size() * 4);
     std::vector<char> host(total, 0);
     for (size_t a = 0; a < parts.size(); a++) std::memcpy(host.data() + offs[a], parts[a].first, parts[a].second);
 
@@ -285,6 +327,7 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     t.lnA = D(); t.b = D(); t.Ta = D(); t.lnA0 = D(); t.b0 = D(); t.Ta0 = D(); t.dnu = D(); t.troe = D();
     t.eff_dv = D(); t.inc_nu = D(); t.job_lo = D(); t.job_hi = D();
     t.rtype = I(); t.slot_sp = I(); t.slot_nu = I(); t.eff_ptr = I(); t.eff_sp = I(); t.inc_ptr = I(); t.inc_rx = I(); t.rdesc = I();
+    t.gat = reinterpret_cast<const int4 *>(I()); t.inc2 = reinterpret_cast<const int2 *>(I()); t.gat_steps = gat_steps;
     t.n_jobs = n_jobs; t.n_fo = n_fo; t.tmid0 = tmid[0];
     m->n_sm = n_sm;
     m->max_smem_optin = optin;

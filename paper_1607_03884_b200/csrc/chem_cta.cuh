@@ -156,15 +156,7 @@ __device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, co
     Grp<G>::sync();
     // ---- species production rates, temperature equation
     double r6[6] = {0, 0, 0, 0, 0, 0};
-    for (int k = lane; k < N; k += G) {
-        double w[3] = {0.0, 0.0, 0.0};
-        for (int p = __ldg(&t.inc_ptr[k]); p < __ldg(&t.inc_ptr[k + 1]); p++) {
-            const double nu = __ldg(&t.inc_nu[p]);
-            const int i = __ldg(&t.inc_rx[p]);
-#pragma unroll
-            for (int s = 0; s < 3; s++)
-                if (s < nstage) w[s] += nu * x.q3[s * NR + i];
-        }
+    auto species_tail = [&](int k, const double (&w)[3]) {
         const double Wk = __ldg(&t.W[k]);
 #pragma unroll
         for (int s = 0; s < 3; s++)
@@ -179,6 +171,41 @@ __device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, co
                 r6[2 * s + 1] += x.C3[64 * s + k] * cpR;
                 if (k < N - 1) fo[s][k + 1] = Wk * w[s] * x.X0[8 * s + 4];
             }
+    };
+    if (t.gat_steps >= 0) {
+        // balanced gather (schedule built by the mechanism compiler): the incidence list of a species is shared by
+        // 2^g.w adjacent threads; long lists (radicals that take part in a third of the reactions) no longer hold the
+        // whole group at the next barrier
+        const int4 g = __ldg(t.gat + lane);
+        double w[3] = {0.0, 0.0, 0.0};
+#pragma unroll 4
+        for (int p = g.y; p < g.z; p++) {
+            const int2 e = __ldg(t.inc2 + p);
+            const double nu = (double)e.y;
+#pragma unroll
+            for (int s = 0; s < 3; s++)
+                if (s < nstage) w[s] += nu * x.q3[s * NR + e.x];
+        }
+        for (int o = 1; o < (1 << t.gat_steps); o <<= 1) {
+#pragma unroll
+            for (int s = 0; s < 3; s++) {
+                const double v = __shfl_xor_sync(0xffffffffu, w[s], o);
+                if (o < (1 << g.w)) w[s] += v;
+            }
+        }
+        if (g.x >= 0 && (lane & ((1 << g.w) - 1)) == 0) species_tail(g.x, w);
+    } else {
+        for (int k = lane; k < N; k += G) {
+            double w[3] = {0.0, 0.0, 0.0};
+            for (int p = __ldg(&t.inc_ptr[k]); p < __ldg(&t.inc_ptr[k + 1]); p++) {
+                const double nu = __ldg(&t.inc_nu[p]);
+                const int i = __ldg(&t.inc_rx[p]);
+#pragma unroll
+                for (int s = 0; s < 3; s++)
+                    if (s < nstage) w[s] += nu * x.q3[s * NR + i];
+            }
+            species_tail(k, w);
+        }
     }
     sum6<G>(r6, x.red6);
     if (lane < nstage) {

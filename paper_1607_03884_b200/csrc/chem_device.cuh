@@ -39,6 +39,11 @@ struct Tables {
     const int *rdesc;                 // [n_rx][8]: factors 0-2 (8 bits each, 63 = unity), factors 3-5, type, extra job, falloff ordinal, eff_lo, eff_hi, 0
     int n_jobs, n_fo;
     double tmid0;
+    // balanced gather schedule of cta_rhs3 (chem.cu): per thread of a group (species or -1, first entry, end, log2 of the
+    // species' thread count); inc2 = (reaction, net coefficient) pairs in inc_ptr order; gat_steps = max log2, -1: none
+    const int4 *gat;
+    const int2 *inc2;
+    int gat_steps;
 };
 
 // ---------------------------------------------------------------------------------------------
