@@ -506,11 +506,19 @@ __device__ __noinline__ int lu2_real(int N, int LD, double *A, const Lu2Aux &x)
         l1 = (k1 < 0) ? a1 * rp : 0.0;
         const int j0 = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
         double *c = A + j0 * LD;
-#pragma unroll 2
-        for (int j = j0; j < N; j += NW, c += NW * LD) {
-            const double u = c[p];
-            c[r0] = fma(-l0, u, c[r0]);
-            c[r1] = fma(-l1, u, c[r1]);
+        // two of this warp's columns per trip, all loads before the stores (the update is bound by shared-memory round
+        // trips; the compiler cannot move a load above a store that might alias)
+#pragma unroll 1
+        for (int j = j0; j < N; j += 2 * NW, c += 2 * NW * LD) {
+            const bool two = j + NW < N;
+            double *c2 = c + (two ? NW * LD : 0);
+            const double u = c[p], x0 = c[r0], x1 = c[r1], u2 = c2[p], y0 = c2[r0], y1 = c2[r1];
+            c[r0] = fma(-l0, u, x0);
+            c[r1] = fma(-l1, u, x1);
+            if (two) {
+                c2[r0] = fma(-l0, u2, y0);
+                c2[r1] = fma(-l1, u2, y1);
+            }
         }
         Grp<G>::sync();
     }
@@ -546,14 +554,22 @@ __device__ __noinline__ int lu2_complex(int N, int LD, double *Ar, double *Ai, c
         l1r = (k1 < 0) ? a1r * qr - a1i * qi : 0.0; l1i = (k1 < 0) ? a1r * qi + a1i * qr : 0.0;
         const int j0 = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
         double *cr = Ar + j0 * LD, *ci = Ai + j0 * LD;
-#pragma unroll 2
-        for (int j = j0; j < N; j += NW, cr += NW * LD, ci += NW * LD) {
-            const double ur = cr[p], ui = ci[p];
-            const double x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
+#pragma unroll 1
+        for (int j = j0; j < N; j += 2 * NW, cr += 2 * NW * LD, ci += 2 * NW * LD) {
+            const bool two = j + NW < N;
+            double *dr = cr + (two ? NW * LD : 0), *di = ci + (two ? NW * LD : 0);
+            const double ur = cr[p], ui = ci[p], x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
+            const double vr = dr[p], vi = di[p], y0r = dr[r0], y0i = di[r0], y1r = dr[r1], y1i = di[r1];
             cr[r0] = fma(-l0r, ur, fma(l0i, ui, x0r));
             ci[r0] = fma(-l0r, ui, fma(-l0i, ur, x0i));
             cr[r1] = fma(-l1r, ur, fma(l1i, ui, x1r));
             ci[r1] = fma(-l1r, ui, fma(-l1i, ur, x1i));
+            if (two) {
+                dr[r0] = fma(-l0r, vr, fma(l0i, vi, y0r));
+                di[r0] = fma(-l0r, vi, fma(-l0i, vr, y0i));
+                dr[r1] = fma(-l1r, vr, fma(l1i, vi, y1r));
+                di[r1] = fma(-l1r, vi, fma(-l1i, vr, y1i));
+            }
         }
         Grp<G>::sync();
     }
