@@ -29,7 +29,7 @@ UNIT = "states/s"
 # ALU roofline: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram bytes per launch of integrate_kernel from the committed ncu --set full capture (profiles/), or None
-NCU_TRAFFIC_BYTES = {1: 117.351936e6 + 84.251136e6}   # profiles/r1_final_config1.md
+NCU_TRAFFIC_BYTES = {1: 115.299840e6 + 109.461760e6}   # profiles/r1_final_config1.md
 
 
 def load_peaks():
