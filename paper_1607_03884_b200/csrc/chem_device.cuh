@@ -576,6 +576,71 @@ __device__ __noinline__ int lu2_complex(int N, int LD, double *Ar, double *Ai, c
     return 0;
 }
 
+// Both factorisations of a Radau step in ONE pass: per elimination step the pivot search, reciprocal and multipliers of the
+// real and of the complex matrix are two independent dependency chains that overlap, and the step needs one barrier
+// instead of two.  Same arithmetic, pivots and storage as lu2_real / lu2_complex; returns k + 1 if either matrix has no
+// usable pivot at step k.
+template <int G>
+__device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xa, double *Ar, double *Ai, const Lu2Aux &xc)
+{
+    const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
+    constexpr int NW = Grp<G>::NW;
+    const int i0 = wl, i1 = wl + 32;
+    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;             // storage rows (N = dummy)
+    int ka0 = (i0 < N) ? -1 : 1 << 30, ka1 = (i1 < N) ? -1 : 1 << 30; // rowk of my two rows in the real matrix
+    int kc0 = ka0, kc1 = ka1;                                         // ... in the complex matrix
+    double l0 = 0.0, l1 = 0.0, l0r = 0.0, l0i = 0.0, l1r = 0.0, l1i = 0.0;
+    for (int k = 0; k < N; k++) {
+        if (k > 0 && wp == (k - 1) % NW) {                            // delayed write-back of the multipliers of column k-1
+            if (ka0 < 0) A[i0 + (k - 1) * LD] = l0;
+            if (ka1 < 0) A[i1 + (k - 1) * LD] = l1;
+            if (kc0 < 0) { Ar[i0 + (k - 1) * LD] = l0r; Ai[i0 + (k - 1) * LD] = l0i; }
+            if (kc1 < 0) { Ar[i1 + (k - 1) * LD] = l1r; Ai[i1 + (k - 1) * LD] = l1i; }
+        }
+        const double a0 = (ka0 < 0) ? A[i0 + k * LD] : 0.0, a1 = (ka1 < 0) ? A[i1 + k * LD] : 0.0;
+        const double a0r = (kc0 < 0) ? Ar[i0 + k * LD] : 0.0, a0i = (kc0 < 0) ? Ai[i0 + k * LD] : 0.0;
+        const double a1r = (kc1 < 0) ? Ar[i1 + k * LD] : 0.0, a1i = (kc1 < 0) ? Ai[i1 + k * LD] : 0.0;
+        const double va0 = (ka0 < 0) ? fabs(a0) : -1.0, va1 = (ka1 < 0) ? fabs(a1) : -1.0;
+        const double vc0 = (kc0 < 0) ? fabs(a0r) + fabs(a0i) : -1.0, vc1 = (kc1 < 0) ? fabs(a1r) + fabs(a1i) : -1.0;
+        const int pa = warp_argmax_row(va1 > va0 ? va1 : va0, va1 > va0 ? i1 : i0);
+        const int pc = warp_argmax_row(vc1 > vc0 ? vc1 : vc0, vc1 > vc0 ? i1 : i0);
+        const double pv = (pa >= 0) ? A[pa + k * LD] : 0.0;
+        const double pr = (pc >= 0) ? Ar[pc + k * LD] : 0.0, pi = (pc >= 0) ? Ai[pc + k * LD] : 0.0;
+        const double den = rcp_nr(pr * pr + pi * pi);
+        if (pa < 0 || !isfinite(pv) || pc < 0 || !isfinite(den)) return k + 1;
+        const double rp = rcp_nr(pv);
+        const double qr = pr * den, qi = -pi * den;                   // 1 / complex pivot
+        if (i0 == pa) ka0 = k;
+        if (i1 == pa) ka1 = k;
+        if (i0 == pc) kc0 = k;
+        if (i1 == pc) kc1 = k;
+        if (lane == 0) {
+            xa.perm[k] = pa; xa.rdr[k] = rp; xa.rowk[pa] = k;
+            xc.perm[k] = pc; xc.rdr[k] = qr; xc.rdi[k] = qi; xc.rowk[pc] = k;
+        }
+        l0 = (ka0 < 0) ? a0 * rp : 0.0;
+        l1 = (ka1 < 0) ? a1 * rp : 0.0;
+        l0r = (kc0 < 0) ? a0r * qr - a0i * qi : 0.0; l0i = (kc0 < 0) ? a0r * qi + a0i * qr : 0.0;
+        l1r = (kc1 < 0) ? a1r * qr - a1i * qi : 0.0; l1i = (kc1 < 0) ? a1r * qi + a1i * qr : 0.0;
+        const int j0 = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
+        double *c = A + j0 * LD, *cr = Ar + j0 * LD, *ci = Ai + j0 * LD;
+#pragma unroll 1
+        for (int j = j0; j < N; j += NW, c += NW * LD, cr += NW * LD, ci += NW * LD) {
+            // one column of each matrix per trip, all loads before the stores
+            const double u = c[pa], x0 = c[r0], x1 = c[r1];
+            const double ur = cr[pc], ui = ci[pc], x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
+            c[r0] = fma(-l0, u, x0);
+            c[r1] = fma(-l1, u, x1);
+            cr[r0] = fma(-l0r, ur, fma(l0i, ui, x0r));
+            ci[r0] = fma(-l0r, ui, fma(-l0i, ur, x0i));
+            cr[r1] = fma(-l1r, ur, fma(l1i, ui, x1r));
+            ci[r1] = fma(-l1r, ui, fma(-l1i, ur, x1i));
+        }
+        Grp<G>::sync();
+    }
+    return 0;
+}
+
 // Solves with the lu2 factors by ONE warp: b (shared, length N, original row order) is overwritten by x.
 __device__ __forceinline__ void solve2_real_warp(int N, int LD, const double *A, const Lu2Aux &x, double *b, int wl)
 {
