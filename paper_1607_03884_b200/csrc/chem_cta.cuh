@@ -67,11 +67,15 @@ __device__ __forceinline__ double job_val(const double *c, double T, double lnT,
 
 // Inputs: stage states ys[0..2] (shared, length N); outputs f[0..2] (shared, length N).  nstage = 1 or 3.
 template <int G>
-__device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, const CtaScratch &x, double P, int nstage,
+__device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, const CtaScratch &xg, double P, int nstage,
                                       const double *ys0, double *f0, double *f1, double *f2)
 {
     const int N = t.n_sp, NR = t.n_rx, nfo = t.n_fo;
     const int lane = Grp<G>::lane();
+    CtaScratch x;        // all of these live in dynamic shared memory: say so to the compiler (shp)
+    x.ys2 = shp(xg.ys2); x.ys3 = shp(xg.ys3); x.C3 = shp(xg.C3); x.X0 = shp(xg.X0); x.X = shp(xg.X); x.q3 = shp(xg.q3);
+    x.red6 = shp(xg.red6);
+    ys0 = shp(ys0); f0 = shp(f0); f1 = shp(f1); f2 = shp(f2);
     const double *ys[3] = {ys0, x.ys2, x.ys3};
     double *fo[3] = {f0, f1, f2};
     // ---- mixture: closure, Wbar, rho, concentrations
@@ -126,7 +130,8 @@ __device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, co
             double c = 1.0;
             if (type != 0) {
                 double M = x.X0[8 * s + 5];
-                for (int p = d1.y; p < d1.z; p++) M += __ldg(&t.eff_dv[p]) * C[__ldg(&t.eff_sp[p])];
+#pragma unroll 4
+                for (int p = d1.y; p < d1.z; p++) M += __ldg(&t.eff_dv[p]) * C[__ldg(&t.eff_sp[p])];   // unrolled: loads batched
                 c = M;
                 if (type >= 2) {
                     const double Pr = job_val(jt + (size_t)d0.w * 8, T, lnT, invT) * M;

@@ -82,6 +82,17 @@ struct Grp {
     }
 };
 
+// Rebase a generic pointer that is known to point into this CTA's dynamic shared memory on the shared window, so that
+// the compiler emits LDS / STS instead of generic LD / ST inside out-of-line routines (where it cannot see the origin
+// of pointer arguments and struct members).
+template <typename T>
+__device__ __forceinline__ T *shp(T *p)
+{
+    extern __shared__ double chem_smem_window_[];
+    const size_t off = __cvta_generic_to_shared(p) - __cvta_generic_to_shared(chem_smem_window_);
+    return reinterpret_cast<T *>(reinterpret_cast<char *>(chem_smem_window_) + off);
+}
+
 __device__ __forceinline__ double rcp_nr(double x)   // 1/x for normal x: MUFU seed + two Newton steps
 {
     double r;
@@ -109,6 +120,14 @@ struct ChemScratch {
     double *dqdT, *tb;                        // [n_rx]      (Jacobian only)
     double *red;                              // [2*NW]
 };
+
+__device__ __forceinline__ ChemScratch shp(const ChemScratch &g)
+{
+    ChemScratch s;
+    s.C = shp(g.C); s.g = shp(g.g); s.hRT = shp(g.hRT); s.cpR = shp(g.cpR); s.dcpR = shp(g.dcpR); s.wdot = shp(g.wdot);
+    s.q = shp(g.q); s.dq = shp(g.dq); s.dqdT = shp(g.dqdT); s.tb = shp(g.tb); s.red = shp(g.red);
+    return s;
+}
 
 // Mixture state derived from ys = (T, Y_1..Y_{N-1}): fills C, g = h/RT - s/R, hRT, cpR (and dcpR).
 // DESIGN.md R1 (state, closure, ideal gas) and R2 (NASA-7).
@@ -248,8 +267,10 @@ __device__ __forceinline__ double reaction(const Tables &t, int i, double T, dou
 
 // Source term f(T, Y; P) of one state (R1): f[0] = dT/dt, f[k+1] = dY_k/dt.  ys, f: shared, length N.
 template <int G>
-__device__ __noinline__ void rhs(const Tables &t, const ChemScratch &s, double P, const double *ys, double *f)
+__device__ __noinline__ void rhs(const Tables &t, const ChemScratch &sg, double P, const double *ys, double *f)
 {
+    const ChemScratch s = shp(sg);     // shared-memory scratch: LDS / STS instead of generic accesses
+    ys = shp(ys); f = shp(f);
     const int N = t.n_sp, NR = t.n_rx;
     const int lane = Grp<G>::lane();
     double T, rho, Wbar;
@@ -277,8 +298,10 @@ __device__ __noinline__ void rhs(const Tables &t, const ChemScratch &s, double P
 // Uses that at constant (T, P) the total concentration is independent of Y, so the unit part of the
 // third-body efficiencies only enters d/dT.
 template <int G>
-__device__ __noinline__ void jacobian(const Tables &t, const ChemScratch &s, double P, const double *ys, double *Jm)
+__device__ __noinline__ void jacobian(const Tables &t, const ChemScratch &sg, double P, const double *ys, double *Jm)
 {
+    const ChemScratch s = shp(sg);     // shared-memory scratch: LDS / STS instead of generic accesses
+    ys = shp(ys); Jm = shp(Jm);
     const int N = t.n_sp, NR = t.n_rx;
     const int lane = Grp<G>::lane();
     double T, rho, Wbar;
@@ -457,6 +480,12 @@ struct Lu2Aux {
     int *perm, *rowk;   // [N] each
     double *rdr, *rdi;  // [N]; rdi unused for the real matrix
 };
+__device__ __forceinline__ Lu2Aux shp(const Lu2Aux &g)
+{
+    Lu2Aux x;
+    x.perm = shp(g.perm); x.rowk = shp(g.rowk); x.rdr = shp(g.rdr); x.rdi = g.rdi ? shp(g.rdi) : nullptr;
+    return x;
+}
 
 // exact arg-max over a warp of (key >= 0 or -1 for inactive, row index); lowest lane wins exact ties
 __device__ __forceinline__ int warp_argmax_row(double v, int row)
@@ -581,8 +610,10 @@ __device__ __noinline__ int lu2_complex(int N, int LD, double *Ar, double *Ai, c
 // instead of two.  Same arithmetic, pivots and storage as lu2_real / lu2_complex; returns k + 1 if either matrix has no
 // usable pivot at step k.
 template <int G>
-__device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xa, double *Ar, double *Ai, const Lu2Aux &xc)
+__device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag, double *Ar, double *Ai, const Lu2Aux &xcg)
 {
+    const Lu2Aux xa = shp(xag), xc = shp(xcg);
+    A = shp(A); Ar = shp(Ar); Ai = shp(Ai);
     const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
     constexpr int NW = Grp<G>::NW;
     const int i0 = wl, i1 = wl + 32;
@@ -711,9 +742,11 @@ __device__ __forceinline__ void solve2_complex_warp(int N, int LD, const double 
     __syncwarp();
 }
 template <int G>
-__device__ __noinline__ void solve2_pair(int N, int LD, const double *E1, const Lu2Aux &x1, double *z1, const double *E2r,
-                                         const double *E2i, const Lu2Aux &x2, double *z2, double *z3)
+__device__ __noinline__ void solve2_pair(int N, int LD, const double *E1, const Lu2Aux &x1g, double *z1, const double *E2r,
+                                         const double *E2i, const Lu2Aux &x2g, double *z2, double *z3)
 {
+    const Lu2Aux x1 = shp(x1g), x2 = shp(x2g);     // everything below is dynamic shared memory
+    E1 = shp(E1); E2r = shp(E2r); E2i = shp(E2i); z1 = shp(z1); z2 = shp(z2); z3 = shp(z3);
     if (G == 32) {
         solve2_real_warp(N, LD, E1, x1, z1, Grp<G>::wlane());
         solve2_complex_warp(N, LD, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
@@ -724,8 +757,10 @@ __device__ __noinline__ void solve2_pair(int N, int LD, const double *E1, const 
     Grp<G>::sync();
 }
 template <int G>
-__device__ __noinline__ void solve2_real(int N, int LD, const double *E1, const Lu2Aux &x1, double *b)
+__device__ __noinline__ void solve2_real(int N, int LD, const double *E1, const Lu2Aux &x1g, double *b)
 {
+    const Lu2Aux x1 = shp(x1g);
+    E1 = shp(E1); b = shp(b);
     if (Grp<G>::warp() == 0) solve2_real_warp(N, LD, E1, x1, b, Grp<G>::wlane());
     Grp<G>::sync();
 }
