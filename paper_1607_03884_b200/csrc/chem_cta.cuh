@@ -67,9 +67,10 @@ __device__ __forceinline__ double job_val(const double *c, double T, double lnT,
 
 // Inputs: stage states ys[0..2] (shared, length N); outputs f[0..2] (shared, length N).  nstage = 1 or 3.
 template <int G>
-__device__ __noinline__ void cta_rhs3(const Tables &t, const ChemScratch &cs, const CtaScratch &xg, double P, int nstage,
+__device__ __noinline__ void cta_rhs3(const Tables &tg, const ChemScratch &cs, const CtaScratch &xg, double P, int nstage,
                                       const double *ys0, double *f0, double *f1, double *f2)
 {
+    const Tables &t = *shp(&tg);     // the kernel's shared copy of the descriptor
     const int N = t.n_sp, NR = t.n_rx, nfo = t.n_fo;
     const int lane = Grp<G>::lane();
     CtaScratch x;        // all of these live in dynamic shared memory: say so to the compiler (shp)

@@ -267,10 +267,11 @@ __device__ __forceinline__ double reaction(const Tables &t, int i, double T, dou
 
 // Source term f(T, Y; P) of one state (R1): f[0] = dT/dt, f[k+1] = dY_k/dt.  ys, f: shared, length N.
 template <int G>
-__device__ __noinline__ void rhs(const Tables &t, const ChemScratch &sg, double P, const double *ys, double *f)
+__device__ __noinline__ void rhs(const Tables &tg, const ChemScratch &sg, double P, const double *ys, double *f)
 {
     const ChemScratch s = shp(sg);     // shared-memory scratch: LDS / STS instead of generic accesses
     ys = shp(ys); f = shp(f);
+    const Tables &t = *shp(&tg);
     const int N = t.n_sp, NR = t.n_rx;
     const int lane = Grp<G>::lane();
     double T, rho, Wbar;
@@ -298,10 +299,11 @@ __device__ __noinline__ void rhs(const Tables &t, const ChemScratch &sg, double 
 // Uses that at constant (T, P) the total concentration is independent of Y, so the unit part of the
 // third-body efficiencies only enters d/dT.
 template <int G>
-__device__ __noinline__ void jacobian(const Tables &t, const ChemScratch &sg, double P, const double *ys, double *Jm)
+__device__ __noinline__ void jacobian(const Tables &tg, const ChemScratch &sg, double P, const double *ys, double *Jm)
 {
     const ChemScratch s = shp(sg);     // shared-memory scratch: LDS / STS instead of generic accesses
     ys = shp(ys); Jm = shp(Jm);
+    const Tables &t = *shp(&tg);
     const int N = t.n_sp, NR = t.n_rx;
     const int lane = Grp<G>::lane();
     double T, rho, Wbar;
