@@ -675,26 +675,38 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
 }
 
 // Solves with the lu2 factors by ONE warp: b (shared, length N, original row order) is overwritten by x.
+// Each step is one link of a dependency chain (broadcast of the finished component -> update of the remaining rows).
+// Everything that is not on the chain is issued ahead of it: the pivot row of the NEXT step is fetched one step early and
+// the matrix entries are loaded unconditionally (storage row N is the dummy row of the lu2 layout) before the broadcast.
 __device__ __forceinline__ void solve2_real_warp(int N, int LD, const double *A, const Lu2Aux &x, double *b, int wl)
 {
     const int i0 = wl, i1 = wl + 32;
+    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;
     const int k0 = (i0 < N) ? x.rowk[i0] : -1, k1 = (i1 < N) ? x.rowk[i1] : -1;   // -1: no such row (never updated)
     double b0 = (i0 < N) ? b[i0] : 0.0, b1 = (i1 < N) ? b[i1] : 0.0;
+    int p = x.perm[0];
 #pragma unroll 1
     for (int k = 0; k < N - 1; k++) {
-        const int p = x.perm[k];
+        const int pn = x.perm[k + 1];
+        const double l0 = A[r0 + k * LD], l1 = A[r1 + k * LD];
         const double bk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31);
-        if (k0 > k) b0 = fma(-A[i0 + k * LD], bk, b0);
-        if (k1 > k) b1 = fma(-A[i1 + k * LD], bk, b1);
+        if (k0 > k) b0 = fma(-l0, bk, b0);
+        if (k1 > k) b1 = fma(-l1, bk, b1);
+        p = pn;
     }
     __syncwarp();
+    double rd = x.rdr[N - 1];
 #pragma unroll 1
     for (int k = N - 1; k >= 0; k--) {
-        const int p = x.perm[k];
-        const double xk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31) * x.rdr[k];
-        if (k0 >= 0 && k0 < k) b0 = fma(-A[i0 + k * LD], xk, b0);
-        if (k1 >= 0 && k1 < k) b1 = fma(-A[i1 + k * LD], xk, b1);
+        const int pn = x.perm[k > 0 ? k - 1 : 0];
+        const double rdn = x.rdr[k > 0 ? k - 1 : 0];
+        const double u0 = A[r0 + k * LD], u1 = A[r1 + k * LD];
+        const double xk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31) * rd;
+        if (k0 >= 0 && k0 < k) b0 = fma(-u0, xk, b0);
+        if (k1 >= 0 && k1 < k) b1 = fma(-u1, xk, b1);
         if (wl == 0) b[k] = xk;
+        p = pn;
+        rd = rdn;
     }
     __syncwarp();
 }
@@ -702,44 +714,48 @@ __device__ __forceinline__ void solve2_complex_warp(int N, int LD, const double 
                                                     double *bi, int wl)
 {
     const int i0 = wl, i1 = wl + 32;
+    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;
     const int k0 = (i0 < N) ? x.rowk[i0] : -1, k1 = (i1 < N) ? x.rowk[i1] : -1;
     double b0r = (i0 < N) ? br[i0] : 0.0, b0i = (i0 < N) ? bi[i0] : 0.0;
     double b1r = (i1 < N) ? br[i1] : 0.0, b1i = (i1 < N) ? bi[i1] : 0.0;
+    int p = x.perm[0];
 #pragma unroll 1
     for (int k = 0; k < N - 1; k++) {
-        const int p = x.perm[k];
+        const int pn = x.perm[k + 1];
+        const double l0r = Ar[r0 + k * LD], l0i = Ai[r0 + k * LD], l1r = Ar[r1 + k * LD], l1i = Ai[r1 + k * LD];
         const double xr = __shfl_sync(0xffffffffu, (p & 32) ? b1r : b0r, p & 31);
         const double xi = __shfl_sync(0xffffffffu, (p & 32) ? b1i : b0i, p & 31);
         if (k0 > k) {
-            const double lr = Ar[i0 + k * LD], li = Ai[i0 + k * LD];
-            b0r = fma(-lr, xr, fma(li, xi, b0r));
-            b0i = fma(-lr, xi, fma(-li, xr, b0i));
+            b0r = fma(-l0r, xr, fma(l0i, xi, b0r));
+            b0i = fma(-l0r, xi, fma(-l0i, xr, b0i));
         }
         if (k1 > k) {
-            const double lr = Ar[i1 + k * LD], li = Ai[i1 + k * LD];
-            b1r = fma(-lr, xr, fma(li, xi, b1r));
-            b1i = fma(-lr, xi, fma(-li, xr, b1i));
+            b1r = fma(-l1r, xr, fma(l1i, xi, b1r));
+            b1i = fma(-l1r, xi, fma(-l1i, xr, b1i));
         }
+        p = pn;
     }
     __syncwarp();
+    double qr = x.rdr[N - 1], qi = x.rdi[N - 1];
 #pragma unroll 1
     for (int k = N - 1; k >= 0; k--) {
-        const int p = x.perm[k];
+        const int kn = k > 0 ? k - 1 : 0;
+        const int pn = x.perm[kn];
+        const double qrn = x.rdr[kn], qin = x.rdi[kn];
+        const double u0r = Ar[r0 + k * LD], u0i = Ai[r0 + k * LD], u1r = Ar[r1 + k * LD], u1i = Ai[r1 + k * LD];
         const double vr = __shfl_sync(0xffffffffu, (p & 32) ? b1r : b0r, p & 31);
         const double vi = __shfl_sync(0xffffffffu, (p & 32) ? b1i : b0i, p & 31);
-        const double qr = x.rdr[k], qi = x.rdi[k];
         const double xr = vr * qr - vi * qi, xi = vr * qi + vi * qr;
         if (k0 >= 0 && k0 < k) {
-            const double ur = Ar[i0 + k * LD], ui = Ai[i0 + k * LD];
-            b0r = fma(-ur, xr, fma(ui, xi, b0r));
-            b0i = fma(-ur, xi, fma(-ui, xr, b0i));
+            b0r = fma(-u0r, xr, fma(u0i, xi, b0r));
+            b0i = fma(-u0r, xi, fma(-u0i, xr, b0i));
         }
         if (k1 >= 0 && k1 < k) {
-            const double ur = Ar[i1 + k * LD], ui = Ai[i1 + k * LD];
-            b1r = fma(-ur, xr, fma(ui, xi, b1r));
-            b1i = fma(-ur, xi, fma(-ui, xr, b1i));
+            b1r = fma(-u1r, xr, fma(u1i, xi, b1r));
+            b1i = fma(-u1r, xi, fma(-u1i, xr, b1i));
         }
         if (wl == 0) { br[k] = xr; bi[k] = xi; }
+        p = pn; qr = qrn; qi = qin;
     }
     __syncwarp();
 }
