@@ -88,14 +88,15 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     std::vector<double> lnA(nr), b(nr), Ta(nr), lnA0(nr, 0.0), b0(nr, 0.0), Ta0(nr, 0.0), dnu(nr), troe(4 * nr, 1.0), eff_dv;
     std::vector<std::vector<std::pair<int, double>>> inc(ns);
     long n_slots_used = 0, n_eff = 0, n_fall = 0, n_troe = 0, n_tb = 0;
-    // Table order: reactions sorted by type (elementary, three-body, Lindemann, Troe; stable), so that the lanes of a
-    // warp that evaluate 32 consecutive reactions follow the same branch (falloff work is not paid by every warp).
+    // Table order: reactions sorted by type, the most expensive first (Troe, Lindemann, three-body, elementary; stable),
+    // so that the lanes of a warp that evaluate 32 consecutive reactions follow the same branch, and so that the first
+    // n_solo (falloff) reactions can be given a thread of their own (see n_solo below).
     std::vector<int> order(nr);
     for (int i = 0; i < nr; i++) {
         if (d->rxn_type[i] < 0 || d->rxn_type[i] > 3) return fail(CHEM_E_ARG, "reaction %d: unknown type %d", i, d->rxn_type[i]);
         order[i] = i;
     }
-    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return d->rxn_type[x] < d->rxn_type[y]; });
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return d->rxn_type[x] > d->rxn_type[y]; });
     for (int i = 0; i < nr; i++) {
         const int si = order[i];              // source reaction of table slot i
         const int ty = d->rxn_type[si];
@@ -196,6 +197,26 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
                 gat[4 * t2 + 3] = lg[k];
             }
             if (lg[k] > gat_steps) gat_steps = lg[k];
+        }
+    }
+    // ---- reaction loop balance of the group kernels: thread t < n_solo evaluates table reaction t only (a Troe reaction
+    // costs six exps against two for an elementary one), the other G - n_solo threads stride over the rest; n_solo
+    // minimises the heaviest thread under the cost model exps + 0.25 per third-body efficiency
+    int n_solo = 0;
+    {
+        std::vector<double> cost(nr);
+        for (int i = 0; i < nr; i++) {
+            const double base = rtype[i] == 3 ? 6.0 : (rtype[i] == 2 ? 3.0 : 2.0);
+            cost[i] = base + (rtype[i] != 0 ? 0.5 + 0.25 * (eff_ptr[i + 1] - eff_ptr[i]) : 0.0);
+        }
+        double best = 1e300;
+        const int n_heavy = (int)(n_fall < G_gather - 1 ? n_fall : G_gather - 1);
+        for (int sN = 0; sN <= n_heavy; sN++) {
+            std::vector<double> load(G_gather - sN, 0.0);
+            for (int i = sN; i < nr; i++) load[(i - sN) % (G_gather - sN)] += cost[i];
+            double mx = sN > 0 ? cost[0] : 0.0;
+            for (double v : load) mx = std::max(mx, v);
+            if (mx < best - 1e-12) { best = mx; n_solo = sN; }
         }
     }
     for (size_t e = 0; e < inc_rx.size(); e++) { inc2.push_back(inc_rx[e]); inc2.push_back((int)inc_nu[e]); }
@@ -327,7 +348,7 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     t.lnA = D(); t.b = D(); t.Ta = D(); t.lnA0 = D(); t.b0 = D(); t.Ta0 = D(); t.dnu = D(); t.troe = D();
     t.eff_dv = D(); t.inc_nu = D(); t.job_lo = D(); t.job_hi = D();
     t.rtype = I(); t.slot_sp = I(); t.slot_nu = I(); t.eff_ptr = I(); t.eff_sp = I(); t.inc_ptr = I(); t.inc_rx = I(); t.rdesc = I();
-    t.gat = reinterpret_cast<const int4 *>(I()); t.inc2 = reinterpret_cast<const int2 *>(I()); t.gat_steps = gat_steps;
+    t.gat = reinterpret_cast<const int4 *>(I()); t.inc2 = reinterpret_cast<const int2 *>(I()); t.gat_steps = gat_steps; t.n_solo = n_solo;
     t.n_jobs = n_jobs; t.n_fo = n_fo; t.tmid0 = tmid[0];
     m->n_sm = n_sm;
     m->max_smem_optin = optin;

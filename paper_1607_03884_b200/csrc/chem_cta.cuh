@@ -109,7 +109,8 @@ __device__ __noinline__ void cta_rhs3(const Tables &tg, const ChemScratch &cs, c
     }
     Grp<G>::sync();
     // ---- rates of progress: each thread owns reactions lane, lane + G, ...; all exps of a reaction in its thread
-    for (int i = lane; i < NR; i += G) {
+    const int rx_step = lane < t.n_solo ? NR : G - t.n_solo;     // the first n_solo (falloff) reactions have a thread each
+    for (int i = lane; i < NR; i += rx_step) {
         const int4 d0 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i);       // f012, f345, type, extra job
         const int4 d1 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i + 1);   // falloff ordinal, eff_lo, eff_hi
         const int type = d0.z;

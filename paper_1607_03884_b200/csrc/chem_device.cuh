@@ -44,6 +44,7 @@ struct Tables {
     const int4 *gat;
     const int2 *inc2;
     int gat_steps;
+    int n_solo;                       // threads t < n_solo evaluate table reaction t only (chem.cu)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -279,7 +280,7 @@ __device__ __noinline__ void rhs(const Tables &tg, const ChemScratch &sg, double
     const double lnT = log(T), invT = 1.0 / T;
     const double Ctot = P / (kRerg * T);
     const double lnPRT = log(kPatm / (kRerg * T));
-    for (int i = lane; i < NR; i += G) s.q[i] = reaction<false>(t, i, T, lnT, invT, lnPRT, Ctot, s);
+    for (int i = lane; i < NR; i += (lane < t.n_solo ? NR : G - t.n_solo)) s.q[i] = reaction<false>(t, i, T, lnT, invT, lnPRT, Ctot, s);
     Grp<G>::sync();
     double hw = 0.0, ccp = 0.0;
     for (int k = lane; k < N; k += G) {
@@ -311,7 +312,7 @@ __device__ __noinline__ void jacobian(const Tables &tg, const ChemScratch &sg, d
     const double lnT = log(T), invT = 1.0 / T;
     const double Ctot = P / (kRerg * T);
     const double lnPRT = log(kPatm / (kRerg * T));
-    for (int i = lane; i < NR; i += G) s.q[i] = reaction<true>(t, i, T, lnT, invT, lnPRT, Ctot, s);
+    for (int i = lane; i < NR; i += (lane < t.n_solo ? NR : G - t.n_solo)) s.q[i] = reaction<true>(t, i, T, lnT, invT, lnPRT, Ctot, s);
     Grp<G>::sync();
     const double invWN = __ldg(&t.invW[N - 1]);
     // rows: species k -> Dw[k][j] = d wdot_k / d y_j, stored in Jm row k
