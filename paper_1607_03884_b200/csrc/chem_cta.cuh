@@ -58,7 +58,7 @@ __device__ __forceinline__ JobRow job_load(const double *c)
 }
 __device__ __forceinline__ double job_eval(const JobRow &r, double T, double lnT, double invT)
 {
-    return exp(r.c01.x + r.c01.y * lnT + r.c23.x * invT + T * (r.c23.y + T * (r.c45.x + T * (r.c45.y + T * r.c67.x))));
+    return exp_f(r.c01.x + r.c01.y * lnT + r.c23.x * invT + T * (r.c23.y + T * (r.c45.x + T * (r.c45.y + T * r.c67.x))));
 }
 __device__ __forceinline__ double job_val(const double *c, double T, double lnT, double invT)
 {
@@ -96,7 +96,7 @@ __device__ __noinline__ void cta_rhs3(const Tables &tg, const ChemScratch &cs, c
         const double sW = vW + YN * __ldg(&t.invW[N - 1]);
         const double invT = 1.0 / T, rho = P / (kRerg * T * sW);
         double *o = x.X0 + 8 * s;
-        o[0] = T; o[1] = log(T); o[2] = invT; o[3] = rho; o[4] = kRerg * T * sW / P; o[5] = P * invT * (1.0 / kRerg);
+        o[0] = T; o[1] = log_f(T); o[2] = invT; o[3] = rho; o[4] = kRerg * T * sW / P; o[5] = P * invT * (1.0 / kRerg);
         x.C3[64 * s + N - 1] = rho * YN * __ldg(&t.invW[N - 1]);
         x.C3[64 * s + 63] = 1.0;
     }
@@ -153,10 +153,10 @@ __device__ __noinline__ void cta_rhs3(const Tables &tg, const ChemScratch &cs, c
     for (int p = lane; p < nstage * nfo; p += G) {
         const double *o = x.X + (size_t)p * 4;
         const double Fc = o[0], Pr = o[1];
-        const double L = log10(Fc);
-        const double At = log10(Pr) - 0.4 - 0.67 * L;
+        const double L = log_f(Fc) * kInvLn10;
+        const double At = log_f(Pr) * kInvLn10 - 0.4 - 0.67 * L;
         const double xx = At * rcp_nr(0.75 - 1.27 * L - 0.14 * At);
-        const double F = exp10(L * rcp_nr(1.0 + xx * xx));
+        const double F = exp_f(kLn10 * L * rcp_nr(1.0 + xx * xx));
         const int s = p / nfo;
         x.q3[s * NR + (int)o[3]] = Pr * rcp_nr(1.0 + Pr) * F * o[2];
     }

@@ -11,6 +11,8 @@
 #include <cuda_runtime.h>
 #include <math.h>
 
+#include "chem_math.cuh"
+
 namespace chem {
 
 constexpr double kRerg = 8.31446261815324e7;  // erg/(mol K)
@@ -92,16 +94,6 @@ __device__ __forceinline__ T *shp(T *p)
     extern __shared__ double chem_smem_window_[];
     const size_t off = __cvta_generic_to_shared(p) - __cvta_generic_to_shared(chem_smem_window_);
     return reinterpret_cast<T *>(reinterpret_cast<char *>(chem_smem_window_) + off);
-}
-
-__device__ __forceinline__ double rcp_nr(double x)   // 1/x for normal x: MUFU seed + two Newton steps
-{
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    return fma(r, e, r);
 }
 
 __device__ __forceinline__ double powi(double c, int nu)
