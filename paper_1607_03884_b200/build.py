@@ -9,8 +9,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libchem.so")
 SOURCES = ["chem.cu"]
-DEPS = ["chem.cu", "chem_device.cuh", "chem_radau.cuh", "chem_kernels.inl", "chem_launch.inl", "chem_warp.cuh",
-        os.path.join("..", "..", "include", "chem.h")]
+
+
+def _deps():
+    """every source, header and .inl under csrc/ plus the C ABI header"""
+    files = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh", ".inl", ".h"))]
+    return files + [os.path.join(HERE, "..", "include", "chem.h")]
 
 
 def nvcc_cmd(extra=()):
@@ -19,7 +23,7 @@ def nvcc_cmd(extra=()):
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    deps = [os.path.join(CSRC, d) for d in DEPS if os.path.exists(os.path.join(CSRC, d))]
+    deps = [d for d in _deps() if os.path.exists(d)]
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     cmd = nvcc_cmd(("-Xptxas", "-v") if verbose else ())
