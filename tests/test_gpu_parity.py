@@ -249,6 +249,25 @@ def test_cost_ordering_does_not_change_results(kind, n, torch_cuda, gpu_mechs, r
     assert np.array_equal(binding.stats_to_numpy(st_a), binding.stats_to_numpy(st_b))
 
 
+@pytest.mark.parametrize("kind,n", [("h2co", 20011), ("gri", 601)])
+def test_results_are_reproducible_and_independent_of_the_batch(kind, n, torch_cuda, gpu_mechs, request):
+    """Work-queue scheduling, the butterfly sums and the gather schedule are deterministic: the same state gives the same
+    bits whatever else is in the batch, in every launch, through the device and the host entry point."""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = descs(request)[kind]
+    y0 = synth.make_states(mech, n, "ignition", 91)
+    y_a, st_a = binding.chem_integrate_ex(gpu_mechs[kind], P, 1e-5, RTOL, ATOL, torch.from_numpy(y0).cuda())
+    y_b, st_b = binding.chem_integrate_ex(gpu_mechs[kind], P, 1e-5, RTOL, ATOL, torch.from_numpy(y0).cuda())
+    assert torch.equal(y_a, y_b)
+    assert np.array_equal(binding.stats_to_numpy(st_a), binding.stats_to_numpy(st_b))
+    perm = np.random.default_rng(5).permutation(n)[: n // 3]            # a shuffled third of the batch
+    y_c, _ = binding.chem_integrate_ex(gpu_mechs[kind], P, 1e-5, RTOL, ATOL, torch.from_numpy(y0[perm].copy()).cuda())
+    assert np.array_equal(y_c.cpu().numpy(), y_a.cpu().numpy()[perm])
+    y_h = binding.chem_integrate_host(gpu_mechs[kind], P, 1e-5, RTOL, ATOL, y0)
+    assert np.array_equal(y_h, y_a.cpu().numpy())
+
+
 @pytest.mark.parametrize("kind,n,kernels", [("h2co", 1500, (1, 2)), ("gri", 300, (0,))])
 def test_finite_difference_jacobian_matches_oracle(kind, n, kernels, torch_cuda, gpu_mechs, orc_mechs, request):
     """PAPER.md L82 / Sec. 3.4: the CVODE-style FD Jacobian variant (R13) against the oracle's"""
