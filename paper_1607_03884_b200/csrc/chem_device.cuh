@@ -664,6 +664,29 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
         }
         Grp<G>::sync();
     }
+    // Epilogue: rows into pivot order (storage row k <- pivot row of step k) and every row of U scaled by 1 / U_kk, so
+    // that a solve is two sweeps whose only chain is shuffle -> fused multiply-add: no pivot look-ups, no selects and
+    // no reciprocal on the chain (solve3_*).  Column by column inside the warp that owns the column: all loads, then
+    // all stores.
+    {
+        const bool g0 = i0 < N, g1 = i1 < N;
+        const int pa0 = g0 ? xa.perm[i0] : N, pa1 = g1 ? xa.perm[i1] : N;
+        const int pc0 = g0 ? xc.perm[i0] : N, pc1 = g1 ? xc.perm[i1] : N;
+        const double ra0 = g0 ? xa.rdr[i0] : 0.0, ra1 = g1 ? xa.rdr[i1] : 0.0;
+        const double qr0 = g0 ? xc.rdr[i0] : 0.0, qi0 = g0 ? xc.rdi[i0] : 0.0;
+        const double qr1 = g1 ? xc.rdr[i1] : 0.0, qi1 = g1 ? xc.rdi[i1] : 0.0;
+#pragma unroll 1
+        for (int j = wp; j < N; j += NW) {
+            double *c = A + j * LD, *cr = Ar + j * LD, *ci = Ai + j * LD;
+            double v0 = c[pa0], v1 = c[pa1];
+            double z0r = cr[pc0], z0i = ci[pc0], z1r = cr[pc1], z1i = ci[pc1];
+            if (j > i0) { v0 *= ra0; const double t = z0r * qr0 - z0i * qi0; z0i = z0r * qi0 + z0i * qr0; z0r = t; }
+            if (j > i1) { v1 *= ra1; const double t = z1r * qr1 - z1i * qi1; z1i = z1r * qi1 + z1i * qr1; z1r = t; }
+            __syncwarp();
+            if (g0) { c[i0] = v0; cr[i0] = z0r; ci[i0] = z0i; }
+            if (g1) { c[i1] = v1; cr[i1] = z1r; ci[i1] = z1i; }
+        }
+    }
     return 0;
 }
 
@@ -752,6 +775,111 @@ __device__ __forceinline__ void solve2_complex_warp(int N, int LD, const double 
     }
     __syncwarp();
 }
+// Solves with the factors as lu2_pair leaves them (rows in pivot order, unit-diagonal scaled U): b (shared, length N,
+// original row order) is overwritten by x.  Lane l holds components l and l + 32; step k broadcasts component k
+// and every later (earlier) row subtracts its multiple: the chain per step is one shuffle and one fused multiply-add
+// (two for the complex system).  Entries outside the triangle are masked to zero when they are loaded, off the chain.
+__device__ __forceinline__ void solve3_real_warp(int N, int LD, const double *A, const Lu2Aux &x, double *b, int wl)
+{
+    const int i0 = wl, i1 = wl + 32;
+    const bool g0 = i0 < N, g1 = i1 < N;
+    const int r0 = g0 ? i0 : N, r1 = g1 ? i1 : N;       // storage rows (N = dummy row of the lu2 layout)
+    double b0 = g0 ? b[x.perm[i0]] : 0.0, b1 = g1 ? b[x.perm[i1]] : 0.0;
+    const double rd0 = g0 ? x.rdr[i0] : 0.0, rd1 = g1 ? x.rdr[i1] : 0.0;
+    const int K1 = N - 1 < 32 ? N - 1 : 32;
+    const double *a0 = A + r0, *a1 = A + r1;
+    int k = 0;
+#pragma unroll 4
+    for (; k < K1; k++, a0 += LD, a1 += LD) {
+        const double l0 = (i0 > k) ? *a0 : 0.0, l1 = g1 ? *a1 : 0.0;
+        const double bk = __shfl_sync(0xffffffffu, b0, k);
+        b0 = fma(-l0, bk, b0);
+        b1 = fma(-l1, bk, b1);
+    }
+#pragma unroll 4
+    for (; k < N - 1; k++, a1 += LD) {
+        const double l1 = (g1 && i1 > k) ? *a1 : 0.0;
+        const double bk = __shfl_sync(0xffffffffu, b1, k - 32);
+        b1 = fma(-l1, bk, b1);
+    }
+    b0 *= rd0; b1 *= rd1;
+    k = N - 1;
+    a0 = A + r0 + k * LD; a1 = A + r1 + k * LD;
+#pragma unroll 4
+    for (; k >= 32; k--, a0 -= LD, a1 -= LD) {
+        const double u0 = *a0, u1 = (i1 < k) ? *a1 : 0.0;
+        const double xk = __shfl_sync(0xffffffffu, b1, k - 32);
+        b0 = fma(-u0, xk, b0);
+        b1 = fma(-u1, xk, b1);
+    }
+#pragma unroll 4
+    for (; k >= 1; k--, a0 -= LD) {
+        const double u0 = (i0 < k) ? *a0 : 0.0;
+        const double xk = __shfl_sync(0xffffffffu, b0, k);
+        b0 = fma(-u0, xk, b0);
+    }
+    __syncwarp();
+    if (g0) b[i0] = b0;
+    if (g1) b[i1] = b1;
+    __syncwarp();
+}
+__device__ __forceinline__ void solve3_complex_warp(int N, int LD, const double *Ar, const double *Ai, const Lu2Aux &x, double *br,
+                                                    double *bi, int wl)
+{
+    const int i0 = wl, i1 = wl + 32;
+    const bool g0 = i0 < N, g1 = i1 < N;
+    const int r0 = g0 ? i0 : N, r1 = g1 ? i1 : N;
+    const int p0 = g0 ? x.perm[i0] : 0, p1 = g1 ? x.perm[i1] : 0;
+    double b0r = g0 ? br[p0] : 0.0, b0i = g0 ? bi[p0] : 0.0, b1r = g1 ? br[p1] : 0.0, b1i = g1 ? bi[p1] : 0.0;
+    const double q0r = g0 ? x.rdr[i0] : 0.0, q0i = g0 ? x.rdi[i0] : 0.0, q1r = g1 ? x.rdr[i1] : 0.0, q1i = g1 ? x.rdi[i1] : 0.0;
+    const int K1 = N - 1 < 32 ? N - 1 : 32;
+    int o0 = r0, o1 = r1;
+    int k = 0;
+#pragma unroll 2
+    for (; k < K1; k++, o0 += LD, o1 += LD) {
+        const bool m0 = i0 > k;
+        const double l0r = m0 ? Ar[o0] : 0.0, l0i = m0 ? Ai[o0] : 0.0, l1r = g1 ? Ar[o1] : 0.0, l1i = g1 ? Ai[o1] : 0.0;
+        const double xr = __shfl_sync(0xffffffffu, b0r, k), xi = __shfl_sync(0xffffffffu, b0i, k);
+        b0r = fma(-l0r, xr, fma(l0i, xi, b0r));
+        b0i = fma(-l0r, xi, fma(-l0i, xr, b0i));
+        b1r = fma(-l1r, xr, fma(l1i, xi, b1r));
+        b1i = fma(-l1r, xi, fma(-l1i, xr, b1i));
+    }
+#pragma unroll 2
+    for (; k < N - 1; k++, o1 += LD) {
+        const bool m1 = g1 && i1 > k;
+        const double l1r = m1 ? Ar[o1] : 0.0, l1i = m1 ? Ai[o1] : 0.0;
+        const double xr = __shfl_sync(0xffffffffu, b1r, k - 32), xi = __shfl_sync(0xffffffffu, b1i, k - 32);
+        b1r = fma(-l1r, xr, fma(l1i, xi, b1r));
+        b1i = fma(-l1r, xi, fma(-l1i, xr, b1i));
+    }
+    { const double t = b0r * q0r - b0i * q0i; b0i = b0r * q0i + b0i * q0r; b0r = t; }
+    { const double t = b1r * q1r - b1i * q1i; b1i = b1r * q1i + b1i * q1r; b1r = t; }
+    k = N - 1;
+    o0 = r0 + k * LD; o1 = r1 + k * LD;
+#pragma unroll 2
+    for (; k >= 32; k--, o0 -= LD, o1 -= LD) {
+        const bool m1 = i1 < k;
+        const double u0r = Ar[o0], u0i = Ai[o0], u1r = m1 ? Ar[o1] : 0.0, u1i = m1 ? Ai[o1] : 0.0;
+        const double xr = __shfl_sync(0xffffffffu, b1r, k - 32), xi = __shfl_sync(0xffffffffu, b1i, k - 32);
+        b0r = fma(-u0r, xr, fma(u0i, xi, b0r));
+        b0i = fma(-u0r, xi, fma(-u0i, xr, b0i));
+        b1r = fma(-u1r, xr, fma(u1i, xi, b1r));
+        b1i = fma(-u1r, xi, fma(-u1i, xr, b1i));
+    }
+#pragma unroll 2
+    for (; k >= 1; k--, o0 -= LD) {
+        const bool m0 = i0 < k;
+        const double u0r = m0 ? Ar[o0] : 0.0, u0i = m0 ? Ai[o0] : 0.0;
+        const double xr = __shfl_sync(0xffffffffu, b0r, k), xi = __shfl_sync(0xffffffffu, b0i, k);
+        b0r = fma(-u0r, xr, fma(u0i, xi, b0r));
+        b0i = fma(-u0r, xi, fma(-u0i, xr, b0i));
+    }
+    __syncwarp();
+    if (g0) { br[i0] = b0r; bi[i0] = b0i; }
+    if (g1) { br[i1] = b1r; bi[i1] = b1i; }
+    __syncwarp();
+}
 template <int G>
 __device__ __noinline__ void solve2_pair(int N, int LD, const double *E1, const Lu2Aux &x1g, double *z1, const double *E2r,
                                          const double *E2i, const Lu2Aux &x2g, double *z2, double *z3)
@@ -759,11 +887,11 @@ __device__ __noinline__ void solve2_pair(int N, int LD, const double *E1, const 
     const Lu2Aux x1 = shp(x1g), x2 = shp(x2g);     // everything below is dynamic shared memory
     E1 = shp(E1); E2r = shp(E2r); E2i = shp(E2i); z1 = shp(z1); z2 = shp(z2); z3 = shp(z3);
     if (G == 32) {
-        solve2_real_warp(N, LD, E1, x1, z1, Grp<G>::wlane());
-        solve2_complex_warp(N, LD, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
+        solve3_real_warp(N, LD, E1, x1, z1, Grp<G>::wlane());
+        solve3_complex_warp(N, LD, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
     } else {
-        if (Grp<G>::warp() == 0) solve2_real_warp(N, LD, E1, x1, z1, Grp<G>::wlane());
-        else if (Grp<G>::warp() == 1) solve2_complex_warp(N, LD, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
+        if (Grp<G>::warp() == 0) solve3_real_warp(N, LD, E1, x1, z1, Grp<G>::wlane());
+        else if (Grp<G>::warp() == 1) solve3_complex_warp(N, LD, E2r, E2i, x2, z2, z3, Grp<G>::wlane());
     }
     Grp<G>::sync();
 }
@@ -772,7 +900,7 @@ __device__ __noinline__ void solve2_real(int N, int LD, const double *E1, const 
 {
     const Lu2Aux x1 = shp(x1g);
     E1 = shp(E1); b = shp(b);
-    if (Grp<G>::warp() == 0) solve2_real_warp(N, LD, E1, x1, b, Grp<G>::wlane());
+    if (Grp<G>::warp() == 0) solve3_real_warp(N, LD, E1, x1, b, Grp<G>::wlane());
     Grp<G>::sync();
 }
 

@@ -175,6 +175,49 @@ __global__ void __launch_bounds__(32) lu_solve_kernel(int n, int batch, int is_c
     }
 }
 
+// The same hook for 16 < n <= 64 through the group kernels' routines (lu2_pair + solve2_pair, chem_device.cuh): one CTA
+// of 128 threads per system.  The routines factor a real and a complex matrix side by side: a real system is given as
+// both (zero imaginary parts), a complex one is paired with the identity.
+__global__ void __launch_bounds__(128) lu2_solve_kernel(int n, int batch, int is_complex, const double *__restrict__ A,
+                                                        const double *__restrict__ b, double *__restrict__ x, int *info)
+{
+    extern __shared__ double smem[];
+    const int LD = n + 1;
+    double *E1 = smem, *E2r = E1 + (size_t)n * LD, *E2i = E2r + (size_t)n * LD, *z1 = E2i + (size_t)n * LD, *z2 = z1 + n, *z3 = z2 + n;
+    Lu2Aux x1, x2;
+    x1.rdr = z3 + n; x1.rdi = nullptr; x2.rdr = x1.rdr + n; x2.rdi = x2.rdr + n;
+    x1.perm = reinterpret_cast<int *>(x2.rdi + n); x1.rowk = x1.perm + n; x2.perm = x1.rowk + n; x2.rowk = x2.perm + n;
+    const int tid = threadIdx.x;
+    for (int s = blockIdx.x; s < batch; s += gridDim.x) {
+        for (int e = tid; e < n * LD; e += 128) { E1[e] = 0.0; E2r[e] = 0.0; E2i[e] = 0.0; }
+        __syncthreads();
+        for (int e = tid; e < n * n; e += 128) {
+            const int i = e / n, j = e % n;
+            const size_t g = (size_t)s * n * n + e;
+            if (is_complex) { E1[i + j * LD] = (i == j) ? 1.0 : 0.0; E2r[i + j * LD] = A[2 * g]; E2i[i + j * LD] = A[2 * g + 1]; }
+            else { E1[i + j * LD] = A[g]; E2r[i + j * LD] = A[g]; }
+        }
+        for (int i = tid; i < n; i += 128) {
+            const size_t g = (size_t)s * n + i;
+            z1[i] = is_complex ? 0.0 : b[g];
+            z2[i] = is_complex ? b[2 * g] : b[g];
+            z3[i] = is_complex ? b[2 * g + 1] : 0.0;
+        }
+        __syncthreads();
+        const int ier = lu2_pair<128>(n, LD, E1, x1, E2r, E2i, x2);
+        __syncthreads();
+        if (!ier) {
+            solve2_pair<128>(n, LD, E1, x1, z1, E2r, E2i, x2, z2, z3);
+            for (int i = tid; i < n; i += 128) {
+                const size_t g = (size_t)s * n + i;
+                if (is_complex) { x[2 * g] = z2[i]; x[2 * g + 1] = z3[i]; } else x[g] = z1[i];
+            }
+        }
+        if (info && tid == 0) info[s] = ier;
+        __syncthreads();
+    }
+}
+
 // The same hook for n <= 16 through the warp path's own routines (gj_warp_pair / solve_warp_pair, chem_warp.cuh):
 // one warp per system, both half-warps are given the system (a real one with zero imaginary parts).
 __global__ void __launch_bounds__(32) lu_solve_warp_kernel(int n, int batch, int is_complex, const double *__restrict__ A,

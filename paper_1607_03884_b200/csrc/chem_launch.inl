@@ -144,6 +144,15 @@ extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const
         CUDA_TRY(cudaGetLastError());
         return CHEM_OK;
     }
+    if (n <= 64) {   // the group kernels' routines (fused real + complex LU, pivot-ordered factors, chain-free solves)
+        const size_t sm = ((size_t)3 * n * (n + 1) + 6 * n) * sizeof(double) + (size_t)4 * n * sizeof(int) + 16;
+        CUDA_TRY(cudaFuncSetAttribute(lu2_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        const int g = batch < 65535 ? batch : 65535;
+        lu2_solve_kernel<<<g, 128, sm, static_cast<cudaStream_t>(stream)>>>(n, batch, is_complex, A, b, x, info);
+        g_launches++;
+        CUDA_TRY(cudaGetLastError());
+        return CHEM_OK;
+    }
     const size_t smem = ((size_t)2 * n * n + 2 * n) * sizeof(double) + (size_t)n * sizeof(int) + 16;
     int dev = 0, optin = 0;
     CUDA_TRY(cudaGetDevice(&dev));

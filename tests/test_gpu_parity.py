@@ -64,7 +64,7 @@ def test_jacobian_matches_oracle(kind, n, torch_cuda, gpu_mechs, orc_mechs, requ
 
 
 @pytest.mark.parametrize("cplx", [False, True])
-@pytest.mark.parametrize("n", [1, 2, 5, 13, 16, 17, 53])    # n <= 16: the warp path's routines, else the group kernels'
+@pytest.mark.parametrize("n", [1, 2, 5, 13, 16, 17, 32, 33, 53, 64, 70])    # n <= 16: warp path routines; <= 64: lu2_pair + solves of the group kernels; above: generic LU
 def test_lu_solve_matches_oracle(n, cplx, torch_cuda):
     from oracle import oracle as orc
     from paper_1607_03884_b200 import binding
@@ -87,7 +87,7 @@ def test_lu_solve_matches_oracle(n, cplx, torch_cuda):
         assert np.allclose(x[s], ref, rtol=1e-9, atol=1e-11 * np.abs(ref).max())
 
 
-@pytest.mark.parametrize("n", [13, 16, 53])
+@pytest.mark.parametrize("n", [13, 16, 40, 53])
 def test_lu_solve_stiff_newton_matrices(n, torch_cuda):
     """Matrices of the shape the integrator factors, gamma/h I - J and (alpha + i beta)/h I - J with a stiff J
     (eigenvalues spread over 12 decades): the residual of the device solve must be at the level of a backward-stable
