@@ -108,12 +108,40 @@ __device__ __noinline__ void cta_rhs3(const Tables &tg, const ChemScratch &cs, c
             if (s < nstage) x.C3[64 * s + k] = x.X0[8 * s + 3] * ys[s][k + 1] * iw;
     }
     Grp<G>::sync();
-    // ---- rates of progress: each thread owns reactions lane, lane + G, ...; all exps of a reaction in its thread
-    const int rx_step = lane < t.n_solo ? NR : G - t.n_solo;     // the first n_solo (falloff) reactions have a thread each
-    for (int i = lane; i < NR; i += rx_step) {
+    // ---- rates of progress.  Work units of equal cost (six exps) and one kind per warp, so that no warp runs two
+    // branches one after the other while the rest of the group waits at the barrier:
+    //   (1) one (falloff reaction, stage) pair per thread: k_f, k_r, k_0/k_inf and the three Troe terms of ONE stage
+    //       (table reactions [0, n_fo) are the falloff reactions: Troe first, then Lindemann);
+    //   (2) one elementary / three-body reaction per thread with ALL stages (two exps per stage), coefficient rows read
+    //       once; the threads behind the last warp that got a falloff pair start first.
+    const int nft = nfo * nstage;
+    for (int q = lane; q < nft; q += G) {
+        const int s = q / nfo, i = q - s * nfo;
         const int4 d0 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i);       // f012, f345, type, extra job
         const int4 d1 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i + 1);   // falloff ordinal, eff_lo, eff_hi
-        const int type = d0.z;
+        const double T = x.X0[8 * s], lnT = x.X0[8 * s + 1], invT = x.X0[8 * s + 2];
+        const double *jt = (T <= t.tmid0) ? t.job_lo : t.job_hi;
+        const double *C = x.C3 + 64 * s;
+        const JobRow rf = job_load(jt + (size_t)i * 8), rr = job_load(jt + (size_t)(NR + i) * 8), r0 = job_load(jt + (size_t)d0.w * 8);
+        const double kf = job_eval(rf, T, lnT, invT), kr = job_eval(rr, T, lnT, invT);
+        const double Rf = kf * (C[d0.x & 255] * C[(d0.x >> 8) & 255] * C[(d0.x >> 16) & 255]);
+        const double Rr = kr * (C[d0.y & 255] * C[(d0.y >> 8) & 255] * C[(d0.y >> 16) & 255]);
+        double M = x.X0[8 * s + 5];
+#pragma unroll 4
+        for (int p = d1.y; p < d1.z; p++) M += __ldg(&t.eff_dv[p]) * C[__ldg(&t.eff_sp[p])];
+        const double Pr = job_eval(r0, T, lnT, invT) * M;
+        double Fc = 1.0;
+        if (d0.z == 3)
+            Fc = job_val(jt + (size_t)(d0.w + 1) * 8, T, lnT, invT) + job_val(jt + (size_t)(d0.w + 2) * 8, T, lnT, invT) +
+                 job_val(jt + (size_t)(d0.w + 3) * 8, T, lnT, invT);
+        double *o = x.X + (size_t)(s * nfo + d1.x) * 4;
+        o[0] = Fc; o[1] = Pr; o[2] = Rf - Rr; o[3] = (double)i;
+    }
+    const int used = nft % G, head = (used + 31) & ~31;                // threads of the last falloff trip, in whole warps
+    const int vt = lane >= head ? lane - head : lane + (G - head);     // virtual thread index of part (2)
+    for (int i = nfo + vt; i < NR; i += G) {
+        const int4 d0 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i);
+        const int4 d1 = __ldg(reinterpret_cast<const int4 *>(t.rdesc) + 2 * i + 1);
         // the coefficient rows of k_f and k_r are read once for all stages when the stages share a NASA range (the rule;
         // job tables live in L2: 49 KB per range for the GRI shape)
         const double *jt0 = (x.X0[0] <= t.tmid0) ? t.job_lo : t.job_hi;
@@ -128,24 +156,14 @@ __device__ __noinline__ void cta_rhs3(const Tables &tg, const ChemScratch &cs, c
             else { kf = job_val(jt + (size_t)i * 8, T, lnT, invT); kr = job_val(jt + (size_t)(NR + i) * 8, T, lnT, invT); }
             const double Rf = kf * (C[d0.x & 255] * C[(d0.x >> 8) & 255] * C[(d0.x >> 16) & 255]);
             const double Rr = kr * (C[d0.y & 255] * C[(d0.y >> 8) & 255] * C[(d0.y >> 16) & 255]);
-            const double rnet = Rf - Rr;
             double c = 1.0;
-            if (type != 0) {
+            if (d0.z != 0) {
                 double M = x.X0[8 * s + 5];
 #pragma unroll 4
                 for (int p = d1.y; p < d1.z; p++) M += __ldg(&t.eff_dv[p]) * C[__ldg(&t.eff_sp[p])];   // unrolled: loads batched
                 c = M;
-                if (type >= 2) {
-                    const double Pr = job_val(jt + (size_t)d0.w * 8, T, lnT, invT) * M;
-                    double Fc = 1.0;
-                    if (type == 3)
-                        Fc = job_val(jt + (size_t)(d0.w + 1) * 8, T, lnT, invT) + job_val(jt + (size_t)(d0.w + 2) * 8, T, lnT, invT) +
-                             job_val(jt + (size_t)(d0.w + 3) * 8, T, lnT, invT);
-                    double *o = x.X + (size_t)(s * nfo + d1.x) * 4;
-                    o[0] = Fc; o[1] = Pr; o[2] = rnet; o[3] = (double)i;
-                }
             }
-            if (type < 2) x.q3[s * NR + i] = c * rnet;
+            x.q3[s * NR + i] = c * (Rf - Rr);
         }
     }
     Grp<G>::sync();
