@@ -499,111 +499,31 @@ __device__ __forceinline__ int warp_argmax_row(double v, int row)
     return __shfl_sync(0xffffffffu, row, __ffs(cand) - 1);
 }
 
-// A is column-major with leading dimension LD = N + 1: row index N is a dummy row that absorbs the updates of
-// row slots that do not exist (lanes with l + 32 >= N), so the trailing update needs no branches; rows that were
-// pivot rows already carry a zero multiplier.
-template <int G>
-__device__ __noinline__ int lu2_real(int N, int LD, double *A, const Lu2Aux &x)
+// exact arg-max of two independent (key, row) sets over a warp in one instruction stream: the two reductions overlap
+// instead of running one after the other; exact ties (rare) take the one-set routine
+__device__ __forceinline__ void warp_argmax_row2(double va, int ra, double vc, int rc, int &pa, int &pc)
 {
-    const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
-    constexpr int NW = Grp<G>::NW;
-    const int i0 = wl, i1 = wl + 32;
-    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;             // storage rows (N = dummy)
-    int k0 = (i0 < N) ? -1 : 1 << 30, k1 = (i1 < N) ? -1 : 1 << 30;   // rowk of my two rows (huge = no such row)
-    double l0 = 0.0, l1 = 0.0;
-    for (int k = 0; k < N; k++) {
-        // delayed write-back of the multipliers of column k-1 by its owner warp
-        if (k > 0 && wp == (k - 1) % NW) {
-            if (k0 < 0) A[i0 + (k - 1) * LD] = l0;
-            if (k1 < 0) A[i1 + (k - 1) * LD] = l1;
-        }
-        const double a0 = (k0 < 0) ? A[i0 + k * LD] : 0.0, a1 = (k1 < 0) ? A[i1 + k * LD] : 0.0;
-        const double v0 = (k0 < 0) ? fabs(a0) : -1.0, v1 = (k1 < 0) ? fabs(a1) : -1.0;
-        const int p = warp_argmax_row(v1 > v0 ? v1 : v0, v1 > v0 ? i1 : i0);
-        const double pv = (p >= 0) ? A[p + k * LD] : 0.0;
-        if (p < 0 || !isfinite(pv)) return k + 1;
-        const double rp = rcp_nr(pv);
-        if (i0 == p) k0 = k;
-        if (i1 == p) k1 = k;
-        if (lane == 0) { x.perm[k] = p; x.rdr[k] = rp; x.rowk[p] = k; }
-        l0 = (k0 < 0) ? a0 * rp : 0.0;
-        l1 = (k1 < 0) ? a1 * rp : 0.0;
-        const int j0 = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
-        double *c = A + j0 * LD;
-        // two of this warp's columns per trip, all loads before the stores (the update is bound by shared-memory round
-        // trips; the compiler cannot move a load above a store that might alias)
-#pragma unroll 1
-        for (int j = j0; j < N; j += 2 * NW, c += 2 * NW * LD) {
-            const bool two = j + NW < N;
-            double *c2 = c + (two ? NW * LD : 0);
-            const double u = c[p], x0 = c[r0], x1 = c[r1], u2 = c2[p], y0 = c2[r0], y1 = c2[r1];
-            c[r0] = fma(-l0, u, x0);
-            c[r1] = fma(-l1, u, x1);
-            if (two) {
-                c2[r0] = fma(-l0, u2, y0);
-                c2[r1] = fma(-l1, u2, y1);
-            }
-        }
-        Grp<G>::sync();
+    const bool aa = va >= 0.0, ac = vc >= 0.0;
+    const unsigned ha = aa ? (unsigned)__double2hiint(va) : 0u, hc = ac ? (unsigned)__double2hiint(vc) : 0u;
+    const unsigned ma = __reduce_max_sync(0xffffffffu, ha), mc = __reduce_max_sync(0xffffffffu, hc);
+    const unsigned ca = __ballot_sync(0xffffffffu, aa && ha == ma), cc = __ballot_sync(0xffffffffu, ac && hc == mc);
+    if (__popc(ca) == 1 && __popc(cc) == 1) {
+        pa = __shfl_sync(0xffffffffu, ra, __ffs(ca) - 1);
+        pc = __shfl_sync(0xffffffffu, rc, __ffs(cc) - 1);
+    } else {
+        pa = warp_argmax_row(va, ra);
+        pc = warp_argmax_row(vc, rc);
     }
-    return 0;
-}
-
-template <int G>
-__device__ __noinline__ int lu2_complex(int N, int LD, double *Ar, double *Ai, const Lu2Aux &x)
-{
-    const int lane = Grp<G>::lane(), wl = Grp<G>::wlane(), wp = Grp<G>::warp();
-    constexpr int NW = Grp<G>::NW;
-    const int i0 = wl, i1 = wl + 32;
-    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;
-    int k0 = (i0 < N) ? -1 : 1 << 30, k1 = (i1 < N) ? -1 : 1 << 30;
-    double l0r = 0.0, l0i = 0.0, l1r = 0.0, l1i = 0.0;
-    for (int k = 0; k < N; k++) {
-        if (k > 0 && wp == (k - 1) % NW) {
-            if (k0 < 0) { Ar[i0 + (k - 1) * LD] = l0r; Ai[i0 + (k - 1) * LD] = l0i; }
-            if (k1 < 0) { Ar[i1 + (k - 1) * LD] = l1r; Ai[i1 + (k - 1) * LD] = l1i; }
-        }
-        const double a0r = (k0 < 0) ? Ar[i0 + k * LD] : 0.0, a0i = (k0 < 0) ? Ai[i0 + k * LD] : 0.0;
-        const double a1r = (k1 < 0) ? Ar[i1 + k * LD] : 0.0, a1i = (k1 < 0) ? Ai[i1 + k * LD] : 0.0;
-        const double v0 = (k0 < 0) ? fabs(a0r) + fabs(a0i) : -1.0, v1 = (k1 < 0) ? fabs(a1r) + fabs(a1i) : -1.0;
-        const int p = warp_argmax_row(v1 > v0 ? v1 : v0, v1 > v0 ? i1 : i0);
-        const double pr = (p >= 0) ? Ar[p + k * LD] : 0.0, pi = (p >= 0) ? Ai[p + k * LD] : 0.0;
-        const double den = rcp_nr(pr * pr + pi * pi);
-        if (p < 0 || !isfinite(den)) return k + 1;
-        const double qr = pr * den, qi = -pi * den;       // 1 / pivot
-        if (i0 == p) k0 = k;
-        if (i1 == p) k1 = k;
-        if (lane == 0) { x.perm[k] = p; x.rdr[k] = qr; x.rdi[k] = qi; x.rowk[p] = k; }
-        l0r = (k0 < 0) ? a0r * qr - a0i * qi : 0.0; l0i = (k0 < 0) ? a0r * qi + a0i * qr : 0.0;
-        l1r = (k1 < 0) ? a1r * qr - a1i * qi : 0.0; l1i = (k1 < 0) ? a1r * qi + a1i * qr : 0.0;
-        const int j0 = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
-        double *cr = Ar + j0 * LD, *ci = Ai + j0 * LD;
-#pragma unroll 1
-        for (int j = j0; j < N; j += 2 * NW, cr += 2 * NW * LD, ci += 2 * NW * LD) {
-            const bool two = j + NW < N;
-            double *dr = cr + (two ? NW * LD : 0), *di = ci + (two ? NW * LD : 0);
-            const double ur = cr[p], ui = ci[p], x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
-            const double vr = dr[p], vi = di[p], y0r = dr[r0], y0i = di[r0], y1r = dr[r1], y1i = di[r1];
-            cr[r0] = fma(-l0r, ur, fma(l0i, ui, x0r));
-            ci[r0] = fma(-l0r, ui, fma(-l0i, ur, x0i));
-            cr[r1] = fma(-l1r, ur, fma(l1i, ui, x1r));
-            ci[r1] = fma(-l1r, ui, fma(-l1i, ur, x1i));
-            if (two) {
-                dr[r0] = fma(-l0r, vr, fma(l0i, vi, y0r));
-                di[r0] = fma(-l0r, vi, fma(-l0i, vr, y0i));
-                dr[r1] = fma(-l1r, vr, fma(l1i, vi, y1r));
-                di[r1] = fma(-l1r, vi, fma(-l1i, vr, y1i));
-            }
-        }
-        Grp<G>::sync();
-    }
-    return 0;
 }
 
 // Both factorisations of a Radau step in ONE pass: per elimination step the pivot search, reciprocal and multipliers of the
 // real and of the complex matrix are two independent dependency chains that overlap, and the step needs one barrier
-// instead of two.  Same arithmetic, pivots and storage as lu2_real / lu2_complex; returns k + 1 if either matrix has no
-// usable pivot at step k.
+// instead of two.  Column-major with leading dimension LD = N + 1 (row N is a dummy row that absorbs the updates of
+// lanes whose second row does not exist, so the trailing update needs no branches; rows that were pivot rows already
+// carry a zero multiplier).  Lane l of EVERY warp tracks rows l and l + 32 (their multipliers stay in registers, the
+// pivot search is done redundantly per warp), warp w updates the columns j = w (mod NW).  Multipliers of column k are
+// written back one step late by the warp that owns the column, so that no warp can still be reading the column.
+// perm[k] = pivot row of step k, rd[k] = 1 / U_kk.  Returns k + 1 if either matrix has no usable pivot at step k.
 template <int G>
 __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag, double *Ar, double *Ai, const Lu2Aux &xcg)
 {
@@ -616,6 +536,7 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
     int ka0 = (i0 < N) ? -1 : 1 << 30, ka1 = (i1 < N) ? -1 : 1 << 30; // rowk of my two rows in the real matrix
     int kc0 = ka0, kc1 = ka1;                                         // ... in the complex matrix
     double l0 = 0.0, l1 = 0.0, l0r = 0.0, l0i = 0.0, l1r = 0.0, l1i = 0.0;
+    const int stride = NW * LD;
     for (int k = 0; k < N; k++) {
         if (k > 0 && wp == (k - 1) % NW) {                            // delayed write-back of the multipliers of column k-1
             if (ka0 < 0) A[i0 + (k - 1) * LD] = l0;
@@ -628,13 +549,13 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
         const double a1r = (kc1 < 0) ? Ar[i1 + k * LD] : 0.0, a1i = (kc1 < 0) ? Ai[i1 + k * LD] : 0.0;
         const double va0 = (ka0 < 0) ? fabs(a0) : -1.0, va1 = (ka1 < 0) ? fabs(a1) : -1.0;
         const double vc0 = (kc0 < 0) ? fabs(a0r) + fabs(a0i) : -1.0, vc1 = (kc1 < 0) ? fabs(a1r) + fabs(a1i) : -1.0;
-        const int pa = warp_argmax_row(va1 > va0 ? va1 : va0, va1 > va0 ? i1 : i0);
-        const int pc = warp_argmax_row(vc1 > vc0 ? vc1 : vc0, vc1 > vc0 ? i1 : i0);
+        int pa, pc;
+        warp_argmax_row2(va1 > va0 ? va1 : va0, va1 > va0 ? i1 : i0, vc1 > vc0 ? vc1 : vc0, vc1 > vc0 ? i1 : i0, pa, pc);
         const double pv = (pa >= 0) ? A[pa + k * LD] : 0.0;
         const double pr = (pc >= 0) ? Ar[pc + k * LD] : 0.0, pi = (pc >= 0) ? Ai[pc + k * LD] : 0.0;
         const double den = rcp_nr(pr * pr + pi * pi);
+        const double rp = rcp_nr(pv);                                 // both reciprocals before the test: they overlap
         if (pa < 0 || !isfinite(pv) || pc < 0 || !isfinite(den)) return k + 1;
-        const double rp = rcp_nr(pv);
         const double qr = pr * den, qi = -pi * den;                   // 1 / complex pivot
         if (i0 == pa) ka0 = k;
         if (i1 == pa) ka1 = k;
@@ -648,19 +569,41 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
         l1 = (ka1 < 0) ? a1 * rp : 0.0;
         l0r = (kc0 < 0) ? a0r * qr - a0i * qi : 0.0; l0i = (kc0 < 0) ? a0r * qi + a0i * qr : 0.0;
         l1r = (kc1 < 0) ? a1r * qr - a1i * qi : 0.0; l1i = (kc1 < 0) ? a1r * qi + a1i * qr : 0.0;
-        const int j0 = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
-        double *c = A + j0 * LD, *cr = Ar + j0 * LD, *ci = Ai + j0 * LD;
+        // Trailing update of this warp's columns, software-pipelined by hand: the operands of the NEXT column are
+        // requested before the results of the current one are stored (the compiler cannot move a load above a store
+        // that might alias, and with two warps per scheduler nothing else hides the shared-memory round trip).  Two
+        // register sets alternate, so nothing is copied.
+        int j = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
+        if (j < N) {
+            double *c = A + j * LD, *cr = Ar + j * LD, *ci = Ai + j * LD;
+            double u = c[pa], x0 = c[r0], x1 = c[r1];
+            double ur = cr[pc], ui = ci[pc], x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
 #pragma unroll 1
-        for (int j = j0; j < N; j += NW, c += NW * LD, cr += NW * LD, ci += NW * LD) {
-            // one column of each matrix per trip, all loads before the stores
-            const double u = c[pa], x0 = c[r0], x1 = c[r1];
-            const double ur = cr[pc], ui = ci[pc], x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
-            c[r0] = fma(-l0, u, x0);
-            c[r1] = fma(-l1, u, x1);
-            cr[r0] = fma(-l0r, ur, fma(l0i, ui, x0r));
-            ci[r0] = fma(-l0r, ui, fma(-l0i, ur, x0i));
-            cr[r1] = fma(-l1r, ur, fma(l1i, ui, x1r));
-            ci[r1] = fma(-l1r, ui, fma(-l1i, ur, x1i));
+            for (;;) {
+                const bool mb = j + NW < N;                           // is there a column for set B?
+                double *d = c + (mb ? stride : 0), *dr = cr + (mb ? stride : 0), *di = ci + (mb ? stride : 0);
+                const double v = d[pa], y0 = d[r0], y1 = d[r1];
+                const double vr = dr[pc], vi = di[pc], y0r = dr[r0], y0i = di[r0], y1r = dr[r1], y1i = di[r1];
+                c[r0] = fma(-l0, u, x0);
+                c[r1] = fma(-l1, u, x1);
+                cr[r0] = fma(-l0r, ur, fma(l0i, ui, x0r));
+                ci[r0] = fma(-l0r, ui, fma(-l0i, ur, x0i));
+                cr[r1] = fma(-l1r, ur, fma(l1i, ui, x1r));
+                ci[r1] = fma(-l1r, ui, fma(-l1i, ur, x1i));
+                if (!mb) break;
+                const bool ma = j + 2 * NW < N;                       // ... and one for set A again?
+                c = d + (ma ? stride : 0); cr = dr + (ma ? stride : 0); ci = di + (ma ? stride : 0);
+                u = c[pa]; x0 = c[r0]; x1 = c[r1];
+                ur = cr[pc]; ui = ci[pc]; x0r = cr[r0]; x0i = ci[r0]; x1r = cr[r1]; x1i = ci[r1];
+                d[r0] = fma(-l0, v, y0);
+                d[r1] = fma(-l1, v, y1);
+                dr[r0] = fma(-l0r, vr, fma(l0i, vi, y0r));
+                di[r0] = fma(-l0r, vi, fma(-l0i, vr, y0i));
+                dr[r1] = fma(-l1r, vr, fma(l1i, vi, y1r));
+                di[r1] = fma(-l1r, vi, fma(-l1i, vr, y1i));
+                if (!ma) break;
+                j += 2 * NW;
+            }
         }
         Grp<G>::sync();
     }
@@ -690,91 +633,6 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
     return 0;
 }
 
-// Solves with the lu2 factors by ONE warp: b (shared, length N, original row order) is overwritten by x.
-// Each step is one link of a dependency chain (broadcast of the finished component -> update of the remaining rows).
-// Everything that is not on the chain is issued ahead of it: the pivot row of the NEXT step is fetched one step early and
-// the matrix entries are loaded unconditionally (storage row N is the dummy row of the lu2 layout) before the broadcast.
-__device__ __forceinline__ void solve2_real_warp(int N, int LD, const double *A, const Lu2Aux &x, double *b, int wl)
-{
-    const int i0 = wl, i1 = wl + 32;
-    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;
-    const int k0 = (i0 < N) ? x.rowk[i0] : -1, k1 = (i1 < N) ? x.rowk[i1] : -1;   // -1: no such row (never updated)
-    double b0 = (i0 < N) ? b[i0] : 0.0, b1 = (i1 < N) ? b[i1] : 0.0;
-    int p = x.perm[0];
-#pragma unroll 1
-    for (int k = 0; k < N - 1; k++) {
-        const int pn = x.perm[k + 1];
-        const double l0 = A[r0 + k * LD], l1 = A[r1 + k * LD];
-        const double bk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31);
-        if (k0 > k) b0 = fma(-l0, bk, b0);
-        if (k1 > k) b1 = fma(-l1, bk, b1);
-        p = pn;
-    }
-    __syncwarp();
-    double rd = x.rdr[N - 1];
-#pragma unroll 1
-    for (int k = N - 1; k >= 0; k--) {
-        const int pn = x.perm[k > 0 ? k - 1 : 0];
-        const double rdn = x.rdr[k > 0 ? k - 1 : 0];
-        const double u0 = A[r0 + k * LD], u1 = A[r1 + k * LD];
-        const double xk = __shfl_sync(0xffffffffu, (p & 32) ? b1 : b0, p & 31) * rd;
-        if (k0 >= 0 && k0 < k) b0 = fma(-u0, xk, b0);
-        if (k1 >= 0 && k1 < k) b1 = fma(-u1, xk, b1);
-        if (wl == 0) b[k] = xk;
-        p = pn;
-        rd = rdn;
-    }
-    __syncwarp();
-}
-__device__ __forceinline__ void solve2_complex_warp(int N, int LD, const double *Ar, const double *Ai, const Lu2Aux &x, double *br,
-                                                    double *bi, int wl)
-{
-    const int i0 = wl, i1 = wl + 32;
-    const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;
-    const int k0 = (i0 < N) ? x.rowk[i0] : -1, k1 = (i1 < N) ? x.rowk[i1] : -1;
-    double b0r = (i0 < N) ? br[i0] : 0.0, b0i = (i0 < N) ? bi[i0] : 0.0;
-    double b1r = (i1 < N) ? br[i1] : 0.0, b1i = (i1 < N) ? bi[i1] : 0.0;
-    int p = x.perm[0];
-#pragma unroll 1
-    for (int k = 0; k < N - 1; k++) {
-        const int pn = x.perm[k + 1];
-        const double l0r = Ar[r0 + k * LD], l0i = Ai[r0 + k * LD], l1r = Ar[r1 + k * LD], l1i = Ai[r1 + k * LD];
-        const double xr = __shfl_sync(0xffffffffu, (p & 32) ? b1r : b0r, p & 31);
-        const double xi = __shfl_sync(0xffffffffu, (p & 32) ? b1i : b0i, p & 31);
-        if (k0 > k) {
-            b0r = fma(-l0r, xr, fma(l0i, xi, b0r));
-            b0i = fma(-l0r, xi, fma(-l0i, xr, b0i));
-        }
-        if (k1 > k) {
-            b1r = fma(-l1r, xr, fma(l1i, xi, b1r));
-            b1i = fma(-l1r, xi, fma(-l1i, xr, b1i));
-        }
-        p = pn;
-    }
-    __syncwarp();
-    double qr = x.rdr[N - 1], qi = x.rdi[N - 1];
-#pragma unroll 1
-    for (int k = N - 1; k >= 0; k--) {
-        const int kn = k > 0 ? k - 1 : 0;
-        const int pn = x.perm[kn];
-        const double qrn = x.rdr[kn], qin = x.rdi[kn];
-        const double u0r = Ar[r0 + k * LD], u0i = Ai[r0 + k * LD], u1r = Ar[r1 + k * LD], u1i = Ai[r1 + k * LD];
-        const double vr = __shfl_sync(0xffffffffu, (p & 32) ? b1r : b0r, p & 31);
-        const double vi = __shfl_sync(0xffffffffu, (p & 32) ? b1i : b0i, p & 31);
-        const double xr = vr * qr - vi * qi, xi = vr * qi + vi * qr;
-        if (k0 >= 0 && k0 < k) {
-            b0r = fma(-u0r, xr, fma(u0i, xi, b0r));
-            b0i = fma(-u0r, xi, fma(-u0i, xr, b0i));
-        }
-        if (k1 >= 0 && k1 < k) {
-            b1r = fma(-u1r, xr, fma(u1i, xi, b1r));
-            b1i = fma(-u1r, xi, fma(-u1i, xr, b1i));
-        }
-        if (wl == 0) { br[k] = xr; bi[k] = xi; }
-        p = pn; qr = qrn; qi = qin;
-    }
-    __syncwarp();
-}
 // Solves with the factors as lu2_pair leaves them (rows in pivot order, unit-diagonal scaled U): b (shared, length N,
 // original row order) is overwritten by x.  Lane l holds components l and l + 32; step k broadcasts component k
 // and every later (earlier) row subtracts its multiple: the chain per step is one shuffle and one fused multiply-add
