@@ -516,14 +516,21 @@ __device__ __forceinline__ void warp_argmax_row2(double va, int ra, double vc, i
     }
 }
 
-// Both factorisations of a Radau step in ONE pass: per elimination step the pivot search, reciprocal and multipliers of the
-// real and of the complex matrix are two independent dependency chains that overlap, and the step needs one barrier
-// instead of two.  Column-major with leading dimension LD = N + 1 (row N is a dummy row that absorbs the updates of
-// lanes whose second row does not exist, so the trailing update needs no branches; rows that were pivot rows already
-// carry a zero multiplier).  Lane l of EVERY warp tracks rows l and l + 32 (their multipliers stay in registers, the
-// pivot search is done redundantly per warp), warp w updates the columns j = w (mod NW).  Multipliers of column k are
-// written back one step late by the warp that owns the column, so that no warp can still be reading the column.
-// perm[k] = pivot row of step k, rd[k] = 1 / U_kk.  Returns k + 1 if either matrix has no usable pivot at step k.
+// Both factorisations of a Radau step in ONE pass, TWO elimination steps per sweep over the trailing matrix.
+// Column-major with leading dimension LD = N + 1 (row N is a dummy row that absorbs the updates of lanes whose second
+// row does not exist, so the trailing update needs no branches; rows that were pivot rows already carry a zero
+// multiplier).  Lane l of EVERY warp tracks rows l and l + 32 (pivot search, reciprocals and multipliers are computed
+// redundantly per warp: no exchange), warp w updates the columns j = w (mod NW).
+// The trailing update is bound by shared-memory bandwidth (a load and a store per fused multiply-add), so steps k and
+// k + 1 share one sweep: after the pivot of step k is known every warp updates column k + 1 for its own rows in
+// registers, finds the pivot of step k + 1 there, and then each entry of the columns j >= k + 2 is loaded once, takes
+//     x <- fma(-m, v', fma(-l, u, x)),   v' = fma(-t, u, v)
+// (u, v = entries of the two pivot rows in column j, l, m = the row's multipliers of the two steps, t = multiplier of
+// step k of pivot row k + 1) and is stored once: the operations and their order are exactly those of two rank-one
+// steps, at 30 instead of 54 shared-memory wavefronts per column and with one barrier for two steps.
+// Columns k and k + 1 (multipliers, and U_{k+1,k+1}) are written back one sweep late by the warps that own them, so
+// that no warp can still be reading them.  perm[k] = pivot row of step k, rd[k] = 1 / U_kk.  Returns k + 1 if either
+// matrix has no usable pivot at step k.
 template <int G>
 __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag, double *Ar, double *Ai, const Lu2Aux &xcg)
 {
@@ -535,15 +542,27 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
     const int r0 = i0 < N ? i0 : N, r1 = i1 < N ? i1 : N;             // storage rows (N = dummy)
     int ka0 = (i0 < N) ? -1 : 1 << 30, ka1 = (i1 < N) ? -1 : 1 << 30; // rowk of my two rows in the real matrix
     int kc0 = ka0, kc1 = ka1;                                         // ... in the complex matrix
+    // multipliers of the first step of a sweep (column k), values for column k + 1 (multiplier or U_{k+1,k+1})
     double l0 = 0.0, l1 = 0.0, l0r = 0.0, l0i = 0.0, l1r = 0.0, l1i = 0.0;
-    const int stride = NW * LD;
-    for (int k = 0; k < N; k++) {
-        if (k > 0 && wp == (k - 1) % NW) {                            // delayed write-back of the multipliers of column k-1
-            if (ka0 < 0) A[i0 + (k - 1) * LD] = l0;
-            if (ka1 < 0) A[i1 + (k - 1) * LD] = l1;
-            if (kc0 < 0) { Ar[i0 + (k - 1) * LD] = l0r; Ai[i0 + (k - 1) * LD] = l0i; }
-            if (kc1 < 0) { Ar[i1 + (k - 1) * LD] = l1r; Ai[i1 + (k - 1) * LD] = l1i; }
+    double w0 = 0.0, w1 = 0.0, w0r = 0.0, w0i = 0.0, w1r = 0.0, w1i = 0.0;
+    auto open_after = [](int kx, int k) { return kx < 0 || (kx > k && kx < (1 << 30)); };   // row not yet a pivot row after step k
+    auto write_back = [&](int k) {       // columns k, k + 1 of the sweep that started at step k
+        const bool e0 = open_after(ka0, k), e1 = open_after(ka1, k), f0 = open_after(kc0, k), f1 = open_after(kc1, k);
+        if (wp == k % NW) {
+            if (e0) A[i0 + k * LD] = l0;
+            if (e1) A[i1 + k * LD] = l1;
+            if (f0) { Ar[i0 + k * LD] = l0r; Ai[i0 + k * LD] = l0i; }
+            if (f1) { Ar[i1 + k * LD] = l1r; Ai[i1 + k * LD] = l1i; }
         }
+        if (k + 1 < N && wp == (k + 1) % NW) {
+            if (e0) A[i0 + (k + 1) * LD] = w0;
+            if (e1) A[i1 + (k + 1) * LD] = w1;
+            if (f0) { Ar[i0 + (k + 1) * LD] = w0r; Ai[i0 + (k + 1) * LD] = w0i; }
+            if (f1) { Ar[i1 + (k + 1) * LD] = w1r; Ai[i1 + (k + 1) * LD] = w1i; }
+        }
+    };
+    for (int k = 0; k < N; k += 2) {
+        // ---- step k: pivot search in column k, reciprocals, multipliers
         const double a0 = (ka0 < 0) ? A[i0 + k * LD] : 0.0, a1 = (ka1 < 0) ? A[i1 + k * LD] : 0.0;
         const double a0r = (kc0 < 0) ? Ar[i0 + k * LD] : 0.0, a0i = (kc0 < 0) ? Ai[i0 + k * LD] : 0.0;
         const double a1r = (kc1 < 0) ? Ar[i1 + k * LD] : 0.0, a1i = (kc1 < 0) ? Ai[i1 + k * LD] : 0.0;
@@ -565,48 +584,82 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
             xa.perm[k] = pa; xa.rdr[k] = rp; xa.rowk[pa] = k;
             xc.perm[k] = pc; xc.rdr[k] = qr; xc.rdi[k] = qi; xc.rowk[pc] = k;
         }
+        // the previous sweep's columns can be written now: every warp has passed the barrier behind its last read
+        // (the values are consumed before l, w are overwritten below)
+        if (k > 0) write_back(k - 2);
         l0 = (ka0 < 0) ? a0 * rp : 0.0;
         l1 = (ka1 < 0) ? a1 * rp : 0.0;
         l0r = (kc0 < 0) ? a0r * qr - a0i * qi : 0.0; l0i = (kc0 < 0) ? a0r * qi + a0i * qr : 0.0;
         l1r = (kc1 < 0) ? a1r * qr - a1i * qi : 0.0; l1i = (kc1 < 0) ? a1r * qi + a1i * qr : 0.0;
-        // Trailing update of this warp's columns, software-pipelined by hand: the operands of the NEXT column are
-        // requested before the results of the current one are stored (the compiler cannot move a load above a store
-        // that might alias, and with two warps per scheduler nothing else hides the shared-memory round trip).  Two
-        // register sets alternate, so nothing is copied.
-        int j = k + 1 + ((wp - (k + 1)) % NW + NW) % NW;
-        if (j < N) {
-            double *c = A + j * LD, *cr = Ar + j * LD, *ci = Ai + j * LD;
-            double u = c[pa], x0 = c[r0], x1 = c[r1];
-            double ur = cr[pc], ui = ci[pc], x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
+        if (k + 1 < N) {
+            // ---- step k + 1: column k + 1 after step k for my rows (registers only), pivot search, multipliers
+            const int kk = k + 1;
+            const double uk = A[pa + kk * LD], ukr = Ar[pc + kk * LD], uki = Ai[pc + kk * LD];
+            const double y0 = (ka0 < 0) ? fma(-l0, uk, A[i0 + kk * LD]) : 0.0, y1 = (ka1 < 0) ? fma(-l1, uk, A[i1 + kk * LD]) : 0.0;
+            double y0r = 0.0, y0i = 0.0, y1r = 0.0, y1i = 0.0;
+            if (kc0 < 0) {
+                const double xr = Ar[i0 + kk * LD], xi = Ai[i0 + kk * LD];
+                y0r = fma(-l0r, ukr, fma(l0i, uki, xr)); y0i = fma(-l0r, uki, fma(-l0i, ukr, xi));
+            }
+            if (kc1 < 0) {
+                const double xr = Ar[i1 + kk * LD], xi = Ai[i1 + kk * LD];
+                y1r = fma(-l1r, ukr, fma(l1i, uki, xr)); y1i = fma(-l1r, uki, fma(-l1i, ukr, xi));
+            }
+            const double ya0 = (ka0 < 0) ? fabs(y0) : -1.0, ya1 = (ka1 < 0) ? fabs(y1) : -1.0;
+            const double yc0 = (kc0 < 0) ? fabs(y0r) + fabs(y0i) : -1.0, yc1 = (kc1 < 0) ? fabs(y1r) + fabs(y1i) : -1.0;
+            int pa2, pc2;
+            warp_argmax_row2(ya1 > ya0 ? ya1 : ya0, ya1 > ya0 ? i1 : i0, yc1 > yc0 ? yc1 : yc0, yc1 > yc0 ? i1 : i0, pa2, pc2);
+            const int sa = pa2 < 0 ? 0 : pa2, sc = pc2 < 0 ? 0 : pc2;
+            // pivot values and the step-k multipliers of the two new pivot rows sit in the lanes that hold those rows
+            const double pv2 = __shfl_sync(0xffffffffu, (sa & 32) ? y1 : y0, sa & 31);
+            const double tl = __shfl_sync(0xffffffffu, (sa & 32) ? l1 : l0, sa & 31);
+            const double pr2 = __shfl_sync(0xffffffffu, (sc & 32) ? y1r : y0r, sc & 31);
+            const double pi2 = __shfl_sync(0xffffffffu, (sc & 32) ? y1i : y0i, sc & 31);
+            const double tlr = __shfl_sync(0xffffffffu, (sc & 32) ? l1r : l0r, sc & 31);
+            const double tli = __shfl_sync(0xffffffffu, (sc & 32) ? l1i : l0i, sc & 31);
+            const double den2 = rcp_nr(pr2 * pr2 + pi2 * pi2);
+            const double rp2 = rcp_nr(pv2);
+            if (pa2 < 0 || !isfinite(pv2) || pc2 < 0 || !isfinite(den2)) return kk + 1;
+            const double qr2 = pr2 * den2, qi2 = -pi2 * den2;
+            if (i0 == pa2) ka0 = kk;
+            if (i1 == pa2) ka1 = kk;
+            if (i0 == pc2) kc0 = kk;
+            if (i1 == pc2) kc1 = kk;
+            if (lane == 0) {
+                xa.perm[kk] = pa2; xa.rdr[kk] = rp2; xa.rowk[pa2] = kk;
+                xc.perm[kk] = pc2; xc.rdr[kk] = qr2; xc.rdi[kk] = qi2; xc.rowk[pc2] = kk;
+            }
+            const double m0 = (ka0 < 0) ? y0 * rp2 : 0.0, m1 = (ka1 < 0) ? y1 * rp2 : 0.0;
+            const double m0r = (kc0 < 0) ? y0r * qr2 - y0i * qi2 : 0.0, m0i = (kc0 < 0) ? y0r * qi2 + y0i * qr2 : 0.0;
+            const double m1r = (kc1 < 0) ? y1r * qr2 - y1i * qi2 : 0.0, m1i = (kc1 < 0) ? y1r * qi2 + y1i * qr2 : 0.0;
+            // column k + 1 as it will be stored: U_{k+1,k+1} in the new pivot row, multipliers below
+            w0 = (ka0 == kk) ? y0 : m0; w1 = (ka1 == kk) ? y1 : m1;
+            w0r = (kc0 == kk) ? y0r : m0r; w0i = (kc0 == kk) ? y0i : m0i;
+            w1r = (kc1 == kk) ? y1r : m1r; w1i = (kc1 == kk) ? y1i : m1i;
+            // ---- both steps on the columns j >= k + 2 of this warp
+            const int j0 = k + 2 + ((wp - (k + 2)) % NW + NW) % NW;
+            double *c = A + j0 * LD, *cr = Ar + j0 * LD, *ci = Ai + j0 * LD;
 #pragma unroll 1
-            for (;;) {
-                const bool mb = j + NW < N;                           // is there a column for set B?
-                double *d = c + (mb ? stride : 0), *dr = cr + (mb ? stride : 0), *di = ci + (mb ? stride : 0);
-                const double v = d[pa], y0 = d[r0], y1 = d[r1];
-                const double vr = dr[pc], vi = di[pc], y0r = dr[r0], y0i = di[r0], y1r = dr[r1], y1i = di[r1];
-                c[r0] = fma(-l0, u, x0);
-                c[r1] = fma(-l1, u, x1);
-                cr[r0] = fma(-l0r, ur, fma(l0i, ui, x0r));
-                ci[r0] = fma(-l0r, ui, fma(-l0i, ur, x0i));
-                cr[r1] = fma(-l1r, ur, fma(l1i, ui, x1r));
-                ci[r1] = fma(-l1r, ui, fma(-l1i, ur, x1i));
-                if (!mb) break;
-                const bool ma = j + 2 * NW < N;                       // ... and one for set A again?
-                c = d + (ma ? stride : 0); cr = dr + (ma ? stride : 0); ci = di + (ma ? stride : 0);
-                u = c[pa]; x0 = c[r0]; x1 = c[r1];
-                ur = cr[pc]; ui = ci[pc]; x0r = cr[r0]; x0i = ci[r0]; x1r = cr[r1]; x1i = ci[r1];
-                d[r0] = fma(-l0, v, y0);
-                d[r1] = fma(-l1, v, y1);
-                dr[r0] = fma(-l0r, vr, fma(l0i, vi, y0r));
-                di[r0] = fma(-l0r, vi, fma(-l0i, vr, y0i));
-                dr[r1] = fma(-l1r, vr, fma(l1i, vi, y1r));
-                di[r1] = fma(-l1r, vi, fma(-l1i, vr, y1i));
-                if (!ma) break;
-                j += 2 * NW;
+            for (int j = j0; j < N; j += NW, c += NW * LD, cr += NW * LD, ci += NW * LD) {
+                const double u = c[pa], v = c[pa2], x0 = c[r0], x1 = c[r1];
+                const double ur = cr[pc], ui = ci[pc], vr = cr[pc2], vi = ci[pc2];
+                const double x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
+                const double v2 = fma(-tl, u, v);
+                const double v2r = fma(-tlr, ur, fma(tli, ui, vr)), v2i = fma(-tlr, ui, fma(-tli, ur, vi));
+                c[r0] = fma(-m0, v2, fma(-l0, u, x0));
+                c[r1] = fma(-m1, v2, fma(-l1, u, x1));
+                const double t0r = fma(-l0r, ur, fma(l0i, ui, x0r)), t0i = fma(-l0r, ui, fma(-l0i, ur, x0i));
+                const double t1r = fma(-l1r, ur, fma(l1i, ui, x1r)), t1i = fma(-l1r, ui, fma(-l1i, ur, x1i));
+                cr[r0] = fma(-m0r, v2r, fma(m0i, v2i, t0r));
+                ci[r0] = fma(-m0r, v2i, fma(-m0i, v2r, t0i));
+                cr[r1] = fma(-m1r, v2r, fma(m1i, v2i, t1r));
+                ci[r1] = fma(-m1r, v2i, fma(-m1i, v2r, t1i));
             }
         }
         Grp<G>::sync();
     }
+    write_back((N - 1) & ~1);
+    Grp<G>::sync();
     // Epilogue: rows into pivot order (storage row k <- pivot row of step k) and every row of U scaled by 1 / U_kk, so
     // that a solve is two sweeps whose only chain is shuffle -> fused multiply-add: no pivot look-ups, no selects and
     // no reciprocal on the chain (solve3_*).  Column by column inside the warp that owns the column: all loads, then
