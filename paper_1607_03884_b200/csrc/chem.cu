@@ -220,6 +220,60 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
         }
     }
     for (size_t e = 0; e < inc_rx.size(); e++) { inc2.push_back(inc_rx[e]); inc2.push_back((int)inc_nu[e]); }
+    // ---- balanced row gather of the analytical Jacobian (jacobian<128>, chem_device.cuh): the same kind of schedule for
+    // as many threads as private rows of N + 3 doubles fit into the matrix storage that is dead during the Jacobian
+    // (E1 and the part of the E2 region in front of the slot derivatives: work_doubles / carve, chem_radau.cuh), and one
+    // packed record per incidence
+    std::vector<int> gatj(4, 0), jinc(8, 0);
+    int gatj_T = 0;
+    if (ns > 32 && ns <= 128) {
+        const size_t e2 = (size_t)2 * ns * (ns + 1) > (size_t)8 * nr ? (size_t)2 * ns * (ns + 1) : (size_t)8 * nr;
+        const size_t pool = (size_t)ns * (ns + 1) + e2 - (size_t)8 * nr;
+        int T = (int)std::min<size_t>(128, pool / (ns + 3));
+        if (T >= ns) {
+            auto groups = [&](int target, std::vector<int> *lg) {
+                int tot = 0;
+                for (int k = 0; k < ns; k++) {
+                    const int len = inc_ptr[k + 1] - inc_ptr[k], need = (len + target - 1) / target;
+                    int m2 = 0;
+                    while ((1 << m2) < need && m2 < 5) m2++;
+                    if (lg) (*lg)[k] = m2;
+                    tot += 1 << m2;
+                }
+                return tot;
+            };
+            int target = 1;
+            while (groups(target, nullptr) > T) target++;
+            std::vector<int> lg(ns, 0), ord(ns);
+            groups(target, &lg);
+            for (int k = 0; k < ns; k++) ord[k] = k;
+            std::stable_sort(ord.begin(), ord.end(), [&](int a, int b2) { return lg[a] > lg[b2]; });   // big groups first: aligned starts
+            gatj.assign(4 * T, 0);
+            for (int t2 = 0; t2 < T; t2++) gatj[4 * t2] = -1;
+            int t2 = 0;
+            for (int k : ord) {
+                const int c = 1 << lg[k], len = inc_ptr[k + 1] - inc_ptr[k];
+                for (int j = 0; j < c; j++, t2++) {
+                    gatj[4 * t2] = k;
+                    gatj[4 * t2 + 1] = inc_ptr[k] + (int)((long long)len * j / c);
+                    gatj[4 * t2 + 2] = inc_ptr[k] + (int)((long long)len * (j + 1) / c);
+                    gatj[4 * t2 + 3] = lg[k];
+                }
+            }
+            gatj_T = T;
+            jinc.assign(8 * std::max<size_t>(inc_rx.size(), 1), 0);
+            for (size_t e = 0; e < inc_rx.size(); e++) {
+                const int i = inc_rx[e];
+                jinc[8 * e] = i;
+                jinc[8 * e + 1] = (int)inc_nu[e];
+                jinc[8 * e + 2] = slot_sp[i] | (slot_sp[nr + i] << 8) | (slot_sp[2 * nr + i] << 16);
+                jinc[8 * e + 3] = slot_sp[3 * nr + i] | (slot_sp[4 * nr + i] << 8) | (slot_sp[5 * nr + i] << 16);
+                jinc[8 * e + 4] = rtype[i] != 0 ? eff_ptr[i] : 0;
+                jinc[8 * e + 5] = rtype[i] != 0 ? eff_ptr[i + 1] : 0;
+                jinc[8 * e + 6] = rtype[i] != 0;
+            }
+        }
+    }
     if (eff_sp.empty()) { eff_sp.push_back(0); eff_dv.push_back(0.0); }
     if (inc_rx.empty()) { inc_rx.push_back(0); inc_nu.push_back(0.0); }
     if (inc2.empty()) { inc2.push_back(0); inc2.push_back(0); }
@@ -320,7 +374,7 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     add(rtype.data(), nr * 4); add(slot_sp.data(), 6 * nr * 4); add(slot_nu.data(), 6 * nr * 4);
     add(eff_ptr.data(), (nr + 1) * 4); add(eff_sp.data(), eff_sp.size() * 4);
     add(inc_ptr.data(), (ns + 1) * 4); add(inc_rx.data(), inc_rx.size() * 4); add(rdesc.data(), rdesc.size() * 4);
-    add(gat.data(), gat.size() * 4); add(inc2.data(), inc2.size() * 4);
+    add(gat.data(), gat.size() * 4); add(inc2.data(), inc2.size() * 4); add(gatj.data(), gatj.size() * 4); add(jinc.data(), jinc.size() * 4);
     std::vector<char> host(total, 0);
     for (size_t a = 0; a < parts.size(); a++) std::memcpy(host.data() + offs[a], parts[a].first, parts[a].second);
 
@@ -349,6 +403,7 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     t.eff_dv = D(); t.inc_nu = D(); t.job_lo = D(); t.job_hi = D();
     t.rtype = I(); t.slot_sp = I(); t.slot_nu = I(); t.eff_ptr = I(); t.eff_sp = I(); t.inc_ptr = I(); t.inc_rx = I(); t.rdesc = I();
     t.gat = reinterpret_cast<const int4 *>(I()); t.inc2 = reinterpret_cast<const int2 *>(I()); t.gat_steps = gat_steps; t.n_solo = n_solo;
+    t.gatj = reinterpret_cast<const int4 *>(I()); t.jinc = reinterpret_cast<const int4 *>(I()); t.gatj_T = gatj_T;
     t.n_jobs = n_jobs; t.n_fo = n_fo; t.tmid0 = tmid[0];
     m->n_sm = n_sm;
     m->max_smem_optin = optin;

@@ -47,6 +47,11 @@ struct Tables {
     const int2 *inc2;
     int gat_steps;
     int n_solo;                       // threads t < n_solo evaluate table reaction t only (chem.cu)
+    // balanced row gather of the analytical Jacobian (jacobian<128>): schedule like `gat` for gatj_T threads (0: none),
+    // jinc = two int4 per incidence: (reaction, net coefficient, slot species 0-2, slot species 3-5), (eff_lo, eff_hi, has [M], 0)
+    const int4 *gatj;
+    const int4 *jinc;
+    int gatj_T;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -112,13 +117,14 @@ struct ChemScratch {
     double *dq;                               // [6][n_rx]   (Jacobian only)
     double *dqdT, *tb;                        // [n_rx]      (Jacobian only)
     double *red;                              // [2*NW]
+    double *jpool;                            // private rows of the balanced Jacobian gather (dead matrix storage)
 };
 
 __device__ __forceinline__ ChemScratch shp(const ChemScratch &g)
 {
     ChemScratch s;
     s.C = shp(g.C); s.g = shp(g.g); s.hRT = shp(g.hRT); s.cpR = shp(g.cpR); s.dcpR = shp(g.dcpR); s.wdot = shp(g.wdot);
-    s.q = shp(g.q); s.dq = shp(g.dq); s.dqdT = shp(g.dqdT); s.tb = shp(g.tb); s.red = shp(g.red);
+    s.q = shp(g.q); s.dq = shp(g.dq); s.dqdT = shp(g.dqdT); s.tb = shp(g.tb); s.red = shp(g.red); s.jpool = g.jpool ? shp(g.jpool) : nullptr;
     return s;
 }
 
@@ -307,24 +313,77 @@ __device__ __noinline__ void jacobian(const Tables &tg, const ChemScratch &sg, d
     for (int i = lane; i < NR; i += (lane < t.n_solo ? NR : G - t.n_solo)) s.q[i] = reaction<true>(t, i, T, lnT, invT, lnPRT, Ctot, s);
     Grp<G>::sync();
     const double invWN = __ldg(&t.invW[N - 1]);
-    // rows: species k -> Dw[k][j] = d wdot_k / d y_j, stored in Jm row k
+    // rows: species k -> Dw[k][j] = d wdot_k / d y_j, stored in Jm row k.
+    // Balanced gather (CTA groups): a few radicals take part in a third of the reactions, and one thread per species
+    // left the group waiting for the longest incidence list.  Species k gets 2^m adjacent threads (schedule from the
+    // mechanism compiler), each accumulates its share of the list in a private row of N + 3 doubles (row, wdot,
+    // d wdot/dT at constant C, third-body sum) in matrix storage that is dead while the Jacobian is evaluated, and the
+    // shares are added in a fixed order (deterministic).  One packed record per incidence: one trip to L2.
+    const bool balanced = G == 128 && t.gatj_T > 0 && s.jpool != nullptr;
+    if (balanced) {
+        const int RS = N + 3;
+        int4 g = make_int4(-1, 0, 0, 0);
+        if (lane < t.gatj_T) g = __ldg(t.gatj + lane);
+        double *row = s.jpool + lane * RS;
+        if (g.x >= 0) {
+            for (int l = 0; l < RS; l++) row[l] = 0.0;
+            double wd = 0.0, dwT = 0.0, u = 0.0;
+#pragma unroll 2
+            for (int p = g.y; p < g.z; p++) {
+                const int4 e0 = __ldg(t.jinc + 2 * p), e1 = __ldg(t.jinc + 2 * p + 1);
+                const int i = e0.x;
+                const double nu = (double)e0.y;
+                wd += nu * s.q[i];
+                dwT += nu * s.dqdT[i];
+                row[e0.z & 255] += nu * s.dq[i];
+                row[(e0.z >> 8) & 255] += nu * s.dq[NR + i];
+                row[(e0.z >> 16) & 255] += nu * s.dq[2 * NR + i];
+                row[e0.w & 255] += nu * s.dq[3 * NR + i];
+                row[(e0.w >> 8) & 255] += nu * s.dq[4 * NR + i];
+                row[(e0.w >> 16) & 255] += nu * s.dq[5 * NR + i];
+                if (e1.z) {
+                    const double v = nu * s.tb[i];
+                    u += v;
+                    for (int pe = e1.x; pe < e1.y; pe++) row[__ldg(&t.eff_sp[pe])] += v * __ldg(&t.eff_dv[pe]);
+                }
+            }
+            row[N] = wd; row[N + 1] = dwT; row[N + 2] = u;
+        }
+        Grp<G>::sync();
+        if (g.x >= 0) {
+            const int c = 1 << g.w, qi = lane & (c - 1);      // groups are aligned to their (power of two) size
+            const double *first = s.jpool + (lane - qi) * RS;
+            for (int l = qi; l < RS; l += c) {
+                double sum = 0.0;
+                for (int m = 0; m < c; m++) sum += first[m * RS + l];
+                if (l < N) Jm[g.x * N + l] = sum;
+                else if (l == N) s.wdot[g.x] = sum;
+                else s.dq[(l - N - 1) * N + g.x] = sum;       // dq is dead by now: [0,N) d wdot/dT, [N,2N) third-body sums
+            }
+        }
+        Grp<G>::sync();
+    }
     double hw = 0.0, ccp = 0.0, cpw = 0.0, cdcp = 0.0;
     for (int k = lane; k < N; k += G) {
         double *row = Jm + k * N;
-        for (int l = 0; l < N; l++) row[l] = 0.0;
         double wd = 0.0, dwT = 0.0, u = 0.0;
-        for (int p = __ldg(&t.inc_ptr[k]); p < __ldg(&t.inc_ptr[k + 1]); p++) {
-            const int i = __ldg(&t.inc_rx[p]);
-            const double nu = __ldg(&t.inc_nu[p]);
-            wd += nu * s.q[i];
-            dwT += nu * s.dqdT[i];
+        if (balanced) {
+            wd = s.wdot[k]; dwT = s.dq[k]; u = s.dq[N + k];
+        } else {
+            for (int l = 0; l < N; l++) row[l] = 0.0;
+            for (int p = __ldg(&t.inc_ptr[k]); p < __ldg(&t.inc_ptr[k + 1]); p++) {
+                const int i = __ldg(&t.inc_rx[p]);
+                const double nu = __ldg(&t.inc_nu[p]);
+                wd += nu * s.q[i];
+                dwT += nu * s.dqdT[i];
 #pragma unroll
-            for (int sl = 0; sl < kSlots; sl++) row[__ldg(&t.slot_sp[sl * NR + i])] += nu * s.dq[sl * NR + i];
-            if (__ldg(&t.rtype[i]) != 0) {
-                const double v = nu * s.tb[i];
-                u += v;
-                for (int pe = __ldg(&t.eff_ptr[i]); pe < __ldg(&t.eff_ptr[i + 1]); pe++)
-                    row[__ldg(&t.eff_sp[pe])] += v * __ldg(&t.eff_dv[pe]);
+                for (int sl = 0; sl < kSlots; sl++) row[__ldg(&t.slot_sp[sl * NR + i])] += nu * s.dq[sl * NR + i];
+                if (__ldg(&t.rtype[i]) != 0) {
+                    const double v = nu * s.tb[i];
+                    u += v;
+                    for (int pe = __ldg(&t.eff_ptr[i]); pe < __ldg(&t.eff_ptr[i + 1]); pe++)
+                        row[__ldg(&t.eff_sp[pe])] += v * __ldg(&t.eff_dv[pe]);
+                }
             }
         }
         double GC = 0.0;

@@ -65,7 +65,11 @@ __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW, int n
     const size_t e2 = (size_t)2 * N * (N + 1) > (size_t)8 * NR ? (size_t)2 * N * (N + 1) : (size_t)8 * NR;
     double *r = take(e2);
     w.E2r = r; w.E2i = r + (size_t)N * (N + 1);
-    w.cs.dq = r; w.cs.dqdT = r + (size_t)6 * NR; w.cs.tb = r + (size_t)7 * NR;   // alive only inside jacobian()
+    // alive only inside jacobian(): slot derivatives at the END of the E2 region, and in front of them E1 + the rest of
+    // E2 as one pool of private rows for the balanced gather
+    double *jq = r + (e2 - (size_t)8 * NR);
+    w.cs.dq = jq; w.cs.dqdT = jq + (size_t)6 * NR; w.cs.tb = jq + (size_t)7 * NR;
+    w.cs.jpool = w.E1;
     w.cs.red = take(2 * NW);
     w.ip1 = reinterpret_cast<int *>(take(N + 2));                  // 2 N ints
     w.ip2 = w.ip1 + N;
