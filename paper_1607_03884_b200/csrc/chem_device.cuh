@@ -757,34 +757,46 @@ __device__ __forceinline__ void solve3_real_warp(int N, int LD, const double *A,
     double b0 = g0 ? b[x.perm[i0]] : 0.0, b1 = g1 ? b[x.perm[i1]] : 0.0;
     const double rd0 = g0 ? x.rdr[i0] : 0.0, rd1 = g1 ? x.rdr[i1] : 0.0;
     const int K1 = N - 1 < 32 ? N - 1 : 32;
+    // the matrix entries of the NEXT step are requested before the broadcast of this one (unconditional loads: the
+    // other triangle and the dummy row are valid memory), so that only shuffle -> fused multiply-add is on the chain
     const double *a0 = A + r0, *a1 = A + r1;
+    double n0 = *a0, n1 = *a1;
     int k = 0;
-#pragma unroll 4
-    for (; k < K1; k++, a0 += LD, a1 += LD) {
-        const double l0 = (i0 > k) ? *a0 : 0.0, l1 = g1 ? *a1 : 0.0;
+#pragma unroll 2
+    for (; k < K1; k++) {
+        const double l0 = (i0 > k) ? n0 : 0.0, l1 = g1 ? n1 : 0.0;
+        a0 += LD; a1 += LD;
+        n0 = *a0; n1 = *a1;
         const double bk = __shfl_sync(0xffffffffu, b0, k);
         b0 = fma(-l0, bk, b0);
         b1 = fma(-l1, bk, b1);
     }
-#pragma unroll 4
-    for (; k < N - 1; k++, a1 += LD) {
-        const double l1 = (g1 && i1 > k) ? *a1 : 0.0;
+#pragma unroll 2
+    for (; k < N - 1; k++) {
+        const double l1 = (g1 && i1 > k) ? n1 : 0.0;
+        a1 += LD;
+        n1 = *a1;
         const double bk = __shfl_sync(0xffffffffu, b1, k - 32);
         b1 = fma(-l1, bk, b1);
     }
     b0 *= rd0; b1 *= rd1;
     k = N - 1;
     a0 = A + r0 + k * LD; a1 = A + r1 + k * LD;
-#pragma unroll 4
-    for (; k >= 32; k--, a0 -= LD, a1 -= LD) {
-        const double u0 = *a0, u1 = (i1 < k) ? *a1 : 0.0;
+    n0 = *a0; n1 = *a1;
+#pragma unroll 2
+    for (; k >= 32; k--) {
+        const double u0 = n0, u1 = (i1 < k) ? n1 : 0.0;
+        a0 -= LD; a1 -= LD;
+        n0 = *a0; n1 = *a1;
         const double xk = __shfl_sync(0xffffffffu, b1, k - 32);
         b0 = fma(-u0, xk, b0);
         b1 = fma(-u1, xk, b1);
     }
-#pragma unroll 4
-    for (; k >= 1; k--, a0 -= LD) {
-        const double u0 = (i0 < k) ? *a0 : 0.0;
+#pragma unroll 2
+    for (; k >= 1; k--) {
+        const double u0 = (i0 < k) ? n0 : 0.0;
+        a0 -= LD;
+        n0 = *a0;
         const double xk = __shfl_sync(0xffffffffu, b0, k);
         b0 = fma(-u0, xk, b0);
     }
@@ -804,11 +816,14 @@ __device__ __forceinline__ void solve3_complex_warp(int N, int LD, const double 
     const double q0r = g0 ? x.rdr[i0] : 0.0, q0i = g0 ? x.rdi[i0] : 0.0, q1r = g1 ? x.rdr[i1] : 0.0, q1i = g1 ? x.rdi[i1] : 0.0;
     const int K1 = N - 1 < 32 ? N - 1 : 32;
     int o0 = r0, o1 = r1;
+    double n0r = Ar[o0], n0i = Ai[o0], n1r = Ar[o1], n1i = Ai[o1];      // entries of the next step, requested early
     int k = 0;
 #pragma unroll 2
-    for (; k < K1; k++, o0 += LD, o1 += LD) {
+    for (; k < K1; k++) {
         const bool m0 = i0 > k;
-        const double l0r = m0 ? Ar[o0] : 0.0, l0i = m0 ? Ai[o0] : 0.0, l1r = g1 ? Ar[o1] : 0.0, l1i = g1 ? Ai[o1] : 0.0;
+        const double l0r = m0 ? n0r : 0.0, l0i = m0 ? n0i : 0.0, l1r = g1 ? n1r : 0.0, l1i = g1 ? n1i : 0.0;
+        o0 += LD; o1 += LD;
+        n0r = Ar[o0]; n0i = Ai[o0]; n1r = Ar[o1]; n1i = Ai[o1];
         const double xr = __shfl_sync(0xffffffffu, b0r, k), xi = __shfl_sync(0xffffffffu, b0i, k);
         b0r = fma(-l0r, xr, fma(l0i, xi, b0r));
         b0i = fma(-l0r, xi, fma(-l0i, xr, b0i));
@@ -816,9 +831,11 @@ __device__ __forceinline__ void solve3_complex_warp(int N, int LD, const double 
         b1i = fma(-l1r, xi, fma(-l1i, xr, b1i));
     }
 #pragma unroll 2
-    for (; k < N - 1; k++, o1 += LD) {
+    for (; k < N - 1; k++) {
         const bool m1 = g1 && i1 > k;
-        const double l1r = m1 ? Ar[o1] : 0.0, l1i = m1 ? Ai[o1] : 0.0;
+        const double l1r = m1 ? n1r : 0.0, l1i = m1 ? n1i : 0.0;
+        o1 += LD;
+        n1r = Ar[o1]; n1i = Ai[o1];
         const double xr = __shfl_sync(0xffffffffu, b1r, k - 32), xi = __shfl_sync(0xffffffffu, b1i, k - 32);
         b1r = fma(-l1r, xr, fma(l1i, xi, b1r));
         b1i = fma(-l1r, xi, fma(-l1i, xr, b1i));
@@ -827,10 +844,13 @@ __device__ __forceinline__ void solve3_complex_warp(int N, int LD, const double 
     { const double t = b1r * q1r - b1i * q1i; b1i = b1r * q1i + b1i * q1r; b1r = t; }
     k = N - 1;
     o0 = r0 + k * LD; o1 = r1 + k * LD;
+    n0r = Ar[o0]; n0i = Ai[o0]; n1r = Ar[o1]; n1i = Ai[o1];
 #pragma unroll 2
-    for (; k >= 32; k--, o0 -= LD, o1 -= LD) {
+    for (; k >= 32; k--) {
         const bool m1 = i1 < k;
-        const double u0r = Ar[o0], u0i = Ai[o0], u1r = m1 ? Ar[o1] : 0.0, u1i = m1 ? Ai[o1] : 0.0;
+        const double u0r = n0r, u0i = n0i, u1r = m1 ? n1r : 0.0, u1i = m1 ? n1i : 0.0;
+        o0 -= LD; o1 -= LD;
+        n0r = Ar[o0]; n0i = Ai[o0]; n1r = Ar[o1]; n1i = Ai[o1];
         const double xr = __shfl_sync(0xffffffffu, b1r, k - 32), xi = __shfl_sync(0xffffffffu, b1i, k - 32);
         b0r = fma(-u0r, xr, fma(u0i, xi, b0r));
         b0i = fma(-u0r, xi, fma(-u0i, xr, b0i));
@@ -838,9 +858,11 @@ __device__ __forceinline__ void solve3_complex_warp(int N, int LD, const double 
         b1i = fma(-u1r, xi, fma(-u1i, xr, b1i));
     }
 #pragma unroll 2
-    for (; k >= 1; k--, o0 -= LD) {
+    for (; k >= 1; k--) {
         const bool m0 = i0 < k;
-        const double u0r = m0 ? Ar[o0] : 0.0, u0i = m0 ? Ai[o0] : 0.0;
+        const double u0r = m0 ? n0r : 0.0, u0i = m0 ? n0i : 0.0;
+        o0 -= LD;
+        n0r = Ar[o0]; n0i = Ai[o0];
         const double xr = __shfl_sync(0xffffffffu, b0r, k), xi = __shfl_sync(0xffffffffu, b0i, k);
         b0r = fma(-u0r, xr, fma(u0i, xi, b0r));
         b0i = fma(-u0r, xi, fma(-u0i, xr, b0i));
