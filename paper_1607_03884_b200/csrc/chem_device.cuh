@@ -745,6 +745,203 @@ __device__ __noinline__ int lu2_pair(int N, int LD, double *A, const Lu2Aux &xag
     return 0;
 }
 
+// ---- warp-specialised form of lu2_pair for a CTA of four warps: warp 0 factors the real matrix alone, warps 1-3 the
+// complex one (four times the arithmetic, columns j = w (mod 3)).  In lu2_pair every warp repeats BOTH pivot chains
+// (~240 instructions per elimination step, more than the trailing update); here a warp runs the chain of one matrix
+// only, the two factorisations never wait for each other (the complex warps meet at a named barrier, the real warp only
+// synchronises with itself), and the shared-memory traffic of the trailing updates splits about evenly (real: all
+// columns x 10 wavefronts per sweep, complex: a third of the columns x 20 per warp).  Same two-steps-per-sweep
+// arithmetic, pivots, result layout and return value as lu2_pair.
+__device__ __forceinline__ int lu2_real_warp(int N, int LD, double *A, const Lu2Aux &xa, int wl)
+{
+    const int i0 = wl, i1 = wl + 32;
+    const bool g0 = i0 < N, g1 = i1 < N;
+    const int r0 = g0 ? i0 : N, r1 = g1 ? i1 : N;                     // storage rows (N = dummy)
+    int ka0 = g0 ? -1 : 1 << 30, ka1 = g1 ? -1 : 1 << 30;
+    for (int k = 0; k < N; k += 2) {
+        const double a0 = (ka0 < 0) ? A[i0 + k * LD] : 0.0, a1 = (ka1 < 0) ? A[i1 + k * LD] : 0.0;
+        const double va0 = (ka0 < 0) ? fabs(a0) : -1.0, va1 = (ka1 < 0) ? fabs(a1) : -1.0;
+        const int pa = warp_argmax_row(va1 > va0 ? va1 : va0, va1 > va0 ? i1 : i0);
+        const double pv = (pa >= 0) ? A[pa + k * LD] : 0.0;
+        const double rp = rcp_nr(pv);
+        if (pa < 0 || !isfinite(pv)) return k + 1;
+        if (i0 == pa) ka0 = k;
+        if (i1 == pa) ka1 = k;
+        if (wl == 0) { xa.perm[k] = pa; xa.rdr[k] = rp; xa.rowk[pa] = k; }
+        const double l0 = (ka0 < 0) ? a0 * rp : 0.0, l1 = (ka1 < 0) ? a1 * rp : 0.0;
+        // a lane only ever reads its own entries of a pivot column and the pivot entry, which its owner leaves alone:
+        // the multipliers can be stored at once
+        if (ka0 < 0) A[i0 + k * LD] = l0;
+        if (ka1 < 0) A[i1 + k * LD] = l1;
+        if (k + 1 < N) {
+            const int kk = k + 1;
+            const double uk = A[pa + kk * LD];
+            const double y0 = (ka0 < 0) ? fma(-l0, uk, A[i0 + kk * LD]) : 0.0, y1 = (ka1 < 0) ? fma(-l1, uk, A[i1 + kk * LD]) : 0.0;
+            const double ya0 = (ka0 < 0) ? fabs(y0) : -1.0, ya1 = (ka1 < 0) ? fabs(y1) : -1.0;
+            const int pa2 = warp_argmax_row(ya1 > ya0 ? ya1 : ya0, ya1 > ya0 ? i1 : i0);
+            const int sa = pa2 < 0 ? 0 : pa2;
+            const double pv2 = __shfl_sync(0xffffffffu, (sa & 32) ? y1 : y0, sa & 31);
+            const double tl = __shfl_sync(0xffffffffu, (sa & 32) ? l1 : l0, sa & 31);
+            const double rp2 = rcp_nr(pv2);
+            if (pa2 < 0 || !isfinite(pv2)) return kk + 1;
+            if (i0 == pa2) ka0 = kk;
+            if (i1 == pa2) ka1 = kk;
+            if (wl == 0) { xa.perm[kk] = pa2; xa.rdr[kk] = rp2; xa.rowk[pa2] = kk; }
+            const double m0 = (ka0 < 0) ? y0 * rp2 : 0.0, m1 = (ka1 < 0) ? y1 * rp2 : 0.0;
+            if (ka0 < 0) A[i0 + kk * LD] = m0; else if (ka0 == kk) A[i0 + kk * LD] = y0;
+            if (ka1 < 0) A[i1 + kk * LD] = m1; else if (ka1 == kk) A[i1 + kk * LD] = y1;
+            // four columns per trip (one warp, nothing else to hide the shared-memory round trip): all loads, then all
+            // stores; a trip that runs past the last column repeats it (same values stored twice)
+            double *c = A + (k + 2) * LD;
+#pragma unroll 1
+            for (int j = k + 2; j < N; j += 4, c += 4 * LD) {
+                double *cB = c + (j + 1 < N ? LD : 0), *cC = c + (j + 2 < N ? 2 * LD : 0), *cD = c + (j + 3 < N ? 3 * LD : 0);
+                const double uA = c[pa], vA = c[pa2], xA0 = c[r0], xA1 = c[r1];
+                const double uB = cB[pa], vB = cB[pa2], xB0 = cB[r0], xB1 = cB[r1];
+                const double uC = cC[pa], vC = cC[pa2], xC0 = cC[r0], xC1 = cC[r1];
+                const double uD = cD[pa], vD = cD[pa2], xD0 = cD[r0], xD1 = cD[r1];
+                const double wA = fma(-tl, uA, vA), wB = fma(-tl, uB, vB), wC = fma(-tl, uC, vC), wD = fma(-tl, uD, vD);
+                __syncwarp();                                         // every lane has read the pivot rows
+                c[r0] = fma(-m0, wA, fma(-l0, uA, xA0));
+                c[r1] = fma(-m1, wA, fma(-l1, uA, xA1));
+                cB[r0] = fma(-m0, wB, fma(-l0, uB, xB0));
+                cB[r1] = fma(-m1, wB, fma(-l1, uB, xB1));
+                cC[r0] = fma(-m0, wC, fma(-l0, uC, xC0));
+                cC[r1] = fma(-m1, wC, fma(-l1, uC, xC1));
+                cD[r0] = fma(-m0, wD, fma(-l0, uD, xD0));
+                cD[r1] = fma(-m1, wD, fma(-l1, uD, xD1));
+            }
+        }
+        __syncwarp();
+    }
+    // rows into pivot order, U scaled by 1 / U_kk (see lu2_pair)
+    const int p0 = g0 ? xa.perm[i0] : N, p1 = g1 ? xa.perm[i1] : N;
+    const double rd0 = g0 ? xa.rdr[i0] : 0.0, rd1 = g1 ? xa.rdr[i1] : 0.0;
+#pragma unroll 2
+    for (int j = 0; j < N; j++) {
+        double *c = A + j * LD;
+        double v0 = c[p0], v1 = c[p1];
+        if (j > i0) v0 *= rd0;
+        if (j > i1) v1 *= rd1;
+        __syncwarp();
+        if (g0) c[i0] = v0;
+        if (g1) c[i1] = v1;
+    }
+    return 0;
+}
+
+// NWc warps (wq = 0 .. NWc-1) on the complex matrix; they meet at named barrier 1
+__device__ __forceinline__ int lu2_complex_warps(int N, int LD, double *Ar, double *Ai, const Lu2Aux &xc, int wl, int wq, int NWc)
+{
+    auto bar = [&]() { asm volatile("bar.sync 1, %0;" ::"r"(NWc * 32) : "memory"); };
+    const int i0 = wl, i1 = wl + 32;
+    const bool g0 = i0 < N, g1 = i1 < N;
+    const int r0 = g0 ? i0 : N, r1 = g1 ? i1 : N;
+    int kc0 = g0 ? -1 : 1 << 30, kc1 = g1 ? -1 : 1 << 30;
+    double l0r = 0.0, l0i = 0.0, l1r = 0.0, l1i = 0.0, w0r = 0.0, w0i = 0.0, w1r = 0.0, w1i = 0.0;
+    auto open_after = [](int kx, int k) { return kx < 0 || (kx > k && kx < (1 << 30)); };
+    auto write_back = [&](int k) {       // columns k, k + 1 of the sweep that started at step k (owner warps, one sweep late)
+        const bool f0 = open_after(kc0, k), f1 = open_after(kc1, k);
+        if (wq == k % NWc) {
+            if (f0) { Ar[i0 + k * LD] = l0r; Ai[i0 + k * LD] = l0i; }
+            if (f1) { Ar[i1 + k * LD] = l1r; Ai[i1 + k * LD] = l1i; }
+        }
+        if (k + 1 < N && wq == (k + 1) % NWc) {
+            if (f0) { Ar[i0 + (k + 1) * LD] = w0r; Ai[i0 + (k + 1) * LD] = w0i; }
+            if (f1) { Ar[i1 + (k + 1) * LD] = w1r; Ai[i1 + (k + 1) * LD] = w1i; }
+        }
+    };
+    for (int k = 0; k < N; k += 2) {
+        const double a0r = (kc0 < 0) ? Ar[i0 + k * LD] : 0.0, a0i = (kc0 < 0) ? Ai[i0 + k * LD] : 0.0;
+        const double a1r = (kc1 < 0) ? Ar[i1 + k * LD] : 0.0, a1i = (kc1 < 0) ? Ai[i1 + k * LD] : 0.0;
+        const double vc0 = (kc0 < 0) ? fabs(a0r) + fabs(a0i) : -1.0, vc1 = (kc1 < 0) ? fabs(a1r) + fabs(a1i) : -1.0;
+        const int pc = warp_argmax_row(vc1 > vc0 ? vc1 : vc0, vc1 > vc0 ? i1 : i0);
+        const double pr = (pc >= 0) ? Ar[pc + k * LD] : 0.0, pi = (pc >= 0) ? Ai[pc + k * LD] : 0.0;
+        const double den = rcp_nr(pr * pr + pi * pi);
+        if (pc < 0 || !isfinite(den)) return k + 1;
+        const double qr = pr * den, qi = -pi * den;                   // 1 / pivot
+        if (i0 == pc) kc0 = k;
+        if (i1 == pc) kc1 = k;
+        if (wq == 0 && wl == 0) { xc.perm[k] = pc; xc.rdr[k] = qr; xc.rdi[k] = qi; xc.rowk[pc] = k; }
+        if (k > 0) write_back(k - 2);
+        l0r = (kc0 < 0) ? a0r * qr - a0i * qi : 0.0; l0i = (kc0 < 0) ? a0r * qi + a0i * qr : 0.0;
+        l1r = (kc1 < 0) ? a1r * qr - a1i * qi : 0.0; l1i = (kc1 < 0) ? a1r * qi + a1i * qr : 0.0;
+        if (k + 1 < N) {
+            const int kk = k + 1;
+            const double ukr = Ar[pc + kk * LD], uki = Ai[pc + kk * LD];
+            double y0r = 0.0, y0i = 0.0, y1r = 0.0, y1i = 0.0;
+            if (kc0 < 0) {
+                const double xr = Ar[i0 + kk * LD], xi = Ai[i0 + kk * LD];
+                y0r = fma(-l0r, ukr, fma(l0i, uki, xr)); y0i = fma(-l0r, uki, fma(-l0i, ukr, xi));
+            }
+            if (kc1 < 0) {
+                const double xr = Ar[i1 + kk * LD], xi = Ai[i1 + kk * LD];
+                y1r = fma(-l1r, ukr, fma(l1i, uki, xr)); y1i = fma(-l1r, uki, fma(-l1i, ukr, xi));
+            }
+            const double yc0 = (kc0 < 0) ? fabs(y0r) + fabs(y0i) : -1.0, yc1 = (kc1 < 0) ? fabs(y1r) + fabs(y1i) : -1.0;
+            const int pc2 = warp_argmax_row(yc1 > yc0 ? yc1 : yc0, yc1 > yc0 ? i1 : i0);
+            const int sc = pc2 < 0 ? 0 : pc2;
+            const double pr2 = __shfl_sync(0xffffffffu, (sc & 32) ? y1r : y0r, sc & 31);
+            const double pi2 = __shfl_sync(0xffffffffu, (sc & 32) ? y1i : y0i, sc & 31);
+            const double tlr = __shfl_sync(0xffffffffu, (sc & 32) ? l1r : l0r, sc & 31);
+            const double tli = __shfl_sync(0xffffffffu, (sc & 32) ? l1i : l0i, sc & 31);
+            const double den2 = rcp_nr(pr2 * pr2 + pi2 * pi2);
+            if (pc2 < 0 || !isfinite(den2)) return kk + 1;
+            const double qr2 = pr2 * den2, qi2 = -pi2 * den2;
+            if (i0 == pc2) kc0 = kk;
+            if (i1 == pc2) kc1 = kk;
+            if (wq == 0 && wl == 0) { xc.perm[kk] = pc2; xc.rdr[kk] = qr2; xc.rdi[kk] = qi2; xc.rowk[pc2] = kk; }
+            const double m0r = (kc0 < 0) ? y0r * qr2 - y0i * qi2 : 0.0, m0i = (kc0 < 0) ? y0r * qi2 + y0i * qr2 : 0.0;
+            const double m1r = (kc1 < 0) ? y1r * qr2 - y1i * qi2 : 0.0, m1i = (kc1 < 0) ? y1r * qi2 + y1i * qr2 : 0.0;
+            w0r = (kc0 == kk) ? y0r : m0r; w0i = (kc0 == kk) ? y0i : m0i;
+            w1r = (kc1 == kk) ? y1r : m1r; w1i = (kc1 == kk) ? y1i : m1i;
+            const int j0 = k + 2 + ((wq - (k + 2)) % NWc + NWc) % NWc;
+            double *cr = Ar + j0 * LD, *ci = Ai + j0 * LD;
+#pragma unroll 1
+            for (int j = j0; j < N; j += NWc, cr += NWc * LD, ci += NWc * LD) {
+                const double ur = cr[pc], ui = ci[pc], vr = cr[pc2], vi = ci[pc2];
+                const double x0r = cr[r0], x0i = ci[r0], x1r = cr[r1], x1i = ci[r1];
+                const double v2r = fma(-tlr, ur, fma(tli, ui, vr)), v2i = fma(-tlr, ui, fma(-tli, ur, vi));
+                const double t0r = fma(-l0r, ur, fma(l0i, ui, x0r)), t0i = fma(-l0r, ui, fma(-l0i, ur, x0i));
+                const double t1r = fma(-l1r, ur, fma(l1i, ui, x1r)), t1i = fma(-l1r, ui, fma(-l1i, ur, x1i));
+                __syncwarp();                                         // every lane has read the two pivot rows
+                cr[r0] = fma(-m0r, v2r, fma(m0i, v2i, t0r));
+                ci[r0] = fma(-m0r, v2i, fma(-m0i, v2r, t0i));
+                cr[r1] = fma(-m1r, v2r, fma(m1i, v2i, t1r));
+                ci[r1] = fma(-m1r, v2i, fma(-m1i, v2r, t1i));
+            }
+        }
+        bar();
+    }
+    write_back((N - 1) & ~1);
+    bar();
+    const int p0 = g0 ? xc.perm[i0] : N, p1 = g1 ? xc.perm[i1] : N;
+    const double q0r = g0 ? xc.rdr[i0] : 0.0, q0i = g0 ? xc.rdi[i0] : 0.0, q1r = g1 ? xc.rdr[i1] : 0.0, q1i = g1 ? xc.rdi[i1] : 0.0;
+#pragma unroll 1
+    for (int j = wq; j < N; j += NWc) {
+        double *cr = Ar + j * LD, *ci = Ai + j * LD;
+        double z0r = cr[p0], z0i = ci[p0], z1r = cr[p1], z1i = ci[p1];
+        if (j > i0) { const double t = z0r * q0r - z0i * q0i; z0i = z0r * q0i + z0i * q0r; z0r = t; }
+        if (j > i1) { const double t = z1r * q1r - z1i * q1i; z1i = z1r * q1i + z1i * q1r; z1r = t; }
+        __syncwarp();
+        if (g0) { cr[i0] = z0r; ci[i0] = z0i; }
+        if (g1) { cr[i1] = z1r; ci[i1] = z1i; }
+    }
+    return 0;
+}
+
+// one CTA of 128 threads; includes the barrier behind the factorisation
+__device__ __noinline__ int lu2_split(int N, int LD, double *A, const Lu2Aux &xag, double *Ar, double *Ai, const Lu2Aux &xcg)
+{
+    const Lu2Aux xa = shp(xag), xc = shp(xcg);
+    A = shp(A); Ar = shp(Ar); Ai = shp(Ai);
+    const int wl = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    int ier;
+    if (wp == 0) ier = lu2_real_warp(N, LD, A, xa, wl);
+    else ier = lu2_complex_warps(N, LD, Ar, Ai, xc, wl, wp - 1, 3);
+    return __syncthreads_or(ier);
+}
+
 // Solves with the factors as lu2_pair leaves them (rows in pivot order, unit-diagonal scaled U): b (shared, length N,
 // original row order) is overwritten by x.  Lane l holds components l and l + 32; step k broadcasts component k
 // and every later (earlier) row subtracts its multiple: the chain per step is one shuffle and one fused multiply-add

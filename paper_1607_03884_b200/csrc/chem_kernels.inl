@@ -204,7 +204,7 @@ __global__ void __launch_bounds__(128) lu2_solve_kernel(int n, int batch, int is
             z3[i] = is_complex ? b[2 * g + 1] : 0.0;
         }
         __syncthreads();
-        const int ier = lu2_pair<128>(n, LD, E1, x1, E2r, E2i, x2);
+        const int ier = (s & 1) ? lu2_pair<128>(n, LD, E1, x1, E2r, E2i, x2) : lu2_split(n, LD, E1, x1, E2r, E2i, x2);   // both forms are tested
         __syncthreads();
         if (!ier) {
             solve2_pair<128>(n, LD, E1, x1, z1, E2r, E2i, x2, z2, z3);

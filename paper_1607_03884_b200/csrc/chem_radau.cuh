@@ -193,7 +193,8 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
             int ier = Grp<G>::any(nonfinite, w.cs.red);   // includes the barrier after the stores
             if (G == 32) __syncwarp();
             if (N <= 64) {
-                if (!ier) ier = lu2_pair<G>(N, LD, w.E1, w.x1, w.E2r, w.E2i, w.x2);
+                if constexpr (G == 128) { if (!ier) ier = lu2_split(N, LD, w.E1, w.x1, w.E2r, w.E2i, w.x2); }
+                else if (!ier) ier = lu2_pair<G>(N, LD, w.E1, w.x1, w.E2r, w.E2i, w.x2);
             } else {
                 if (!ier) ier = lu_real<G>(N, w.E1, w.ip1);
                 if (!ier) ier = lu_complex<G>(N, w.E2r, w.E2i, w.ip2);
