@@ -87,7 +87,8 @@ typedef struct chem_opts {
     double h0;           /* first internal step size; 0 -> t_end (R9)                      */
     int32_t max_steps;   /* limit on internal step attempts per state; 0 -> 100000                    */
     int32_t newton_max;  /* max simplified-Newton iterations per step; 0 -> 7                         */
-    int32_t kernel;      /* 0 auto; 1 shared-memory group kernel; 2 compact warp-per-state kernel (small mechanisms) */
+    int32_t kernel;      /* 0 auto; 1 shared-memory group kernel (warp or CTA per state); 2 warp-per-state kernel and
+                            3 thread-per-state kernel (both: small mechanisms only, N_sp <= 16, N_rx <= 32) */
     int32_t reorder;     /* 1: start the states in order of decreasing cost_hint ("reordering IVPs"); 0 off */
     const double *P_per_state;  /* device [n_states] or NULL: per-state pressure overriding P        */
     const int32_t *cost_hint;   /* device [n_states] or NULL: predicted cost per state, e.g. chem_stats.nstep of the
@@ -153,6 +154,10 @@ int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, doubl
 
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 int64_t chem_launch_count(void);
+
+/* Kernel id (1, 2 or 3 as in chem_opts.kernel) of the last chem_integrate / chem_integrate_ex / chem_integrate_host
+ * launch issued with this mechanism; 0 before the first.  Not synchronised with concurrent callers. */
+int chem_last_kernel(const chem_mech *mech);
 
 /* Algorithmic floating-point operation counts of the compiled mechanism:
  * out[0] = one source-term evaluation, out[1] = one Jacobian evaluation, out[2] = one LU pair (real + complex),

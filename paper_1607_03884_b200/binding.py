@@ -45,7 +45,7 @@ assert STATS_DTYPE.itemsize == 48
 
 EXPORTS = ["chem_mech_load", "chem_mech_free", "chem_mech_info", "chem_rhs", "chem_jacobian", "chem_lu_solve",
            "chem_integrate", "chem_integrate_ex", "chem_integrate_host", "chem_launch_count", "chem_flop_model",
-           "chem_last_error"]
+           "chem_last_error", "chem_last_kernel"]
 
 _lib = None
 
@@ -75,6 +75,7 @@ def lib():
         L.chem_integrate_host.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
                                           C.c_void_p, C.c_void_p, C.POINTER(chem_opts), C.c_void_p]
         L.chem_flop_model.argtypes = [C.c_void_p, _dp]
+        L.chem_last_kernel.argtypes = [C.c_void_p]
         _lib = L
     return _lib
 
@@ -227,6 +228,14 @@ def chem_integrate_host(mech: Mechanism, P: float, t_end: float, rtol: float, at
                                      C.c_void_p(y_out_host.ctypes.data), C.byref(o),
                                      C.c_void_p(stats.ctypes.data) if want_stats else None))
     return (y_out_host, stats) if want_stats else y_out_host
+
+
+KERNEL_NAMES = {0: "none", 1: "integrate_kernel (group per state)", 2: "integrate_warp_kernel (warp per state)",
+                3: "integrate_tps_kernel (thread per state)"}
+
+
+def chem_last_kernel(mech: Mechanism) -> int:
+    return int(lib().chem_last_kernel(mech._h))
 
 
 def chem_launch_count() -> int:

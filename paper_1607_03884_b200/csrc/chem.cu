@@ -1,23 +1,20 @@
 // chem.cu -- C ABI (include/chem.h): mechanism compiler, kernels, launch logic.
 // sm_100a only; no CPU fallback: every compute entry point fails with CHEM_E_CUDA without a device.
-#include "../../include/chem.h"
-
-#include <cuda_runtime.h>
+#include "chem_host.h"
+#include "chem_radau_warp.cuh"
 
 #include <algorithm>
-#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
-#include "chem_radau_warp.cuh"
-
 using namespace chem;
 
-namespace {
+namespace chem_host {
 
 thread_local std::string g_err;
 std::atomic<int64_t> g_launches{0};
@@ -32,31 +29,33 @@ int fail(int code, const char *fmt, ...)
     g_err = buf;
     return code;
 }
-#define CUDA_TRY(expr)                                                                              \
-    do {                                                                                            \
-        cudaError_t e_ = (expr);                                                                    \
-        if (e_ != cudaSuccess) return fail(CHEM_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e_));   \
-    } while (0)
 
-}  // namespace
+// Stream-ordered scratch: the default memory pool of the device with its release threshold lifted once, so that the
+// blocks of one launch are reused by the next without going back to the driver.
+int scratch_alloc(void **p, size_t bytes, cudaStream_t st)
+{
+    static std::once_flag once;
+    std::call_once(once, [] {
+        int dev = 0;
+        cudaMemPool_t pool;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            uint64_t keep = UINT64_MAX;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    });
+    *p = nullptr;
+    CUDA_TRY(cudaMallocAsync(p, bytes, st));
+    return CHEM_OK;
+}
+void scratch_free(void *p, cudaStream_t st)
+{
+    if (p) cudaFreeAsync(p, st);
+}
 
-struct chem_mech {
-    Tables t{};
-    void *dev_blob = nullptr;   // one allocation holding every table
-    int *counter = nullptr;     // work-queue head (device)
-    int n_sm = 0;
-    int max_smem_optin = 0;
-    // algorithmic flop model
-    double flops[5] = {0, 0, 0, 0, 0};
-    FastTables fast{};          // register-resident warp path (chem_warp.cuh), if eligible
-    void *fast_blob = nullptr;
-    void *order_buf = nullptr;  // scratch of the optional cost ordering (grown on demand)
-    size_t order_bytes = 0;
-    // host-buffer entry point: cached device staging buffer and two streams for chunked copy/compute overlap
-    void *host_buf = nullptr;
-    size_t host_bytes = 0;
-    cudaStream_t hs[2] = {nullptr, nullptr};
-};
+}  // namespace chem_host
+
+using chem_host::fail;
+using chem_host::g_launches;
 
 #include "chem_fast.inl"
 
@@ -380,15 +379,14 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
 
     chem_mech *m = new (std::nothrow) chem_mech;
     if (!m) return fail(CHEM_E_NOMEM, "out of host memory");
-    if (cudaMalloc(&m->dev_blob, total) != cudaSuccess || cudaMalloc(&m->counter, 64) != cudaSuccess) {
+    if (cudaMalloc(&m->dev_blob, total) != cudaSuccess) {
         cudaError_t e = cudaGetLastError();
-        if (m->dev_blob) cudaFree(m->dev_blob);
         delete m;
         return fail(CHEM_E_CUDA, "cudaMalloc: %s", cudaGetErrorString(e));
     }
     if (cudaMemcpy(m->dev_blob, host.data(), total, cudaMemcpyHostToDevice) != cudaSuccess) {
         cudaError_t e = cudaGetLastError();
-        cudaFree(m->dev_blob); cudaFree(m->counter);
+        cudaFree(m->dev_blob);
         delete m;
         return fail(CHEM_E_CUDA, "cudaMemcpy: %s", cudaGetErrorString(e));
     }
@@ -431,11 +429,8 @@ extern "C" void chem_mech_free(chem_mech *m)
 {
     if (!m) return;
     if (m->dev_blob) cudaFree(m->dev_blob);
-    if (m->counter) cudaFree(m->counter);
     if (m->fast_blob) cudaFree(m->fast_blob);
-    if (m->order_buf) cudaFree(m->order_buf);
-    if (m->host_buf) cudaFree(m->host_buf);
-    for (int i = 0; i < 2; i++)
+    for (int i = 0; i < 4; i++)
         if (m->hs[i]) cudaStreamDestroy(m->hs[i]);
     delete m;
 }
@@ -456,6 +451,6 @@ extern "C" int chem_flop_model(const chem_mech *m, double out[5])
 }
 
 extern "C" int64_t chem_launch_count(void) { return g_launches.load(); }
-extern "C" const char *chem_last_error(void) { return g_err.c_str(); }
+extern "C" const char *chem_last_error(void) { return chem_host::g_err.c_str(); }
 
 #include "chem_kernels.inl"

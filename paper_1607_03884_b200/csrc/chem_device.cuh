@@ -11,48 +11,9 @@
 #include <cuda_runtime.h>
 #include <math.h>
 
-#include "chem_math.cuh"
+#include "chem_common.cuh"
 
 namespace chem {
-
-constexpr double kRerg = 8.31446261815324e7;  // erg/(mol K)
-constexpr double kRcal = 1.98720425864083;    // cal/(mol K)
-constexpr double kPatm = 1.01325e6;           // dyn/cm^2
-constexpr int kSlots = 6;                     // 3 reactant + 3 product slots per reaction
-
-// Packed device tables written by the mechanism compiler (chem_mech_load).
-struct Tables {
-    int n_sp, n_rx;
-    const double *W, *invW;           // [n_sp]
-    const double *nasa_lo, *nasa_hi;  // [7][n_sp], coefficient-major
-    const double *tmid;               // [n_sp]
-    const int *rtype;                 // [n_rx]
-    const double *lnA, *b, *Ta;       // [n_rx]  ln A, b, Ea/R [K]
-    const double *lnA0, *b0, *Ta0;    // [n_rx]  low-pressure limit
-    const double *dnu;                // [n_rx]  sum nu'' - sum nu'
-    const double *troe;               // [4][n_rx]
-    const int *slot_sp, *slot_nu;     // [6][n_rx]; slots 0-2 reactants, 3-5 products; unused: sp 0, nu 0
-    const int *eff_ptr, *eff_sp;      // CSR over reactions
-    const double *eff_dv;             // alpha - 1
-    const int *inc_ptr, *inc_rx;      // CSR over species: reactions the species takes part in
-    const double *inc_nu;             // net stoichiometric coefficient nu'' - nu'
-    // exp-job form of the rate constants (chem_cta.cuh); n_jobs == 0: not available for this mechanism
-    const double *job_lo, *job_hi;    // [n_jobs][8]: k_f [0,n_rx), k_r [n_rx,2 n_rx), then k_0/k_inf and Troe terms
-    const int *rdesc;                 // [n_rx][8]: factors 0-2 (8 bits each, 63 = unity), factors 3-5, type, extra job, falloff ordinal, eff_lo, eff_hi, 0
-    int n_jobs, n_fo;
-    double tmid0;
-    // balanced gather schedule of cta_rhs3 (chem.cu): per thread of a group (species or -1, first entry, end, log2 of the
-    // species' thread count); inc2 = (reaction, net coefficient) pairs in inc_ptr order; gat_steps = max log2, -1: none
-    const int4 *gat;
-    const int2 *inc2;
-    int gat_steps;
-    int n_solo;                       // threads t < n_solo evaluate table reaction t only (chem.cu)
-    // balanced row gather of the analytical Jacobian (jacobian<128>): schedule like `gat` for gatj_T threads (0: none),
-    // jinc = two int4 per incidence: (reaction, net coefficient, slot species 0-2, slot species 3-5), (eff_lo, eff_hi, has [M], 0)
-    const int4 *gatj;
-    const int4 *jinc;
-    int gatj_T;
-};
 
 // ---------------------------------------------------------------------------------------------
 template <int G>

@@ -30,8 +30,8 @@ __device__ __forceinline__ int next_state(int *counter, int *bcast)
 
 template <int G>
 __global__ void __launch_bounds__(block_of<G>(), G > kBlock ? 2 : 1) integrate_kernel(Tables t_arg, int n_states, double P, const double *P_per_state,
-                                                           RadauParams prm, const double *__restrict__ y_in,
-                                                           double *__restrict__ y_out, chem_stats *stats, int *counter,
+                                                           RadauParams prm, const double *y_in,
+                                                           double *y_out, chem_stats *stats, int *counter,
                                                            const int *order)
 {
     extern __shared__ double smem[];
@@ -71,7 +71,7 @@ constexpr int kWarpBlock = 640;
 
 __global__ void __launch_bounds__(kWarpBlock, 1) integrate_warp_kernel(Tables t, FastTables ft, int n_states, double P,
                                                                     const double *P_per_state, RadauParams prm,
-                                                                    const double *__restrict__ y_in, double *__restrict__ y_out,
+                                                                    const double *y_in, double *y_out,
                                                                     chem_stats *stats, int *counter, const int *order)
 {
     extern __shared__ double smem[];
@@ -239,7 +239,7 @@ __global__ void __launch_bounds__(32) lu_solve_warp_kernel(int n, int batch, int
         double rdr = 0.0, rdi = 0.0;
         const int ier = gj_warp_pair(Z, LD, n, myk, src, rdr, rdi);
         __syncwarp();
-        if (lane == 0) info[s] = ier;
+        if (info && lane == 0) info[s] = ier;
         if (!ier) {
             const size_t g = (size_t)s * n + (r < n ? r : 0);
             const double br = is_complex ? b[2 * g] : b[g], bi = is_complex ? b[2 * g + 1] : 0.0;

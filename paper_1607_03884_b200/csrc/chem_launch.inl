@@ -27,21 +27,17 @@ __global__ void iota_kernel(int n, int *v)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) v[i] = i;
 }
-int build_order(const chem_mech *m, int n, const int32_t *cost, int **order_out, cudaStream_t st)
+// Builds the start order in per-launch scratch (stream-ordered allocation; the caller frees *scratch after its launch).
+int build_order(int n, const int32_t *cost, int **order_out, void **scratch, cudaStream_t st)
 {
-    chem_mech *mm = const_cast<chem_mech *>(m);
     size_t tmp_bytes = 0;
     cub::DeviceRadixSort::SortPairsDescending(nullptr, tmp_bytes, cost, (int32_t *)nullptr, (int *)nullptr, (int *)nullptr, n, 0, 32, st);
-    const size_t need = (size_t)3 * n * sizeof(int) + tmp_bytes + 256;
-    if (need > mm->order_bytes) {
-        if (mm->order_buf) cudaFree(mm->order_buf);
-        mm->order_buf = nullptr; mm->order_bytes = 0;
-        CUDA_TRY(cudaMalloc(&mm->order_buf, need));
-        mm->order_bytes = need;
-    }
-    int *idx = static_cast<int *>(mm->order_buf), *ord = idx + n;
+    const size_t head = ((size_t)3 * n * sizeof(int) + 255) & ~size_t(255);
+    int rc = chem_host::scratch_alloc(scratch, head + tmp_bytes + 256, st);
+    if (rc) return rc;
+    int *idx = static_cast<int *>(*scratch), *ord = idx + n;
     int32_t *keys_out = reinterpret_cast<int32_t *>(ord + n);
-    void *tmp = reinterpret_cast<char *>(mm->order_buf) + (((size_t)3 * n * sizeof(int) + 255) & ~size_t(255));
+    void *tmp = static_cast<char *>(*scratch) + head;
     iota_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, idx);
     g_launches++;
     CUDA_TRY(cub::DeviceRadixSort::SortPairsDescending(tmp, tmp_bytes, cost, keys_out, idx, ord, n, 0, 32, st));
@@ -66,9 +62,11 @@ int launch_eval(const chem_mech *m, int n, double P, const double *y, double *ou
     return CHEM_OK;
 }
 
+// Every launch has its own work-queue head (4 bytes of stream-ordered scratch, zeroed on the stream), so launches on
+// different streams with the same mechanism do not interfere.
 template <int G>
 int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
-                     const chem_opts *o, chem_stats *stats, cudaStream_t st, int slot)
+                     const chem_opts *o, chem_stats *stats, const int *order, cudaStream_t st)
 {
     const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (block_of<G>() / G);
     int occ = 0;
@@ -77,19 +75,24 @@ int launch_integrate(const chem_mech *m, int n, double P, const RadauParams &prm
     const int gpb = block_of<G>() / G;
     int grid = (n + gpb - 1) / gpb;
     if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, groups pull work from the queue
-    int *counter = m->counter + slot;     // one work-queue head per concurrently running launch
-    CUDA_TRY(cudaMemsetAsync(counter, 0, sizeof(int), st));
-    int *order = nullptr;
-    if (o && o->reorder && o->cost_hint) { rc = build_order(m, n, o->cost_hint, &order, st); if (rc) return rc; }
-    integrate_kernel<G><<<grid, block_of<G>(), smem, st>>>(m->t, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats,
-                                                    counter, order);
-    g_launches++;
-    CUDA_TRY(cudaGetLastError());
+    void *scratch = nullptr;
+    rc = chem_host::scratch_alloc(&scratch, 256, st);
+    if (rc) return rc;
+    int *counter = static_cast<int *>(scratch);
+    cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(int), st);
+    if (e == cudaSuccess) {
+        integrate_kernel<G><<<grid, block_of<G>(), smem, st>>>(m->t, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats,
+                                                        counter, order);
+        g_launches++;
+        e = cudaGetLastError();
+    }
+    chem_host::scratch_free(scratch, st);
+    CUDA_TRY(e);
     return CHEM_OK;
 }
 
 int launch_integrate_warp(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
-                          const chem_opts *o, chem_stats *stats, cudaStream_t st, int slot)
+                          const chem_opts *o, chem_stats *stats, const int *order, cudaStream_t st)
 {
     const int wpb = kWarpBlock / 32;
     const size_t smem = ((size_t)m->fast.blob_doubles + (size_t)wpb * warp_ws_doubles(m->t.n_sp, m->t.n_rx)) * sizeof(double);
@@ -100,14 +103,19 @@ int launch_integrate_warp(const chem_mech *m, int n, double P, const RadauParams
     if (occ < 1) return fail(CHEM_E_UNSUPPORTED, "warp kernel does not fit on an SM");
     int grid = (n + wpb - 1) / wpb;
     if (grid > m->n_sm * occ) grid = m->n_sm * occ;   // persistent: one wave, warps pull states from the queue
-    int *counter = m->counter + slot;
-    CUDA_TRY(cudaMemsetAsync(counter, 0, sizeof(int), st));
-    int *order = nullptr;
-    if (o && o->reorder && o->cost_hint) { const int rc = build_order(m, n, o->cost_hint, &order, st); if (rc) return rc; }
-    integrate_warp_kernel<<<grid, kWarpBlock, smem, st>>>(m->t, m->fast, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out,
-                                                          stats, counter, order);
-    g_launches++;
-    CUDA_TRY(cudaGetLastError());
+    void *scratch = nullptr;
+    const int rc = chem_host::scratch_alloc(&scratch, 256, st);
+    if (rc) return rc;
+    int *counter = static_cast<int *>(scratch);
+    cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(int), st);
+    if (e == cudaSuccess) {
+        integrate_warp_kernel<<<grid, kWarpBlock, smem, st>>>(m->t, m->fast, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out,
+                                                              stats, counter, order);
+        g_launches++;
+        e = cudaGetLastError();
+    }
+    chem_host::scratch_free(scratch, st);
+    CUDA_TRY(e);
     return CHEM_OK;
 }
 
@@ -167,11 +175,24 @@ extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const
 }
 
 namespace {
+// Kernel ids (chem_opts.kernel, chem_last_kernel): 1 shared-memory group kernel, 2 warp-per-state, 3 thread-per-state.
+// Auto picks the fastest measured mapping (profiles/r2_mapping_config1.md, r2_mapping_config2.md): the warp-per-state
+// kernel when the mechanism is eligible, else the group kernel; the thread-per-state kernel is chosen explicitly.
+int pick_kernel(const chem_mech *m, int n, const chem_opts *o)
+{
+    (void)n;
+    const int want = o ? o->kernel : 0;
+    if (want != 0) return want;
+    if (warp_path_available(m)) return 2;
+    return 1;
+}
+
 int integrate_impl(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol, const double *y_in,
-                   double *y_out, const chem_opts *o, chem_stats *stats, cudaStream_t st, int slot)
+                   double *y_out, const chem_opts *o, chem_stats *stats, cudaStream_t st)
 {
     if (!m || n < 0 || (n > 0 && (!y_in || !y_out))) return fail(CHEM_E_ARG, "bad argument");
     if (!(t_end > 0.0) || !(rtol > 0.0) || !(atol > 0.0)) return fail(CHEM_E_ARG, "t_end, rtol and atol must be positive");
+    if (o && (o->kernel < 0 || o->kernel > 3)) return fail(CHEM_E_ARG, "chem_opts.kernel must be 0..3");
     if (n == 0) return CHEM_OK;
     RadauParams prm;
     prm.t_end = t_end; prm.rtol = rtol; prm.atol = atol;
@@ -184,18 +205,32 @@ int integrate_impl(const chem_mech *m, int32_t n, double P, double t_end, double
     prm.atol_t = prm.rtol_t * (atol / rtol);
     prm.fnewt = std::fmax(10.0 * 2.220446049250313e-16 / prm.rtol_t, std::fmin(0.03, std::sqrt(prm.rtol_t)));
     prm.inv_fnewt = 1.0 / prm.fnewt; prm.inv_n = 1.0 / m->t.n_sp; prm.inv_3n = 1.0 / (3 * m->t.n_sp);
-    const int kernel = o ? o->kernel : 0;
-    if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "register-resident warp kernel not available for this mechanism");
-    if (kernel != 1 && warp_path_available(m)) return launch_integrate_warp(m, n, P, prm, y_in, y_out, o, stats, st, slot);
-    return group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, st, slot)
-                               : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, st, slot);
+    const int kernel = pick_kernel(m, n, o);
+    if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "warp-per-state kernel not available for this mechanism");
+    if (kernel == 3 && !chem_tps_available(m)) return fail(CHEM_E_UNSUPPORTED, "thread-per-state kernel not available for this mechanism");
+    int *order = nullptr;
+    void *order_scratch = nullptr;
+    if (o && o->reorder && o->cost_hint) {
+        const int rc = build_order(n, o->cost_hint, &order, &order_scratch, st);
+        if (rc) { chem_host::scratch_free(order_scratch, st); return rc; }
+    }
+    int rc;
+    if (kernel == 3) rc = chem_tps_launch(m, n, P, prm, y_in, y_out, o, stats, order, st);
+    else if (kernel == 2) rc = launch_integrate_warp(m, n, P, prm, y_in, y_out, o, stats, order, st);
+    else rc = group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, order, st)
+                                  : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, order, st);
+    chem_host::scratch_free(order_scratch, st);
+    if (rc == CHEM_OK) const_cast<chem_mech *>(m)->last_kernel = kernel;
+    return rc;
 }
 }  // namespace
+
+extern "C" int chem_last_kernel(const chem_mech *m) { return m ? m->last_kernel : 0; }
 
 extern "C" int chem_integrate_ex(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
                                  const double *y_in, double *y_out, const chem_opts *o, chem_stats *stats, void *stream)
 {
-    return integrate_impl(m, n, P, t_end, rtol, atol, y_in, y_out, o, stats, static_cast<cudaStream_t>(stream), 0);
+    return integrate_impl(m, n, P, t_end, rtol, atol, y_in, y_out, o, stats, static_cast<cudaStream_t>(stream));
 }
 
 extern "C" int chem_integrate(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
@@ -212,20 +247,17 @@ extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, doub
     chem_mech *mm = const_cast<chem_mech *>(m);
     const int N = m->t.n_sp;
     const size_t ybytes = (size_t)n * N * sizeof(double), sbytes = stats_host ? (size_t)n * sizeof(chem_stats) : 0;
-    if (ybytes + sbytes > mm->host_bytes) {          // cached staging buffer, grown on demand
-        if (mm->host_buf) cudaFree(mm->host_buf);
-        mm->host_buf = nullptr; mm->host_bytes = 0;
-        CUDA_TRY(cudaMalloc(&mm->host_buf, ybytes + sbytes));
-        mm->host_bytes = ybytes + sbytes;
-    }
     for (int i = 0; i < 2; i++)
         if (!mm->hs[i]) CUDA_TRY(cudaStreamCreateWithFlags(&mm->hs[i], cudaStreamNonBlocking));
-    double *d_y = static_cast<double *>(mm->host_buf);
-    chem_stats *d_st = stats_host ? reinterpret_cast<chem_stats *>(static_cast<char *>(mm->host_buf) + ybytes) : nullptr;
+    void *buf = nullptr;
+    int rc = chem_host::scratch_alloc(&buf, ybytes + sbytes + 256, mm->hs[0]);
+    if (rc) return rc;
+    CUDA_TRY(cudaStreamSynchronize(mm->hs[0]));       // the block is used from both streams
+    double *d_y = static_cast<double *>(buf);
+    chem_stats *d_st = stats_host ? reinterpret_cast<chem_stats *>(static_cast<char *>(buf) + ((ybytes + 255) & ~size_t(255))) : nullptr;
     // chunks alternate between two streams so that the copies of one chunk overlap the kernel of the other
     // (the paper's GPU timings include the transfers); per-state results do not depend on the chunking
-    const int n_chunks = n >= 65536 ? 2 : 1;     // every extra launch adds one tail (slowest states) of ~2 ms
-    int rc = CHEM_OK;
+    const int n_chunks = n >= 65536 ? 2 : 1;     // every extra launch adds one tail (slowest states)
     cudaError_t e = cudaSuccess;
     for (int c = 0; c < n_chunks && rc == CHEM_OK && e == cudaSuccess; c++) {
         const int lo = (int)((long long)n * c / n_chunks), hi = (int)((long long)n * (c + 1) / n_chunks);
@@ -235,13 +267,13 @@ extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, doub
         if (o) {
             oc = *o;
             if (oc.P_per_state) oc.P_per_state += lo;
-            oc.reorder = 0;          // the ordering scratch is shared by launches; chunks are short anyway
+            oc.reorder = 0;          // cost hints are device arrays of the whole batch; chunks are short anyway
             oc.cost_hint = nullptr;
         }
         const size_t off = (size_t)lo * N, cnt = (size_t)(hi - lo) * N;
         e = cudaMemcpyAsync(d_y + off, y_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) break;
-        rc = integrate_impl(m, hi - lo, P, t_end, rtol, atol, d_y + off, d_y + off, o ? &oc : nullptr, d_st ? d_st + lo : nullptr, st, 1 + (c & 1));
+        rc = integrate_impl(m, hi - lo, P, t_end, rtol, atol, d_y + off, d_y + off, o ? &oc : nullptr, d_st ? d_st + lo : nullptr, st);
         if (rc != CHEM_OK) break;
         e = cudaMemcpyAsync(y_out_host + off, d_y + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess && stats_host)
@@ -251,6 +283,7 @@ extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, doub
         const cudaError_t e2 = cudaStreamSynchronize(mm->hs[i]);
         if (e == cudaSuccess) e = e2;
     }
+    chem_host::scratch_free(buf, mm->hs[0]);
     if (rc != CHEM_OK) return rc;
     if (e != cudaSuccess) return fail(CHEM_E_CUDA, "chem_integrate_host: %s", cudaGetErrorString(e));
     return CHEM_OK;

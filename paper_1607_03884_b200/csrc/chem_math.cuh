@@ -21,9 +21,9 @@ constexpr double kLn10 = 2.302585092994045684, kInvLn10 = 0.4342944819032518277;
 // this path).  Polynomial coefficients sit in constant memory so that each Horner step is ONE DFMA with a constant-bank
 // operand (the libdevice versions spend two UMOVs per coefficient and are 2-3x larger, which matters for the 32 KB
 // instruction cache).  Accuracy ~1-2 ulp; no special-case handling beyond what is stated.
-__constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320, 1.0 / 362880,
+static __constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320, 1.0 / 362880,
                                  1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
-__constant__ double kAtanhC[11] = {2.0, 2.0 / 3, 2.0 / 5, 2.0 / 7, 2.0 / 9, 2.0 / 11, 2.0 / 13, 2.0 / 15, 2.0 / 17, 2.0 / 19, 2.0 / 21};
+static __constant__ double kAtanhC[11] = {2.0, 2.0 / 3, 2.0 / 5, 2.0 / 7, 2.0 / 9, 2.0 / 11, 2.0 / 13, 2.0 / 15, 2.0 / 17, 2.0 / 19, 2.0 / 21};
 
 // 1/x for normal x (rcp_nr above): hardware seed + two Newton steps; no denormal / zero / inf handling
 __device__ __forceinline__ double rcp_f(double x) { return rcp_nr(x); }

@@ -10,23 +10,6 @@
 
 namespace chem {
 
-// Method constants (R7).  The real matrices T, T^-1 block-diagonalise A^-1 into
-// gamma (real) and alpha +- i beta; values to 20 digits from Hairer & Wanner, Sec. IV.8.
-namespace rk {
-constexpr double SQ6 = 2.449489742783178098;
-constexpr double C1 = (4.0 - SQ6) / 10.0, C2 = (4.0 + SQ6) / 10.0;
-constexpr double C1M1 = C1 - 1.0, C2M1 = C2 - 1.0, C1MC2 = C1 - C2;
-constexpr double DD1 = -(13.0 + 7.0 * SQ6) / 3.0, DD2 = (-13.0 + 7.0 * SQ6) / 3.0, DD3 = -1.0 / 3.0;
-// 1/u1, alpha/(alpha^2+beta^2), beta/(alpha^2+beta^2) of RADAU5, evaluated once in extended precision
-constexpr double U1 = 3.637834252744495732, ALPH = 2.681082873627752134, BETA = 3.050430199247410569;
-constexpr double T11 = 9.1232394870892942792e-02, T12 = -0.14125529502095420843, T13 = -3.0029194105147424492e-02;
-constexpr double T21 = 0.24171793270710701896, T22 = 0.20412935229379993199, T23 = 0.38294211275726193779;
-constexpr double T31 = 0.96604818261509293619;
-constexpr double TI11 = 4.3255798900631553510, TI12 = 0.33919925181580986954, TI13 = 0.54177053993587487119;
-constexpr double TI21 = -4.1787185915519047273, TI22 = -0.32768282076106238708, TI23 = 0.47662355450055045196;
-constexpr double TI31 = -0.50287263494578687595, TI32 = 2.5719269498556054292, TI33 = -0.59603920482822492497;
-}  // namespace rk
-
 // Shared-memory work area of one group (pointers into the CTA's dynamic shared memory).
 struct Work {
     double *y, *f0, *scal, *z1, *z2, *z3, *w1, *w2, *w3, *c1, *c2, *c3, *ys, *a1, *a2, *a3;  // [N] each
@@ -83,20 +66,6 @@ __device__ __forceinline__ Work carve(double *base, int N, int NR, int NW, int n
     w.cx.red6 = take(6 * NW + 2);
     return w;
 }
-
-struct RadauParams {
-    double t_end, rtol, atol, h0;
-    int max_steps, newton_max;
-    int fd_jacobian;                // 1: CVODE-style difference-quotient Jacobian (R13)
-    int fixed_steps;                // > 0: that many equal steps, no error control
-    double rtol_t, atol_t, fnewt;   // RADAU5's transformed tolerances and Newton stopping level (R8), set on the host
-    double inv_fnewt, inv_n, inv_3n; // 1/fnewt, 1/N, 1/(3N): host-side divisions for the warp path
-};
-
-struct RadauResult {
-    int status, nstep, naccpt, nrejct, nfcn, njac, ndec, nsol, nnewt_fail;
-    double h_last;
-};
 
 // Integrate the state in w.y from 0 to t_end.  Uniform control flow across the group.
 template <int G>

@@ -1,0 +1,508 @@
+// chem_tps.cuh -- thread-per-state path for small mechanisms (N_sp <= 16, N_rx <= 32): device routines.
+//
+// The paper's own GPU mapping is one CUDA thread per IVP, and it names the two things that
+// limit it: thread divergence (L184, L194) and the storage of the Jacobian and its factors (L182).  This is that
+// mapping rebuilt for sm_100a:
+//   * every lane of a warp owns one state and runs the Radau IIA controller as a STATE MACHINE; a warp executes the
+//     phases (Newton iteration, error estimate, source term, Jacobian, factorisation) one after the other, each for the
+//     lanes that want it, and a lane that finishes its state pulls the next one from the work queue at once -- so the
+//     spread of step counts between states (Eq. 3) costs nothing, and what is left of divergence is the share of lanes
+//     that sit out a phase;
+//   * all data of a lane is addressed [element][lane] (structure of arrays across the warp): every access of a warp is
+//     one coalesced 256-byte row, in shared memory (work vectors, conflict-free) and in global memory (the matrices,
+//     L2-resident); element indices are uniform across the warp except for the row interchanges of partial pivoting;
+//   * there is no cross-lane communication at all: no shuffles, no reductions, no barriers after the tables are staged.
+// The arithmetic is that of chem_warp.cuh (exp-job tables of the mechanism compiler, R1-R12) with plain LU +
+// triangular solves, left-looking so that each factor entry is written once.
+#pragma once
+#include "chem_common.cuh"
+
+namespace chem {
+namespace tps {
+
+typedef unsigned long long u64;
+
+// lane-private element e of an array whose rows are 32 lanes wide
+#define TL(p, e) (p)[(e) * 32]
+
+// Shared-memory elements per lane: y[N], 1/scal[N], z1..z3[3N], a1..a3[3N], q[QL], C[N+1], row[N+1], S[N].
+// The Jacobian's per-reaction records (4 per reaction) alias z, a and q, which are dead then; QL >= N_rx makes them fit.
+struct Lay {
+    int N, NR, oC, n_sm;   // oC: offset of C; row = oC + N + 1; S = row + N + 1
+    int n_gw;              // global elements per lane: J[N^2], E1[N^2], E2[N^2] complex, f0[N], cont[3N], w1..w3[3N]
+};
+__host__ __device__ inline Lay make_lay(int N, int NR)
+{
+    Lay L;
+    L.N = N; L.NR = NR;
+    const int need = 4 * NR, have = 6 * N + NR;
+    const int ql = NR + (need > have ? need - have : 0);
+    L.oC = 8 * N + ql;
+    L.n_sm = L.oC + (N + 1) + (N + 1) + N;
+    L.n_gw = 4 * N * N + 7 * N;
+    return L;
+}
+__host__ __device__ inline int oIS(int N) { return N; }
+__host__ __device__ inline int oZ(int N) { return 2 * N; }
+__host__ __device__ inline int oA(int N) { return 5 * N; }
+__host__ __device__ inline int oQ(int N) { return 8 * N; }
+__host__ __device__ inline int gE1(int N) { return N * N; }
+__host__ __device__ inline int gE2(int N) { return 2 * N * N; }   // in doubles; E2 is addressed as double2 from here
+__host__ __device__ inline int gF0(int N) { return 4 * N * N; }
+__host__ __device__ inline int gCT(int N) { return 4 * N * N + N; }
+__host__ __device__ inline int gW(int N) { return 4 * N * N + 4 * N; }
+
+__device__ __forceinline__ double nan_d() { return __longlong_as_double(0x7ff8000000000000LL); }
+
+// ------------------------------------------------------------------------------------------------ source term
+// f(T, Y; P) at the state y + vs * v (R1-R5; same mathematics as warp_rhs_body, chem_warp.cuh), all lane-private:
+// y = sm[0..N), v = sm[ov..), result -> sm[of..).  tab = staged table blob (shared, read with uniform indices).
+__device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, int oC, double tmid, double P, double invP,
+                                 int ov, double vs, int of)
+{
+    const int *hdr = reinterpret_cast<const int *>(tab);
+    const int4 *desc = reinterpret_cast<const int4 *>(tab + kOffDesc);
+    const double *y = sm, *v = sm + ov * 32;
+    double *C = sm + oC * 32, *q = sm + oQ(N) * 32, *out = sm + of * 32;
+    const double *spw = tab + kOffSpLo;                       // W and 1/W are the same in both NASA ranges
+    const double T = fma(vs, TL(v, 0), TL(y, 0));
+    double sY = 0.0, sYW = 0.0;
+#pragma unroll 4
+    for (int k = 0; k < N - 1; k++) {
+        const double Yk = fma(vs, TL(v, k + 1), TL(y, k + 1));
+        sY += Yk;
+        sYW = fma(Yk, spw[k * kJobW + 7], sYW);
+        TL(C, k) = Yk;
+    }
+    const double YN = 1.0 - sY;                               // closure: last species
+    TL(C, N - 1) = YN;
+    const double sW = fma(YN, spw[(N - 1) * kJobW + 7], sYW); // 1 / Wbar
+    const double Wbar = rcp_f(sW), invT = rcp_f(T);
+    const double rho = P * Wbar * invT * (1.0 / kRerg), inv_rho = kRerg * T * sW * invP;
+    const double lnT = T > 0.0 ? log_f(T) : nan_d();          // a Newton iterate may overshoot to T <= 0: failed step (R11)
+#pragma unroll 4
+    for (int k = 0; k < N; k++) TL(C, k) = rho * TL(C, k) * spw[k * kJobW + 7];
+    TL(C, N) = 1.0;                                           // unity factor of unused slots
+    const bool lo = T <= tmid;
+    const double *jt = tab + (lo ? kOffJobLo : kOffJobHi);
+    // mass-action part of every reaction: two exp jobs (k_f, k_r with K_c folded in) and three factors per side
+#pragma unroll 2
+    for (int i = 0; i < NR; i++) {
+        const double kf = exp_f(job_arg(jt + i * kJobW, T, lnT, invT));
+        const double kr = exp_f(job_arg(jt + (32 + i) * kJobW, T, lnT, invT));
+        const int sl = desc[i].x;
+        const double Rf = kf * (TL(C, min(sl & 31, N)) * TL(C, min((sl >> 5) & 31, N)) * TL(C, min((sl >> 10) & 31, N)));
+        const double Rr = kr * (TL(C, min((sl >> 15) & 31, N)) * TL(C, min((sl >> 20) & 31, N)) * TL(C, min((sl >> 25) & 31, N)));
+        TL(q, i) = Rf - Rr;
+    }
+    // third-body and falloff factors (the reaction type is uniform across the warp)
+    const double Ctot = P * invT * (1.0 / kRerg);
+    const double *eff_dv = tab + hdr[4];
+    const int *eff_sp = reinterpret_cast<const int *>(tab + hdr[5]);
+#pragma unroll 1
+    for (int i = 0; i < NR; i++) {
+        const int4 d0 = desc[i];
+        if (d0.z <= 0) continue;
+        const int4 d1 = desc[32 + i];
+        double cm = Ctot;
+#pragma unroll 1
+        for (int p = d1.x; p < d1.y; p++) cm = fma(eff_dv[p], TL(C, eff_sp[p]), cm);
+        if (d0.z >= 2) {
+            const double Pr = exp_f(job_arg(jt + (d0.w & 255) * kJobW, T, lnT, invT)) * cm;
+            double F = 1.0;
+            if (d0.z == 3) {
+                const double *c = jt + ((d0.w >> 8) & 255) * kJobW;
+                const double Fc = exp_f(job_arg(c, T, lnT, invT)) + exp_f(job_arg(c + kJobW, T, lnT, invT)) +
+                                  exp_f(job_arg(c + 2 * kJobW, T, lnT, invT));
+                const double lg = log_f(Fc) * kInvLn10, lPr = log_f(Pr) * kInvLn10;
+                const double At = lPr - 0.4 - 0.67 * lg;
+                const double x = At * rcp_f(0.75 - 1.27 * lg - 0.14 * At);
+                F = exp_f(kLn10 * lg * rcp_f(fma(x, x, 1.0)));
+            }
+            cm = Pr * rcp_f(1.0 + Pr) * F;
+        }
+        TL(q, i) *= cm;
+    }
+    // species production rates, temperature equation
+    const int2 *inc = reinterpret_cast<const int2 *>(tab + hdr[3]);
+    const double *spt = tab + (lo ? kOffSpLo : kOffSpHi);
+    double hw = 0.0, ccp = 0.0;
+#pragma unroll 1
+    for (int k = 0; k < N; k++) {
+        const int4 d1 = desc[32 + k];
+        double w0 = 0.0, w1 = 0.0;
+        int p = d1.z;
+#pragma unroll 2
+        for (; p + 1 < d1.w; p += 2) {
+            const int2 e0 = inc[p], e1 = inc[p + 1];
+            w0 = fma((double)e0.y, TL(q, e0.x), w0);
+            w1 = fma((double)e1.y, TL(q, e1.x), w1);
+        }
+        if (p < d1.w) { const int2 e0 = inc[p]; w0 = fma((double)e0.y, TL(q, e0.x), w0); }
+        const double w = w0 + w1;
+        const double *sc = spt + k * kJobW;
+        const double cpR = sc[0] + T * (sc[1] + T * (sc[2] + T * (sc[3] + T * sc[4])));
+        const double hRT = sc[0] + T * (sc[1] * 0.5 + T * (sc[2] * (1.0 / 3.0) + T * (sc[3] * 0.25 + T * (sc[4] * 0.2)))) + sc[5] * invT;
+        hw = fma(hRT, w, hw);
+        ccp = fma(TL(C, k), cpR, ccp);
+        if (k < N - 1) TL(out, k + 1) = sc[6] * w * inv_rho;
+    }
+    TL(out, 0) = -T * hw * rcp_f(ccp);
+}
+
+// ------------------------------------------------------------------------------------------------ analytical Jacobian
+// J[i*N + j] = d f_i / d y_j at y -> global gJ (R6; the formulation of warp_jacobian, chem_warp.cuh).  Pass 1
+// leaves four numbers per reaction (c k_f, -c k_r, dq/dT at constant C, dq/d[M]) in shared memory that is dead while a
+// Jacobian is evaluated; pass 2 builds d wdot_k / d C row by row in a lane-private row buffer, applies the chain rule
+// C -> (T, Y) and writes row k + 1 of J straight to global memory: N^2 global stores, no global read-modify-write.
+__device__ __noinline__ void jacobian(const double *tab, double *sm, double *gJ, int N, int NR, int oC, double tmid, double P,
+                                      double invP)
+{
+    const int *hdr = reinterpret_cast<const int *>(tab);
+    const int4 *desc = reinterpret_cast<const int4 *>(tab + kOffDesc);
+    const double *y = sm;
+    double *C = sm + oC * 32, *row = C + (N + 1) * 32, *S = row + (N + 1) * 32;
+    double *rd = sm + oZ(N) * 32;                              // [4][NR]
+    const double *spw = tab + kOffSpLo;
+    const double *eff_dv = tab + hdr[4];
+    const int *eff_sp = reinterpret_cast<const int *>(tab + hdr[5]);
+    const int2 *inc = reinterpret_cast<const int2 *>(tab + hdr[3]);
+    const double T = TL(y, 0);
+    double sY = 0.0, sYW = 0.0;
+#pragma unroll 4
+    for (int k = 0; k < N - 1; k++) {
+        const double Yk = TL(y, k + 1);
+        sY += Yk;
+        sYW = fma(Yk, spw[k * kJobW + 7], sYW);
+        TL(C, k) = Yk;
+    }
+    const double YN = 1.0 - sY;
+    TL(C, N - 1) = YN;
+    const double invWN = spw[(N - 1) * kJobW + 7];
+    const double sW = fma(YN, invWN, sYW);
+    const double Wbar = rcp_f(sW), invT = rcp_f(T);
+    const double rho = P * Wbar * invT * (1.0 / kRerg), inv_rho = kRerg * T * sW * invP;
+    const double lnT = T > 0.0 ? log_f(T) : nan_d();
+#pragma unroll 4
+    for (int k = 0; k < N; k++) TL(C, k) = rho * TL(C, k) * spw[k * kJobW + 7];
+    TL(C, N) = 1.0;
+    const bool lo = T <= tmid;
+    const double *jt = tab + (lo ? kOffJobLo : kOffJobHi);
+    const double Ctot = P * invT * (1.0 / kRerg);
+    // pass 1: per-reaction records
+#pragma unroll 1
+    for (int i = 0; i < NR; i++) {
+        const int4 d0 = desc[i];
+        const int sl = d0.x;
+        const double kf = exp_f(job_arg(jt + i * kJobW, T, lnT, invT));
+        const double kr = exp_f(job_arg(jt + (32 + i) * kJobW, T, lnT, invT));
+        const double dlnkf = job_darg(jt + i * kJobW, T, invT), dlnkr = job_darg(jt + (32 + i) * kJobW, T, invT);
+        const double Rf = kf * (TL(C, min(sl & 31, N)) * TL(C, min((sl >> 5) & 31, N)) * TL(C, min((sl >> 10) & 31, N)));
+        const double Rr = kr * (TL(C, min((sl >> 15) & 31, N)) * TL(C, min((sl >> 20) & 31, N)) * TL(C, min((sl >> 25) & 31, N)));
+        const double rnet = Rf - Rr;
+        double c = 1.0, dc_dT = 0.0, dc_dM = 0.0;
+        if (d0.z > 0) {
+            const int4 d1 = desc[32 + i];
+            double M = Ctot;
+#pragma unroll 1
+            for (int p = d1.x; p < d1.y; p++) M = fma(eff_dv[p], TL(C, eff_sp[p]), M);
+            c = M;
+            dc_dM = 1.0;
+            if (d0.z >= 2) {
+                const int ks = d0.w & 255;
+                const double k0k = exp_f(job_arg(jt + ks * kJobW, T, lnT, invT)), Pr = k0k * M;
+                const double dlnPr = job_darg(jt + ks * kJobW, T, invT);
+                double F = 1.0, dF_dT = 0.0, dF_dPr = 0.0;
+                if (d0.z == 3) {
+                    const double *cj = jt + ((d0.w >> 8) & 255) * kJobW;
+                    const double e3 = exp_f(job_arg(cj, T, lnT, invT)), e1 = exp_f(job_arg(cj + kJobW, T, lnT, invT));
+                    const double e2 = exp_f(job_arg(cj + 2 * kJobW, T, lnT, invT));
+                    const double Fc = e3 + e1 + e2;
+                    const double dFc = e3 * job_darg(cj, T, invT) + e1 * job_darg(cj + kJobW, T, invT) + e2 * job_darg(cj + 2 * kJobW, T, invT);
+                    const double L = log_f(Fc) * kInvLn10, dL = dFc * rcp_f(Fc) * kInvLn10;
+                    const double At = log_f(Pr) * kInvLn10 - 0.4 - 0.67 * L;
+                    const double Bt = 0.75 - 1.27 * L - 0.14 * At, rB = rcp_f(Bt);
+                    const double x = At * rB, rden = rcp_f(fma(x, x, 1.0));
+                    F = exp_f(kLn10 * L * rden);
+                    const double dA_T = dlnPr * kInvLn10 - 0.67 * dL, dB_T = -1.27 * dL - 0.14 * dA_T;
+                    const double dx_T = (dA_T * Bt - At * dB_T) * rB * rB;
+                    const double dx_P = rcp_f(Pr) * kInvLn10 * (Bt + 0.14 * At) * rB * rB;
+                    const double wF = -L * 2.0 * x * rden * rden;
+                    dF_dT = F * kLn10 * (dL * rden + wF * dx_T);
+                    dF_dPr = F * kLn10 * wF * dx_P;
+                }
+                const double op = rcp_f(1.0 + Pr);
+                c = Pr * op * F;
+                dc_dT = Pr * dlnPr * op * op * F + Pr * op * dF_dT;
+                dc_dM = (op * op * F + Pr * op * dF_dPr) * k0k;
+            }
+        }
+        TL(rd, i) = c * kf;
+        TL(rd, NR + i) = -c * kr;
+        TL(rd, 2 * NR + i) = dc_dT * rnet + c * (Rf * dlnkf - Rr * dlnkr);
+        TL(rd, 3 * NR + i) = d0.z > 0 ? dc_dM * rnet : 0.0;
+    }
+    // pass 2: rows
+    const double *spt = tab + (lo ? kOffSpLo : kOffSpHi);
+#pragma unroll 4
+    for (int j = 0; j < N; j++) TL(S, j) = 0.0;
+    double hw = 0.0, ccp = 0.0, cpw = 0.0, cdcp = 0.0;
+#pragma unroll 1
+    for (int k = 0; k < N; k++) {
+#pragma unroll 4
+        for (int l = 0; l <= N; l++) TL(row, l) = 0.0;
+        const int4 dk = desc[32 + k];
+        double wd = 0.0, dwT = 0.0, u = 0.0;
+#pragma unroll 1
+        for (int p = dk.z; p < dk.w; p++) {
+            const int2 e = inc[p];
+            const int i = e.x;
+            const double nu = (double)e.y;
+            const int4 e0 = desc[i];
+            const int sl = e0.x;
+            const int f0 = min(sl & 31, N), f1 = min((sl >> 5) & 31, N), f2 = min((sl >> 10) & 31, N);
+            const int f3 = min((sl >> 15) & 31, N), f4 = min((sl >> 20) & 31, N), f5 = min((sl >> 25) & 31, N);
+            const double c0 = TL(C, f0), c1 = TL(C, f1), c2 = TL(C, f2), c3 = TL(C, f3), c4 = TL(C, f4), c5 = TL(C, f5);
+            const double ckf = nu * TL(rd, i), ckr = nu * TL(rd, NR + i);
+            const double a12 = ckf * c1 * c2, b45 = ckr * c4 * c5;
+            wd += a12 * c0 + b45 * c3;                         // nu q_i
+            dwT = fma(nu, TL(rd, 2 * NR + i), dwT);
+            TL(row, f0) += a12;
+            TL(row, f1) += ckf * c0 * c2;
+            TL(row, f2) += ckf * c0 * c1;
+            TL(row, f3) += b45;
+            TL(row, f4) += ckr * c3 * c5;
+            TL(row, f5) += ckr * c3 * c4;
+            if (e0.z > 0) {
+                const int4 e1 = desc[32 + i];
+                const double vv = nu * TL(rd, 3 * NR + i);
+                u += vv;
+#pragma unroll 1
+                for (int pe = e1.x; pe < e1.y; pe++) TL(row, eff_sp[pe]) = fma(vv, eff_dv[pe], TL(row, eff_sp[pe]));
+            }
+        }
+        double GC = 0.0;
+#pragma unroll 4
+        for (int l = 0; l < N; l++) GC = fma(TL(row, l), TL(C, l), GC);
+        const double GN = TL(row, N - 1) * invWN;
+#pragma unroll 1
+        for (int j = N - 1; j >= 1; j--) {
+            const double iw = spw[(j - 1) * kJobW + 7];
+            TL(row, j) = -Wbar * (iw - invWN) * GC + rho * (TL(row, j - 1) * iw - GN);
+        }
+        TL(row, 0) = dwT - (GC + u * Ctot) * invT;
+        const double *sc = spt + k * kJobW;
+        const double cpR = sc[0] + T * (sc[1] + T * (sc[2] + T * (sc[3] + T * sc[4])));
+        const double dcpR = sc[1] + T * (2.0 * sc[2] + T * (3.0 * sc[3] + T * (4.0 * sc[4])));
+        const double hRT = sc[0] + T * (sc[1] * 0.5 + T * (sc[2] * (1.0 / 3.0) + T * (sc[3] * 0.25 + T * (sc[4] * 0.2)))) + sc[5] * invT;
+        const double Ck = TL(C, k);
+        hw = fma(hRT, wd, hw); ccp = fma(Ck, cpR, ccp); cpw = fma(cpR, wd, cpw); cdcp = fma(Ck, dcpR, cdcp);
+        const double Wr = sc[6] * inv_rho;
+#pragma unroll 2
+        for (int j = 0; j < N; j++) {
+            const double r = TL(row, j);
+            TL(S, j) = fma(hRT, r, TL(S, j));
+            if (k < N - 1) {
+                const double dlnrho = j == 0 ? -invT : -Wbar * (spw[(j - 1) * kJobW + 7] - invWN);
+                TL(gJ, (k + 1) * N + j) = Wr * (r - wd * dlnrho);
+            }
+        }
+    }
+    const double rccp = rcp_f(ccp);
+    const double Tdot = -T * hw * rccp;
+    const double cpN = spt[(N - 1) * kJobW] + T * (spt[(N - 1) * kJobW + 1] + T * (spt[(N - 1) * kJobW + 2] +
+                       T * (spt[(N - 1) * kJobW + 3] + T * spt[(N - 1) * kJobW + 4])));
+#pragma unroll 1
+    for (int j = 0; j < N; j++) {
+        double dlnrho, drcp;
+        if (j == 0) {
+            dlnrho = -invT;
+            drcp = -ccp * invT + cdcp;
+        } else {
+            const double *sc = spt + (j - 1) * kJobW;
+            const double iw = spw[(j - 1) * kJobW + 7];
+            const double cpj = sc[0] + T * (sc[1] + T * (sc[2] + T * (sc[3] + T * sc[4])));
+            dlnrho = -Wbar * (iw - invWN);
+            drcp = dlnrho * ccp + rho * (cpj * iw - cpN * invWN);
+        }
+        TL(gJ, j) = -(T * TL(S, j) + (j == 0 ? cpw : 0.0)) * rccp - Tdot * drcp * rccp;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ LU and solves
+// Both factorisations of a Radau step, left-looking, in one pass over the columns of J:
+//   E1 = fac1 I - J (real) and E2 = (alphn + i betan) I - J (complex), column-major in global memory, unit lower factor
+//   below the diagonal, U above it, the RECIPROCAL of the pivot on the diagonal; LAPACK row order (rows are swapped
+//   physically, only by the lanes that pivot off the diagonal), pivot rows packed four bits per step in ip1 / ip2.
+// Column j is loaded from J once, brought up to date in a lane-private shared-memory column (col: 3N entries) with the
+// finished columns k < j -- the same operations in the same order as right-looking elimination, but every factor entry
+// is written once -- then the pivot is searched (|re| + |im| for the complex matrix, first maximum wins: DESIGN.md R10).
+// Returns 0, or j + 1 if a matrix has no usable pivot in column j or J is not finite.
+__device__ __noinline__ int lu_pair(const double *gJ, double *g1, double2 *g2, double *col, int N, double fac1, double alphn,
+                                    double betan, u64 &ip1_out, u64 &ip2_out)
+{
+    double *c1 = col, *cr = col + N * 32, *ci = col + 2 * N * 32;
+    u64 ip1 = 0, ip2 = 0;
+    int ier = 0;
+#pragma unroll 1
+    for (int j = 0; j < N; j++) {
+        bool bad = false;
+#pragma unroll 4
+        for (int i = 0; i < N; i++) {
+            const double v = -TL(gJ, i * N + j);
+            bad |= !isfinite(v);
+            TL(c1, i) = v; TL(cr, i) = v; TL(ci, i) = 0.0;
+        }
+        TL(c1, j) += fac1; TL(cr, j) += alphn; TL(ci, j) = betan;
+        // interchanges of the finished steps
+#pragma unroll 1
+        for (int k = 0; k < j; k++) {
+            const int p1 = (int)(ip1 >> (4 * k)) & 15, p2 = (int)(ip2 >> (4 * k)) & 15;
+            if (p1 != k) { const double t = TL(c1, k); TL(c1, k) = TL(c1, p1); TL(c1, p1) = t; }
+            if (p2 != k) {
+                const double t = TL(cr, k), s = TL(ci, k);
+                TL(cr, k) = TL(cr, p2); TL(ci, k) = TL(ci, p2);
+                TL(cr, p2) = t; TL(ci, p2) = s;
+            }
+        }
+        // forward substitution with the finished columns
+#pragma unroll 1
+        for (int k = 0; k < j; k++) {
+            const double u1 = TL(c1, k), ur = TL(cr, k), ui = TL(ci, k);
+            const double *l1 = g1 + k * N * 32;
+            const double2 *l2 = g2 + k * N * 32;
+#pragma unroll 4
+            for (int i = k + 1; i < N; i++) {
+                const double a = TL(l1, i);
+                const double2 b = TL(l2, i);
+                TL(c1, i) = fma(-a, u1, TL(c1, i));
+                TL(cr, i) = fma(-b.x, ur, fma(b.y, ui, TL(cr, i)));
+                TL(ci, i) = fma(-b.x, ui, fma(-b.y, ur, TL(ci, i)));
+            }
+        }
+        // pivots
+        double best1 = -1.0, best2 = -1.0;
+        int p1 = j, p2 = j;
+#pragma unroll 1
+        for (int i = j; i < N; i++) {
+            const double v1 = fabs(TL(c1, i)), v2 = fabs(TL(cr, i)) + fabs(TL(ci, i));
+            if (v1 > best1) { best1 = v1; p1 = i; }
+            if (v2 > best2) { best2 = v2; p2 = i; }
+        }
+        if (!ier && (bad || !(best1 > 0.0) || !isfinite(best1) || !(best2 > 0.0) || !isfinite(best2))) ier = j + 1;
+        ip1 |= (u64)p1 << (4 * j);
+        ip2 |= (u64)p2 << (4 * j);
+        if (p1 != j) {
+            const double t = TL(c1, j); TL(c1, j) = TL(c1, p1); TL(c1, p1) = t;
+#pragma unroll 1
+            for (int k = 0; k < j; k++) { const double s = TL(g1, k * N + j); TL(g1, k * N + j) = TL(g1, k * N + p1); TL(g1, k * N + p1) = s; }
+        }
+        if (p2 != j) {
+            const double t = TL(cr, j), s = TL(ci, j);
+            TL(cr, j) = TL(cr, p2); TL(ci, j) = TL(ci, p2);
+            TL(cr, p2) = t; TL(ci, p2) = s;
+#pragma unroll 1
+            for (int k = 0; k < j; k++) { const double2 w = TL(g2, k * N + j); TL(g2, k * N + j) = TL(g2, k * N + p2); TL(g2, k * N + p2) = w; }
+        }
+        const double r1 = rcp_f(TL(c1, j));
+        const double pr = TL(cr, j), pi = TL(ci, j);
+        const double den = rcp_f(pr * pr + pi * pi);
+        const double qr = pr * den, qi = -pi * den;            // 1 / pivot
+        double *o1 = g1 + j * N * 32;
+        double2 *o2 = g2 + j * N * 32;
+#pragma unroll 4
+        for (int i = 0; i < N; i++) {
+            double a = TL(c1, i), br = TL(cr, i), bi = TL(ci, i);
+            if (i > j) {
+                a *= r1;
+                const double tr = br * qr - bi * qi, ti = br * qi + bi * qr;
+                br = tr; bi = ti;
+            } else if (i == j) {
+                a = r1; br = qr; bi = qi;
+            }
+            TL(o1, i) = a;
+            TL(o2, i) = make_double2(br, bi);
+        }
+    }
+    ip1_out = ip1;
+    ip2_out = ip2;
+    return ier;
+}
+
+__device__ __forceinline__ void apply_perm(double *b, int N, u64 ip)
+{
+#pragma unroll 1
+    for (int k = 0; k < N; k++) {
+        const int p = (int)(ip >> (4 * k)) & 15;
+        if (p != k) { const double t = TL(b, k); TL(b, k) = TL(b, p); TL(b, p) = t; }
+    }
+}
+
+// E1 x = b in place (b lane-private in shared memory)
+__device__ __noinline__ void solve_real(const double *g1, double *b, int N, u64 ip)
+{
+    apply_perm(b, N, ip);
+#pragma unroll 1
+    for (int i = 1; i < N; i++) {
+        double s = TL(b, i);
+#pragma unroll 4
+        for (int k = 0; k < i; k++) s = fma(-TL(g1, k * N + i), TL(b, k), s);
+        TL(b, i) = s;
+    }
+#pragma unroll 1
+    for (int i = N - 1; i >= 0; i--) {
+        double s = TL(b, i);
+#pragma unroll 4
+        for (int j = i + 1; j < N; j++) s = fma(-TL(g1, j * N + i), TL(b, j), s);
+        TL(b, i) = s * TL(g1, i * N + i);
+    }
+}
+
+// E1 x1 = b1 and E2 (x2 + i x3) = b2 + i b3 in place, one loop nest (three independent dependency chains)
+__device__ __noinline__ void solve3(const double *g1, const double2 *g2, double *b1, double *b2, double *b3, int N, u64 ip1, u64 ip2)
+{
+    apply_perm(b1, N, ip1);
+#pragma unroll 1
+    for (int k = 0; k < N; k++) {
+        const int p = (int)(ip2 >> (4 * k)) & 15;
+        if (p != k) {
+            const double t = TL(b2, k), s = TL(b3, k);
+            TL(b2, k) = TL(b2, p); TL(b3, k) = TL(b3, p);
+            TL(b2, p) = t; TL(b3, p) = s;
+        }
+    }
+#pragma unroll 1
+    for (int i = 1; i < N; i++) {
+        double s1 = TL(b1, i), sr = TL(b2, i), si = TL(b3, i);
+#pragma unroll 4
+        for (int k = 0; k < i; k++) {
+            const double a = TL(g1, k * N + i);
+            const double2 c = TL(g2, k * N + i);
+            const double x1 = TL(b1, k), xr = TL(b2, k), xi = TL(b3, k);
+            s1 = fma(-a, x1, s1);
+            sr = fma(-c.x, xr, fma(c.y, xi, sr));
+            si = fma(-c.x, xi, fma(-c.y, xr, si));
+        }
+        TL(b1, i) = s1; TL(b2, i) = sr; TL(b3, i) = si;
+    }
+#pragma unroll 1
+    for (int i = N - 1; i >= 0; i--) {
+        double s1 = TL(b1, i), sr = TL(b2, i), si = TL(b3, i);
+#pragma unroll 4
+        for (int j = i + 1; j < N; j++) {
+            const double a = TL(g1, j * N + i);
+            const double2 c = TL(g2, j * N + i);
+            const double x1 = TL(b1, j), xr = TL(b2, j), xi = TL(b3, j);
+            s1 = fma(-a, x1, s1);
+            sr = fma(-c.x, xr, fma(c.y, xi, sr));
+            si = fma(-c.x, xi, fma(-c.y, xr, si));
+        }
+        const double2 d = TL(g2, i * N + i);
+        TL(b1, i) = s1 * TL(g1, i * N + i);
+        TL(b2, i) = sr * d.x - si * d.y;
+        TL(b3, i) = sr * d.y + si * d.x;
+    }
+}
+
+}  // namespace tps
+}  // namespace chem

@@ -15,23 +15,6 @@
 
 namespace chem {
 
-constexpr int kJobW = 9;     // doubles per job row (7 used; 8 for species rows); ODD: lane-per-row reads are bank-conflict free
-constexpr int kJobs = 64;    // 2 rounds x 32 lanes
-// fixed part of the staged table blob (doubles)
-constexpr int kOffJobLo = 8, kOffJobHi = kOffJobLo + kJobs * kJobW, kOffSpLo = kOffJobHi + kJobs * kJobW;
-constexpr int kOffSpHi = kOffSpLo + 16 * kJobW, kOffDesc = kOffSpHi + 16 * kJobW;   // desc: 2 planes x 32 lanes x int4 = 128 doubles
-constexpr int kOffLists = kOffDesc + 128;
-
-// Tables of the fast path: one blob in global memory, staged into shared memory once per CTA.
-// blob[0..7] is a header of ints: {n_sp, n_rx, off_inc_nu, off_inc (int pairs), off_eff_dv, off_eff_sp, LD, n_falloff} (offsets in doubles).
-struct FastTables {
-    int enabled;
-    int n_sp, n_rx;
-    int blob_doubles;
-    double tmid;             // common NASA switch temperature
-    const double *blob;
-};
-
 __device__ __forceinline__ double warp_sum(double v)
 {
 #pragma unroll
@@ -55,16 +38,6 @@ __device__ __forceinline__ double pow_ni(double a, double b) { return exp_ni(b *
 // per-warp scratch layout (doubles), three stage slots each: C[3][32] (C[s][31] = 1 for unused factor slots),
 // E[3][64] exp-job results, q[3][32] rates of progress, X[48] stage parameters and phase-2 jobs; then matrices
 constexpr int kWsC = 0, kWsE = 96, kWsQ = kWsE + 3 * kJobs, kWsX = kWsQ + 96, kWsMat = kWsX + 48;
-
-// exponent of job row c at T and its temperature derivative
-__device__ __forceinline__ double job_arg(const double *c, double T, double lnT, double invT)
-{
-    return c[0] + c[1] * lnT + c[2] * invT + T * (c[3] + T * (c[4] + T * (c[5] + T * c[6])));
-}
-__device__ __forceinline__ double job_darg(const double *c, double T, double invT)
-{
-    return (c[1] - c[2] * invT) * invT + c[3] + T * (2.0 * c[4] + T * (3.0 * c[5] + T * (4.0 * c[6])));
-}
 
 // Mixture front end shared by the source term and the Jacobian: returns T, fills C[], E[] (exp jobs).
 struct WarpMix {

@@ -137,8 +137,8 @@ def test_integrate_matches_oracle(kind, dist, t_end, n, torch_cuda, gpu_mechs, o
     mech = descs(request)[kind]
     y0 = synth.make_states(mech, n, dist, synth.STATE_SEED)
     y_ref, st_ref, _ = orc_mechs[kind].integrate(y0, P, t_end, RTOL, ATOL)
-    # kernel 1 = generic shared-memory groups, kernel 2 = register-resident warp path (h2co only), 0 = auto
-    for kernel in ((1, 2, 0) if kind == "h2co" else (1, 0)):
+    # kernel 1 = shared-memory groups, 2 = warp per state, 3 = thread per state (2, 3: h2co only), 0 = auto
+    for kernel in ((1, 2, 3, 0) if kind == "h2co" else (1, 0)):
         y_dev, st = binding.chem_integrate_ex(gpu_mechs[kind], P, t_end, RTOL, ATOL, torch.from_numpy(y0).cuda(),
                                               kernel=kernel)
         torch.cuda.synchronize()
@@ -268,7 +268,7 @@ def test_results_are_reproducible_and_independent_of_the_batch(kind, n, torch_cu
     assert np.array_equal(y_h, y_a.cpu().numpy())
 
 
-@pytest.mark.parametrize("kind,n,kernels", [("h2co", 1500, (1, 2)), ("gri", 300, (0,))])
+@pytest.mark.parametrize("kind,n,kernels", [("h2co", 1500, (1, 2, 3)), ("gri", 300, (0,))])
 def test_finite_difference_jacobian_matches_oracle(kind, n, kernels, torch_cuda, gpu_mechs, orc_mechs, request):
     """PAPER.md L82 / Sec. 3.4: the CVODE-style FD Jacobian variant (R13) against the oracle's"""
     from paper_1607_03884_b200 import binding
@@ -297,7 +297,7 @@ def test_finite_difference_jacobian_matches_oracle(kind, n, kernels, torch_cuda,
         assert (st["njac"] == st_ref["njac"]).mean() >= 0.97
 
 
-@pytest.mark.parametrize("kind,n,kernels", [("h2co", 600, (1, 2)), ("gri", 60, (0,))])
+@pytest.mark.parametrize("kind,n,kernels", [("h2co", 600, (1, 2, 3)), ("gri", 60, (0,))])
 def test_fixed_step_mode_matches_oracle(kind, n, kernels, torch_cuda, gpu_mechs, orc_mechs, request):
     """solver-verification mode of PAPER.md L106-L128: a given number of equal internal steps, no error control"""
     from paper_1607_03884_b200 import binding
@@ -367,7 +367,7 @@ def test_tiny_mechanisms_every_reaction_type(rxn_type, torch_cuda):
     J, J_ref = binding.chem_jacobian(gm, P, yd).cpu().numpy(), om.jacobian(P, y0)
     assert np.all(np.abs(J - J_ref) <= 1e-9 * np.abs(J_ref).max(axis=1, keepdims=True) + 1e-300)
     y_ref, st_ref, _ = om.integrate(y0, P, 1e-3, RTOL, ATOL)
-    for kernel in (1, 2):
+    for kernel in (1, 2, 3):
         y, st = binding.chem_integrate_ex(gm, P, 1e-3, RTOL, ATOL, yd, kernel=kernel)
         compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
 
