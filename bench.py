@@ -2,9 +2,11 @@
 """bench.py -- states integrated per second over one global step (BASELINE.json metric).
 
 `python bench.py --gpus N --steps K --warmup W` : one "step" = one pass of the whole hot path
-(chem_integrate over the config's batch of synthetic states).  N = 1 workload: BASELINE.json
-configs[1] (h2co-shaped 13 species / 27 reactions, 1,048,576 states, dt = 1e-6 s).  N > 1: every rank
-integrates its own batch of that size (weak scaling, no collective on the data path).
+(chem_integrate over the config's batch of synthetic states).  The top-level line is BASELINE.json
+configs[1] (h2co-shaped 13 species / 27 reactions, 1,048,576 states, dt = 1e-6 s); at N = 1 the same line
+carries `"configs"`: the other four BASELINE.json configs, each timed the same way (device-resident and end to end)
+with its roofline fraction, failed-state count and the divergence measure D of PAPER.md Eq. 3.
+N > 1: every rank integrates its own batch of that size (weak scaling, no collective on the data path).
 `--impl reference` times the CPU oracle as it stands on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -22,14 +24,18 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_1607_03884_b200 import shard, synth  # noqa: E402
+from paper_1607_03884_b200 import diagnostics, shard, synth  # noqa: E402
 
 METRIC = "states integrated/sec per global step (fp64)"
 UNIT = "states/s"
-# ALU roofline: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
+# ALU roofline: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz; measured 36.3 TFLOP/s
+# (profiles/r2_fp64_peak.md)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram bytes per launch of integrate_kernel from the committed ncu --set full capture (profiles/), or None
-NCU_TRAFFIC_BYTES = {1: 115.299840e6 + 109.461760e6}   # profiles/r1_final_config1.md
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the integration kernel from the committed
+# `ncu --set full` captures, keyed by (config index, kernel id); None where no capture of that pair is on file.
+NCU_TRAFFIC = {
+    (1, 2): (115.299840e6 + 109.461760e6, "profiles/r1_final_config1.md"),
+}
 
 
 def load_peaks():
@@ -80,6 +86,16 @@ def algorithmic_flops(stats, fm):
     return s["nfcn"] * fm["rhs"] + s["njac"] * fm["jac"] + s["ndec"] * fm["lu"] + s["nsol"] * fm["newton"] + s["nstep"] * fm["err"]
 
 
+def config_dict(cfg, N, NR, world):
+    """the `config` object of a bench line: the same for the GPU arm and the reference arm"""
+    return {"workload": cfg["name"], "mechanism": f"{cfg['kind']}-shaped synthetic, {N} species / {NR} reactions",
+            "states_per_gpu": cfg["n_states"], "t_end": cfg["t_end"], "rtol": synth.RTOL, "atol": synth.ATOL, "P": synth.P_ATM,
+            "parallelism": f"batch sharded over {world} GPU(s), no collective",
+            "l2": f"inputs+outputs {2 * cfg['n_states'] * N * 8 / 1e6:.0f} MB per step"
+                  + (" exceed the 126 MB L2 (no flush)" if 2 * cfg["n_states"] * N * 8 > 126e6 else
+                     ": smaller than the 126 MB L2, a 256 MB buffer is written between timed steps (flush)")}
+
+
 def cpu_baseline(mech, cfg, y0, seconds_target=12.0):
     """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
     from oracle import oracle as orc
@@ -113,15 +129,109 @@ def run_reference(args, cfg, mech):
         _, _, cores = M.integrate(y0, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL)
     dt = time.perf_counter() - t0
     value = n * args.steps / dt
-    sample = f"first {n} states of the {cfg['n_states']}-state batch per step"
+    sample = (f"each step integrates the first {n} states of the {cfg['n_states']}-state batch of the workload "
+              f"(the metric is intensive: states/s)")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "states_per_step": n, "t_end": cfg["t_end"], "rtol": synth.RTOL, "atol": synth.ATOL},
+        "config": config_dict(cfg, int(mech["n_species"]), int(mech["n_reactions"]), max(args.gpus, 1)),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(cores), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+class Flusher:
+    """writes a buffer larger than the 126 MB L2 (timing rule for inputs smaller than L2)"""
+
+    def __init__(self, torch):
+        self.buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+
+    def __call__(self):
+        self.buf.fill_(1)
+
+
+def time_config(torch, binding, gm, mech, cfg, steps, warmup, kernel, rank, world, e2e_steps, sampler=None):
+    """Device-resident and end-to-end timing of one config; returns the measured numbers (rank-local reductions done)."""
+    n = cfg["n_states"]
+    N = gm.n_species
+    y0 = synth.make_states(mech, n, cfg["dist"], synth.STATE_SEED + rank)
+    y_dev = torch.from_numpy(y0).cuda()
+    y_out = torch.empty_like(y_dev)
+    y_pin = torch.from_numpy(y0).pin_memory()
+    y_out_pin = torch.empty(y_pin.shape, dtype=torch.float64, pin_memory=True)     # empty_like would not be pinned
+    flush = Flusher(torch) if 2 * n * N * 8 <= 126e6 else None
+    if kernel == 0:
+        run = lambda: binding.chem_integrate(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out)
+    else:
+        run = lambda: binding.chem_integrate_ex(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out,
+                                                want_stats=False, kernel=kernel)
+    # per-state counters for the flop model and the divergence measure (outside the timed region)
+    _, st = binding.chem_integrate_ex(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out, kernel=kernel)
+    torch.cuda.synchronize()
+    used_kernel = binding.chem_last_kernel(gm)
+    stats = binding.stats_to_numpy(st)
+    failed = int((stats["status"] != 0).sum())
+    flops_per_launch = algorithmic_flops(stats, gm.flop_model())
+    D = diagnostics.divergence_summary(stats["nstep"])
+    steps_hist = np.bincount(np.minimum(stats["nstep"], 64), minlength=65)
+
+    for _ in range(warmup):
+        run()
+    torch.cuda.synchronize()
+    if sampler is not None and rank == 0:
+        sampler.start()
+    shard.barrier()
+    torch.cuda.synchronize()
+    l0 = binding.chem_launch_count()
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    for i in range(steps):
+        if flush is not None:
+            flush()
+        ev0[i].record()
+        run()
+        ev1[i].record()
+    torch.cuda.synchronize()
+    shard.barrier()
+    launches = binding.chem_launch_count() - l0
+    clocks = sampler.stop() if (sampler is not None and rank == 0) else None
+    step_ms = np.array([ev0[i].elapsed_time(ev1[i]) for i in range(steps)])
+    total_s = float(step_ms.sum()) * 1e-3
+    total_s, units = shard.reduce_max_sum(total_s, float(n * steps), device="cuda")
+
+    # end to end through the C ABI with HOST (pinned) buffers: H2D + kernel + D2H inside the call
+    host = lambda: binding.chem_integrate_host(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_pin.numpy(),
+                                               y_out_pin.numpy(), kernel=kernel)
+    host()
+    shard.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        host()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_s, e2e_units = shard.reduce_max_sum(e2e_s, float(n * e2e_steps), device="cuda")
+    assert np.array_equal(y_out_pin.numpy(), y_out.cpu().numpy()), "host-buffer path disagrees with device path"
+    del y_dev, y_out, flush
+    torch.cuda.empty_cache()
+    return dict(n=n, N=N, total_s=total_s, units=units, kernel_s=float(step_ms.mean()) * 1e-3, launches=int(launches),
+                clocks=clocks, e2e_s=e2e_s, e2e_units=e2e_units, e2e_steps=e2e_steps, failed=failed,
+                flops_per_launch=flops_per_launch, D=D, used_kernel=used_kernel, y0=y0,
+                mean_steps=float(stats["nstep"].mean()), max_steps=int(stats["nstep"].max()),
+                steps_hist=[int(v) for v in steps_hist])
+
+
+def roofline(binding, ci, r, peaks, which):
+    achieved = r["flops_per_launch"] / r["kernel_s"] / 1e12
+    traffic = NCU_TRAFFIC.get((ci, r["used_kernel"]))
+    return {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+            "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic[0] if traffic else None,
+            "traffic_source": traffic[1] if traffic else None,
+            "kernel": binding.KERNEL_NAMES.get(r["used_kernel"], "?"), "kernel_ms": 1e3 * r["kernel_s"],
+            "flops_per_launch": r["flops_per_launch"],
+            "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7; measured 36.3, profiles/r2_fp64_peak.md)",
+            "hbm_frac": (2 * r["n"] * r["N"] * 8 / r["kernel_s"] / 1e9) / peaks["hbm_gbs"], "hbm_peak_source": which}
 
 
 def main():
@@ -130,9 +240,10 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs of the top-level line (default 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic shared-memory kernel, 2 warp kernel")
+    ap.add_argument("--only", action="store_true", help="time the top-level config only (no `configs` array)")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 group kernel, 2 warp per state, 3 thread per state")
     ap.add_argument("--states", type=int, default=0, help="profiling aid: use only the first N states of the config (not a bench line)")
     args = ap.parse_args()
     cfg = dict(synth.CONFIGS[args.config])
@@ -152,90 +263,57 @@ def main():
     torch.cuda.set_device(local_rank)
     shard.init_process_group("nccl")
     warmup = max(args.warmup, 3)
+    peaks, which = load_peaks()
 
-    n = cfg["n_states"]                          # per rank (weak scaling)
-    y0 = synth.make_states(mech, n, cfg["dist"], synth.STATE_SEED + rank)
-    gm = binding.chem_mech_load(mech)
-    N = gm.n_species
-    y_dev = torch.from_numpy(y0).cuda()
-    y_out = torch.empty_like(y_dev)
-    y_pin = torch.from_numpy(y0).pin_memory()
-    y_out_pin = torch.empty_like(y_pin)
-    if args.kernel == 0:
-        run = lambda: binding.chem_integrate(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out)
-    else:
-        run = lambda: binding.chem_integrate_ex(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out,
-                                                want_stats=False, kernel=args.kernel)
+    mechs, gms = {cfg["kind"]: mech}, {}
 
-    # per-state counters for the flop model (outside the timed region)
-    _, st = binding.chem_integrate_ex(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_dev, y_out)
-    torch.cuda.synchronize()
-    stats = binding.stats_to_numpy(st)
-    failed = int((stats["status"] != 0).sum())
-    flops_per_launch = algorithmic_flops(stats, gm.flop_model())
+    def gm_of(kind):
+        if kind not in mechs:
+            mechs[kind] = synth.make_mechanism(kind, synth.MECH_SEED)
+        if kind not in gms:
+            gms[kind] = binding.chem_mech_load(mechs[kind])
+        return gms[kind], mechs[kind]
 
-    for _ in range(warmup):
-        run()
-    torch.cuda.synchronize()
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
-    shard.barrier()
-    torch.cuda.synchronize()
-    l0 = binding.chem_launch_count()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    ev[0].record()
-    for i in range(args.steps):
-        run()
-        ev[i + 1].record()
-    torch.cuda.synchronize()
-    shard.barrier()
-    launches = binding.chem_launch_count() - l0
-    clocks = sampler.stop() if rank == 0 else None
-    step_ms = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)])
-    total_s = float(ev[0].elapsed_time(ev[-1])) * 1e-3
-    total_s, units = shard.reduce_max_sum(total_s, float(n * args.steps), device="cuda")
-
-    # end to end through the C ABI with HOST (pinned) buffers: H2D + kernel + D2H inside the call
-    e2e_steps = max(3, min(args.steps, 5))
-    binding.chem_integrate_host(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_pin.numpy(), y_out_pin.numpy())
-    shard.barrier()
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        binding.chem_integrate_host(gm, synth.P_ATM, cfg["t_end"], synth.RTOL, synth.ATOL, y_pin.numpy(), y_out_pin.numpy())
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    e2e_s, e2e_units = shard.reduce_max_sum(e2e_s, float(n * e2e_steps), device="cuda")
-    assert np.array_equal(y_out_pin.numpy(), y_out.cpu().numpy()), "host-buffer path disagrees with device path"
-
+    gm, _ = gm_of(cfg["kind"])
+    r = time_config(torch, binding, gm, mech, cfg, args.steps, warmup, args.kernel, rank, world,
+                    max(3, min(args.steps, 5)), sampler=ClockSampler(local_rank))
+    others = []
+    if world == 1 and not args.only and args.states == 0:
+        for ci, c in enumerate(synth.CONFIGS):
+            if ci == args.config:
+                continue
+            g2, m2 = gm_of(c["kind"])
+            steps2 = 20 if c["n_states"] <= 65536 else 3
+            r2 = time_config(torch, binding, g2, m2, c, steps2, 3, args.kernel, rank, world, 3)
+            others.append({
+                "index": ci, "workload": c["name"], "config": config_dict(c, r2["N"], g2.n_reactions, world),
+                "value": r2["units"] / r2["total_s"], "unit": UNIT, "steps": steps2, "warmup": 3,
+                "ms_per_step": 1e3 * r2["total_s"] / steps2, "us_per_state": 1e6 * r2["total_s"] / r2["units"],
+                "roofline": roofline(binding, ci, r2, peaks, which),
+                "e2e": {"value": r2["e2e_units"] / r2["e2e_s"], "unit": UNIT, "h2d_bytes_per_step": r2["n"] * r2["N"] * 8,
+                        "d2h_bytes_per_step": r2["n"] * r2["N"] * 8, "steps": r2["e2e_steps"], "host_memory": "pinned"},
+                "gpu_launches": r2["launches"], "failed_states": r2["failed"],
+                "internal_steps": {"mean": r2["mean_steps"], "max": r2["max_steps"]}, "D": r2["D"]})
+            del r2
     if rank != 0:
         return
-    peaks, which = load_peaks()
-    kernel_s = float(step_ms.mean()) * 1e-3
-    achieved = flops_per_launch / kernel_s / 1e12
+    n, N = r["n"], r["N"]
+    cdict = config_dict(cfg, N, gm.n_reactions, world)
+    cdict.update({"failed_states": r["failed"], "us_per_state": 1e6 * r["total_s"] / r["units"] * world})
     out = {
-        "metric": METRIC, "value": units / total_s, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
-        "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "mechanism": f"{cfg['kind']}-shaped synthetic, {N} species / {gm.n_reactions} reactions",
-                   "states_per_gpu": n, "t_end": cfg["t_end"], "rtol": synth.RTOL, "atol": synth.ATOL, "P": synth.P_ATM,
-                   "parallelism": f"batch sharded over {world} GPU(s), no collective",
-                   "l2": f"inputs+outputs {2 * n * N * 8 / 1e6:.0f} MB per step exceed the 126 MB L2 (no flush)",
-                   "failed_states": failed, "us_per_state": 1e6 * total_s / units * world},
-        "clocks": clocks,
-        "e2e": {"value": e2e_units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": n * N * 8, "d2h_bytes_per_step": n * N * 8,
-                "steps": e2e_steps, "host_memory": "pinned"},
-        "gpu_launches": int(launches),
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-                     "kernel": ("integrate_warp_kernel" if (N <= 16 and args.kernel != 1) else "integrate_kernel<128>"),
-                     "kernel_ms": 1e3 * kernel_s, "flops_per_launch": flops_per_launch,
-                     "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
-                     "hbm_frac": (2 * n * N * 8 / kernel_s / 1e9) / peaks["hbm_gbs"], "hbm_peak_source": which},
+        "metric": METRIC, "value": r["units"] / r["total_s"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
+        "ms_per_step": 1e3 * r["total_s"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": cdict, "clocks": r["clocks"],
+        "e2e": {"value": r["e2e_units"] / r["e2e_s"], "unit": UNIT, "h2d_bytes_per_step": n * N * 8, "d2h_bytes_per_step": n * N * 8,
+                "steps": r["e2e_steps"], "host_memory": "pinned"},
+        "gpu_launches": r["launches"],
+        "roofline": roofline(binding, args.config, r, peaks, which),
+        "internal_steps": {"mean": r["mean_steps"], "max": r["max_steps"]}, "D": r["D"],
     }
+    if others:
+        out["configs"] = others
     if world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(mech, cfg, y0)
+        out["cpu_baseline"] = cpu_baseline(mech, cfg, r["y0"])
     print(json.dumps(out))
 
 

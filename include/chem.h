@@ -25,7 +25,9 @@
  *     "host" pointers are ordinary host memory.  Nothing is retained after a
  *     call returns except inside the opaque chem_mech.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).
- *     Calls taking a stream are asynchronous with respect to the host.
+ *     Calls taking a stream are asynchronous with respect to the host.  Every launch takes its work-queue head and
+ *     scratch from the stream-ordered allocator (cudaMallocAsync on `stream`), so calls on different streams may run
+ *     concurrently with the same chem_mech.
  *   - there is NO CPU fallback: without a CUDA device every compute call fails
  *     with CHEM_E_CUDA.
  */
@@ -144,11 +146,12 @@ int chem_integrate(const chem_mech *mech, int32_t n_states, double P, double t_e
 int chem_integrate_ex(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
                       const double *y_in, double *y_out, const chem_opts *opts, chem_stats *stats, void *stream);
 
-/* End-to-end form with HOST buffers (the paper's timings include the transfers):
- * copies y_in to the device, integrates, copies y_out (and stats if not NULL) back, synchronises.  Large batches are
- * processed in chunks on two internal streams so that copies overlap kernels (pinned host memory makes the copies
- * asynchronous); the device staging buffer is cached in the mechanism object.  `reorder` is ignored here.
- * Not thread-safe per mechanism object. */
+/* End-to-end form with HOST buffers (the paper's timings include the transfers): integrates the states
+ * of y_in_host into y_out_host (and stats_host if not NULL) and synchronises.  Page-locked (pinned) buffers are read and
+ * written by the kernel itself through their device mapping, state by state, so the transfers overlap the integration;
+ * pageable buffers are staged through device memory in two chunks on two internal streams.  The buffers may alias.
+ * `reorder` is ignored here.  The internal streams belong to the mechanism object: one chem_integrate_host call per
+ * mechanism at a time. */
 int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
                         const double *y_in_host, double *y_out_host, const chem_opts *opts, chem_stats *stats_host);
 

@@ -430,7 +430,7 @@ extern "C" void chem_mech_free(chem_mech *m)
     if (!m) return;
     if (m->dev_blob) cudaFree(m->dev_blob);
     if (m->fast_blob) cudaFree(m->fast_blob);
-    for (int i = 0; i < 4; i++)
+    for (int i = 0; i < 2; i++)
         if (m->hs[i]) cudaStreamDestroy(m->hs[i]);
     delete m;
 }

@@ -31,7 +31,7 @@ struct chem_mech {
     chem::FastTables fast{};    // exp-job tables of the warp-per-state and thread-per-state paths, if eligible
     void *fast_blob = nullptr;
     // host-buffer entry point: two streams for chunked copy/compute overlap (created on first use)
-    cudaStream_t hs[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaStream_t hs[2] = {nullptr, nullptr};
     int last_kernel = 0;        // kernel id of the last chem_integrate* launch (chem_last_kernel)
 };
 

@@ -35,7 +35,8 @@ def descs(request):
 
 @pytest.mark.parametrize("kind,n", [("h2co", 203), ("gri", 67)])
 def test_rhs_matches_oracle(kind, n, torch_cuda, gpu_mechs, orc_mechs, request):
-    """relative 1e-12 on f, scaled per component by the largest contribution"""
+    """1e-10 x the per-state magnitude of the species source terms (1e-11 x the batch maximum); the
+    temperature equation against |f_T| + 1e5 x that magnitude"""
     from paper_1607_03884_b200 import binding
     torch = torch_cuda
     mech = descs(request)[kind]
@@ -52,7 +53,7 @@ def test_rhs_matches_oracle(kind, n, torch_cuda, gpu_mechs, orc_mechs, request):
 
 @pytest.mark.parametrize("kind,n", [("h2co", 101), ("gri", 37)])
 def test_jacobian_matches_oracle(kind, n, torch_cuda, gpu_mechs, orc_mechs, request):
-    """1e-10 column-scaled on J (the two sides use different but equivalent formulations)"""
+    """1e-9 x the column maximum of J (the two sides use different but equivalent formulations)"""
     from paper_1607_03884_b200 import binding
     torch = torch_cuda
     mech = descs(request)[kind]
@@ -232,6 +233,13 @@ def test_full_size_other_configs_sampled_against_oracle(ci, n_sample, torch_cuda
     y_ref, st_ref, _ = orc_mechs[cfg["kind"]].integrate(y0[idx], P, cfg["t_end"], RTOL, ATOL)
     assert np.all(st_ref["status"] == 0)
     assert np.all(np.abs(y1[idx] - y_ref) <= 1e-9 + 1e-6 * np.abs(y_ref))
+    # step counts of the sampled states (the same states through chem_integrate_ex; results do not depend on the batch)
+    y_s, st = binding.chem_integrate_ex(gpu_mechs[cfg["kind"]], P, cfg["t_end"], RTOL, ATOL, torch.from_numpy(y0[idx].copy()).cuda())
+    st = binding.stats_to_numpy(st)
+    assert np.array_equal(y_s.cpu().numpy(), y1[idx])
+    assert np.all(st["status"] == 0)
+    assert (st["naccpt"] == st_ref["naccpt"]).mean() >= 0.99
+    assert (st["nstep"] == st_ref["nstep"]).mean() >= 0.99
 
 
 @pytest.mark.parametrize("kind,n", [("h2co", 5000), ("gri", 300)])
@@ -315,7 +323,7 @@ def test_fixed_step_mode_matches_oracle(kind, n, kernels, torch_cuda, gpu_mechs,
             assert np.array_equal(st["naccpt"][fin], st_ref["naccpt"][fin]) and np.all(st["naccpt"][fin] == steps)
             y = y.cpu().numpy()
             ok = np.all(np.abs(y[fin] - y_ref[fin]) <= 1e-9 + 1e-6 * np.abs(y_ref[fin]), axis=1)
-            assert ok.mean() >= 0.99, (steps, kernel, ok.mean())
+            assert ok.all(), (steps, kernel, ok.mean())
 
 
 def test_fixed_step_convergence_like_fig2(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
@@ -405,3 +413,93 @@ def test_single_state_and_per_state_pressure(torch_cuda, gpu_mechs, orc_mechs, m
     for s in (0, 16, 32):
         yr, _, _ = orc_mechs["h2co"].integrate(y0[s:s + 1], float(Ps[s]), 1e-6, RTOL, ATOL)
         assert np.all(np.abs(y[s] - yr[0]) <= 1e-9 + 1e-6 * np.abs(yr[0]))
+
+
+def test_concurrent_launches_on_two_streams(torch_cuda, gpu_mechs, mech_h2co):
+    """include/chem.h: calls on different streams may run concurrently with the same chem_mech (every launch has its own
+    work-queue head and scratch).  Two different batches on two streams, interleaved several times, must give the bits
+    of sequential runs -- for every kernel."""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    m = gpu_mechs["h2co"]
+    ya = torch.from_numpy(synth.make_states(mech_h2co, 30011, "ignition", 101)).cuda()
+    yb = torch.from_numpy(synth.make_states(mech_h2co, 17003, "uniform", 102)).cuda()
+    for kernel in (1, 2, 3):
+        ref_a, sa = binding.chem_integrate_ex(m, P, 1e-5, RTOL, ATOL, ya, kernel=kernel)
+        ref_b, sb = binding.chem_integrate_ex(m, P, 1e-6, RTOL, ATOL, yb, kernel=kernel)
+        torch.cuda.synchronize()
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        outs = []
+        for rep in range(4):
+            oa, ta = binding.chem_integrate_ex(m, P, 1e-5, RTOL, ATOL, ya, kernel=kernel, stream=s1)
+            ob, tb = binding.chem_integrate_ex(m, P, 1e-6, RTOL, ATOL, yb, kernel=kernel, stream=s2)
+            outs.append((oa, ta, ob, tb))
+        torch.cuda.synchronize()
+        for oa, ta, ob, tb in outs:
+            assert torch.equal(oa, ref_a) and torch.equal(ob, ref_b), kernel
+            assert torch.equal(ta, sa) and torch.equal(tb, sb), kernel
+
+
+def test_divergence_measure_matches_oracle_definition(torch_cuda, gpu_mechs, mech_h2co):
+    """PAPER.md Eq. 3 (L190): the product-side D (paper_1607_03884_b200/diagnostics.py, reported by bench.py) against the
+    oracle's routine on the SAME per-state step counters taken from the GPU run; Eq. 1-2 likewise"""
+    from oracle import oracle as orc
+    from paper_1607_03884_b200 import binding, diagnostics
+    torch = torch_cuda
+    y0 = synth.make_states(mech_h2co, 4099, "ignition", 111)           # ragged: 128 complete warps + 3 states
+    y, st = binding.chem_integrate_ex(gpu_mechs["h2co"], P, 1e-4, RTOL, ATOL, torch.from_numpy(y0).cuda())
+    st = binding.stats_to_numpy(st)
+    D = diagnostics.divergence(st["nstep"])
+    D_ref = orc.divergence(st["nstep"])
+    assert D.shape == D_ref.shape == (128,)
+    assert np.array_equal(D, D_ref)
+    assert 0.0 <= D.min() and D.max() < 1.0 and D.mean() > 0.1            # dt = 1e-4: visibly divergent step counts
+    summ = diagnostics.divergence_summary(st["nstep"])
+    assert summ["warps"] == 128 and abs(sum(summ["hist"]) - 1.0) < 1e-3
+    y = y.cpu().numpy()
+    Emax, E = diagnostics.error_metric(y, y0, RTOL, ATOL)
+    Emax_ref, E_ref = orc.error_metric(y, y0, RTOL, ATOL)
+    assert np.allclose(E, E_ref, rtol=1e-13, atol=0.0) and np.isclose(Emax, Emax_ref, rtol=1e-13)
+
+
+def _backward_error(A, x, b):
+    """componentwise backward error of x for A x = b (Oettli-Prager): max_i |A x - b|_i / (|A| |x| + |b|)_i"""
+    return (np.abs(A @ x - b) / (np.abs(A) @ np.abs(x) + np.abs(b))).max()
+
+
+@pytest.mark.parametrize("ci", [1, 2])
+def test_linear_algebra_on_the_matrices_the_integrator_forms(ci, torch_cuda, gpu_mechs, mech_h2co):
+    """the device solve (n = 13: the warp path's pivoted Gauss-Jordan inverse) on the
+    WORST-conditioned matrices the integrator actually forms: E1 = gamma/h I - J and E2 = (alpha + i beta)/h I - J rebuilt
+    from chem_jacobian at the states of the config with h = h_last of their integration, ranked by condition number.
+    The bar is a componentwise BACKWARD error in units of u (DESIGN.md 8 states the measured worst case)."""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    cfg = synth.CONFIGS[ci]
+    m = gpu_mechs["h2co"]
+    y0 = synth.make_states(mech_h2co, 8192, cfg["dist"], synth.STATE_SEED)
+    yd = torch.from_numpy(y0).cuda()
+    y1, st = binding.chem_integrate_ex(m, P, cfg["t_end"], RTOL, ATOL, yd)
+    h = binding.stats_to_numpy(st)["h_last"]
+    J = np.concatenate([binding.chem_jacobian(m, P, yd).cpu().numpy(), binding.chem_jacobian(m, P, y1).cpu().numpy()])
+    h = np.concatenate([h, h])
+    U1, AL, BE = 3.637834252744495732, 2.681082873627752134, 3.050430199247410569
+    eye = np.eye(13)
+    E1 = (U1 / h)[:, None, None] * eye - J
+    E2 = ((AL + 1j * BE) / h)[:, None, None] * eye - J
+    cond = np.linalg.cond(E1)
+    worst = np.argsort(cond)[-256:]
+    rng = np.random.default_rng(5 + ci)
+    u = 2.0 ** -53
+    worst_eta = 0.0
+    for A in (E1[worst], E2[worst]):
+        b = rng.standard_normal((256, 13)) + (1j * rng.standard_normal((256, 13)) if np.iscomplexobj(A) else 0)
+        x, info = binding.chem_lu_solve(torch.from_numpy(np.ascontiguousarray(A)).cuda(), torch.from_numpy(b).cuda())
+        x, info = x.cpu().numpy(), info.cpu().numpy()
+        assert np.all(info == 0)
+        eta = max(_backward_error(A[s], x[s], b[s]) for s in range(256))
+        eta_ref = max(_backward_error(A[s], np.linalg.solve(A[s], b[s]), b[s]) for s in range(256))
+        worst_eta = max(worst_eta, eta)
+        print(f"config {ci} {'complex' if np.iscomplexobj(A) else 'real'}: cond up to {cond[worst].max():.2e}, "
+              f"backward error device {eta / u:.3g} u, LAPACK {eta_ref / u:.3g} u")
+    assert worst_eta <= 64 * u, worst_eta / u
