@@ -222,7 +222,12 @@ def time_config(torch, binding, gm, mech, cfg, steps, warmup, kernel, rank, worl
                 steps_hist=[int(v) for v in steps_hist])
 
 
+_probe = {}
+
+
 def roofline(binding, ci, r, peaks, which):
+    if "tf" not in _probe:
+        _probe["tf"] = binding.chem_fp64_probe()          # outside every timed region
     achieved = r["flops_per_launch"] / r["kernel_s"] / 1e12
     traffic = NCU_TRAFFIC.get((ci, r["used_kernel"]))
     return {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
@@ -230,7 +235,8 @@ def roofline(binding, ci, r, peaks, which):
             "traffic_source": traffic[1] if traffic else None,
             "kernel": binding.KERNEL_NAMES.get(r["used_kernel"], "?"), "kernel_ms": 1e3 * r["kernel_s"],
             "flops_per_launch": r["flops_per_launch"],
-            "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7; measured 36.3, profiles/r2_fp64_peak.md)",
+            "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7, profiles/r2_fp64_peak.md)",
+            "peak_measured_dfma_probe": _probe["tf"],
             "hbm_frac": (2 * r["n"] * r["N"] * 8 / r["kernel_s"] / 1e9) / peaks["hbm_gbs"], "hbm_peak_source": which}
 
 

@@ -167,6 +167,11 @@ int chem_last_kernel(const chem_mech *mech);
  * out[3] = one Newton iteration's solves and vector work (excluding its 3 source terms), out[4] = error estimate. */
 int chem_flop_model(const chem_mech *mech, double out[5]);
 
+/* Diagnostic, not on the hot path: the fp64 FMA rate of the device measured with dependent-free DFMA streams
+ * (`iters` fused multiply-adds x 8 accumulators per thread, 8 CTAs of 256 threads per SM, best of `reps` launches, in
+ * TFLOP/s); bench.py reports it beside the derived peak of the "alu" roofline. */
+int chem_fp64_probe(int32_t iters, int32_t reps, double *tflops_best);
+
 const char *chem_last_error(void);
 
 #ifdef __cplusplus

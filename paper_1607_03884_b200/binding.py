@@ -45,7 +45,7 @@ assert STATS_DTYPE.itemsize == 48
 
 EXPORTS = ["chem_mech_load", "chem_mech_free", "chem_mech_info", "chem_rhs", "chem_jacobian", "chem_lu_solve",
            "chem_integrate", "chem_integrate_ex", "chem_integrate_host", "chem_launch_count", "chem_flop_model",
-           "chem_last_error", "chem_last_kernel"]
+           "chem_last_error", "chem_last_kernel", "chem_fp64_probe"]
 
 _lib = None
 
@@ -76,6 +76,7 @@ def lib():
                                           C.c_void_p, C.c_void_p, C.POINTER(chem_opts), C.c_void_p]
         L.chem_flop_model.argtypes = [C.c_void_p, _dp]
         L.chem_last_kernel.argtypes = [C.c_void_p]
+        L.chem_fp64_probe.argtypes = [C.c_int32, C.c_int32, _dp]
         _lib = L
     return _lib
 
@@ -236,6 +237,13 @@ KERNEL_NAMES = {0: "none", 1: "integrate_kernel (group per state)", 2: "integrat
 
 def chem_last_kernel(mech: Mechanism) -> int:
     return int(lib().chem_last_kernel(mech._h))
+
+
+def chem_fp64_probe(iters: int = 1 << 16, reps: int = 5) -> float:
+    """measured fp64 FMA rate of the device in TFLOP/s (diagnostic; include/chem.h)"""
+    out = C.c_double(0.0)
+    _check(lib().chem_fp64_probe(iters, reps, C.byref(out)))
+    return float(out.value)
 
 
 def chem_launch_count() -> int:

@@ -310,3 +310,51 @@ extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, doub
     if (e != cudaSuccess) return fail(CHEM_E_CUDA, "chem_integrate_host: %s", cudaGetErrorString(e));
     return CHEM_OK;
 }
+
+// ------------------------------------------------------------------------------------------------ fp64 peak probe
+// Dependent-free DFMA streams (8 accumulators per thread, full occupancy): measures the fp64 FMA rate that the "alu"
+// roofline of DESIGN.md 7 is derived from (148 SM x 64 lanes x 2 flop x clock).  Diagnostic only, not on the hot path.
+namespace {
+__global__ void __launch_bounds__(256) fp64_probe_kernel(int iters, double seed, double *sink)
+{
+    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 1.0 - 1e-9, c = 1e-9;
+#pragma unroll 4
+    for (int i = 0; i < iters; i++) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (r == 12345.678) sink[0] = r;      // never true: keeps the loop alive
+}
+}  // namespace
+
+extern "C" int chem_fp64_probe(int32_t iters, int32_t reps, double *tflops_best)
+{
+    if (iters < 1 || reps < 1 || !tflops_best) return fail(CHEM_E_ARG, "bad argument");
+    int dev = 0, n_sm = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    double *sink = nullptr;
+    CUDA_TRY(cudaMalloc(&sink, 8));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0));
+    CUDA_TRY(cudaEventCreate(&e1));
+    const int grid = n_sm * 8;
+    double best = 0.0;
+    for (int r = 0; r < reps + 1; r++) {
+        cudaEventRecord(e0);
+        fp64_probe_kernel<<<grid, 256>>>(iters, 1.0, sink);
+        cudaEventRecord(e1);
+        g_launches++;
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaFree(sink); return fail(CHEM_E_CUDA, "fp64 probe: %s", cudaGetErrorString(e)); }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = (double)grid * 256 * 8 * 2.0 * iters / (ms * 1e-3) / 1e12;
+        if (r > 0 && tf > best) best = tf;       // the first launch is a warm-up
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    *tflops_best = best;
+    return CHEM_OK;
+}
