@@ -176,13 +176,16 @@ extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const
 
 namespace {
 // Kernel ids (chem_opts.kernel, chem_last_kernel): 1 shared-memory group kernel, 2 warp-per-state, 3 thread-per-state.
-// Auto picks the fastest measured mapping (profiles/r2_mapping_config1.md, r2_mapping_config2.md): the warp-per-state
-// kernel when the mechanism is eligible, else the group kernel; the thread-per-state kernel is chosen explicitly.
+// Auto picks the fastest measured mapping (profiles/r2_mapping_config1.md, r2_mapping_config2.md): for an eligible small
+// mechanism the thread-per-state kernel when the batch fills its lanes at least eight times over (it processes a state
+// in ~36 us of SM time against ~56 us for the warp-per-state kernel, but the end of a launch, when the queue is empty
+// and every warp waits for its slowest lanes, costs it ~6 ms more: break-even at ~300,000 states at dt = 1e-6 s), else
+// the warp-per-state kernel; the group kernel for everything else.
 int pick_kernel(const chem_mech *m, int n, const chem_opts *o)
 {
-    (void)n;
     const int want = o ? o->kernel : 0;
     if (want != 0) return want;
+    if (chem_tps_available(m) && (long long)n >= 8LL * chem_tps_slots(m)) return 3;
     if (warp_path_available(m)) return 2;
     return 1;
 }

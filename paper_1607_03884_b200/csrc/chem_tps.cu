@@ -10,11 +10,8 @@ using namespace chem::tps;
 
 namespace {
 
-constexpr int kTpsWarps = 4;                 // warps per CTA, one CTA per SM (shared memory bound)
-constexpr int kTpsBlock = 32 * kTpsWarps;
-
 struct TpsArgs {
-    int n_states, N, NR, oC, n_sm, n_gw;
+    int n_states, N, NR, n_sm, n_gw;
     double P, tmid;
     const double *P_per_state;
     RadauParams prm;
@@ -30,20 +27,24 @@ struct TpsArgs {
 
 enum Act { A_IDLE = 0, A_FREE, A_F0, A_JAC, A_FACT, A_STEP, A_NEWT, A_ERR };
 
-__global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __grid_constant__ TpsArgs a)
+// NT > 0: number of unknowns known at compile time (register-resident LU column and solve vectors, chem_tps.cuh);
+// NT = 0: any N <= 16 through the runtime-N routines.  WARPS: warps per CTA, one CTA per SM.
+template <int NT, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS, 1) integrate_tps_kernel(const __grid_constant__ TpsArgs a)
 {
     using namespace rk;
     extern __shared__ double smem[];
-    for (int i = threadIdx.x; i < a.blob_doubles; i += kTpsBlock) smem[i] = a.blob[i];   // stage the tables once per CTA
+    for (int i = threadIdx.x; i < a.blob_doubles; i += 32 * WARPS) smem[i] = a.blob[i];   // stage the tables once per CTA
     __syncthreads();
     const double *tab = smem;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int N = a.N, NR = a.NR, oC = a.oC;
+    const int N = NT > 0 ? NT : a.N, NR = a.NR;
     double *sm = smem + ((a.blob_doubles + 31) & ~31) + (size_t)wib * a.n_sm * 32 + lane;
-    double *gw = a.gws + ((size_t)blockIdx.x * kTpsWarps + wib) * (size_t)a.n_gw * 32 + lane;
+    double *gw = a.gws + ((size_t)blockIdx.x * WARPS + wib) * (size_t)a.n_gw * 32 + lane;
     double *gJ = gw, *g1 = gw + gE1(N) * 32, *gF = gw + gF0(N) * 32, *gC = gw + gCT(N) * 32, *gWv = gw + gW(N) * 32;
+    double *gAv = gw + gA(N) * 32, *gRd = gw + gR(N) * 32;
     double2 *g2 = reinterpret_cast<double2 *>(gw + gE2(N) * 32 - lane) + lane;
-    double *y = sm, *isc = sm + oIS(N) * 32, *z = sm + oZ(N) * 32, *av = sm + oA(N) * 32;
+    double *y = sm, *z = sm + oZ(N) * 32, *U = sm + oU(N) * 32;
 
     const RadauParams &prm = a.prm;
     const int NIT = prm.newton_max > 0 ? prm.newton_max : 7;
@@ -63,13 +64,14 @@ __global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __gri
     bool REJECT = false, FIRST = true, LAST = false, CALJAC = false;
     double H = 0, HOLD = 0, X = 0, FACCON = 1, THETA = 0, HACC = 0, ERRACC = 0, DYNOLD = 0, THQOLD = 0, h_last = 0;
     double P = a.P, invP = rcp_f(a.P);
-    u64 ip1 = 0, ip2 = 0;
+    u64 ip1 = 0, ip2 = 0;                    // pivots: sequence of interchanges (NT = 0) or permutation (NT > 0)
     bool exhausted = false;
 
-    // a finished state (or a failed one) leaves through here
+    // 1 / scal_i of DESIGN.md R8, recomputed where it is used (shared memory is what limits the resident warps)
+    auto iscal = [&](int i) { return rcp_f(ATOL + RTOL * fabs(TL(y, i))); };
+    // a finished state (or a failed one) leaves through here; its y is written out by the whole warp at the next refill
+    bool pend = false;
     auto retire = [&]() {
-#pragma unroll 1
-        for (int i = 0; i < N; i++) a.y_out[(size_t)sidx * N + i] = TL(y, i);
         if (a.stats) {
             chem_stats o;
             o.status = status; o.nstep = nstep; o.naccpt = naccpt; o.nrejct = nrejct; o.nfcn = nfcn;
@@ -77,40 +79,45 @@ __global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __gri
             o.h_last = h_last;
             a.stats[sidx] = o;
         }
+        pend = true;
         act = A_FREE;
+    };
+    auto solve_e1 = [&](double *b) {
+        if constexpr (NT > 0) solve_real_t<NT>(g1, b, ip1); else solve_real(g1, b, N, ip1);
     };
 
     for (;;) {
         // ------------------------------------------------------------------ simplified-Newton iterations (R10): the lanes
         // of the warp advance in lockstep by STEP ATTEMPTS; the iteration counts of one attempt differ little between
-        // states (about two, rarely more than four), so the lanes that converge early wait for few rounds
-        // while at least as many lanes want one as want something else (the few lanes that need a third, fourth, ...
-        // iteration carry on in the next round together with the lanes that start their next attempt then)
+        // states (about two, rarely more than four).  Rounds run while at least half as many lanes want one as want
+        // something else; the few lanes that need more carry on in the next rounds together with the lanes that start
+        // their next attempt then (running every attempt to its end costs 12 %: 60 % of the rounds then have <= 8 lanes).
         for (;;) {
         const int n_newt = __popc(__ballot_sync(0xffffffffu, act == A_NEWT));
         const int n_other = __popc(__ballot_sync(0xffffffffu, act != A_NEWT && act != A_IDLE));
-        if (n_newt == 0 || n_newt < n_other) break;
+        if (n_newt == 0 || 2 * n_newt < n_other) break;
+        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
         if (act == A_NEWT) {
             const double invH = rcp_f(H);
             const double FAC1 = U1 * invH, ALPHN = ALPH * invH, BETAN = BETA * invH;
 #pragma unroll 1
-            for (int s = 0; s < 3; s++) rhs(tab, sm, N, NR, oC, tmid, P, invP, oZ(N) + s * N, 1.0, oA(N) + s * N);
+            for (int s = 0; s < 3; s++) rhs(tab, sm, N, NR, tmid, P, invP, z + s * N * 32, 1.0, gAv + s * N * 32);
             nfcn += 3;
 #pragma unroll 2
             for (int i = 0; i < N; i++) {
-                const double a1 = TL(av, i), a2 = TL(av, N + i), a3 = TL(av, 2 * N + i);
+                const double a1 = TL(gAv, i), a2 = TL(gAv, N + i), a3 = TL(gAv, 2 * N + i);
                 const double w1 = TL(gWv, i), w2 = TL(gWv, N + i), w3 = TL(gWv, 2 * N + i);
                 TL(z, i) = TI11 * a1 + TI12 * a2 + TI13 * a3 - w1 * FAC1;
                 TL(z, N + i) = TI21 * a1 + TI22 * a2 + TI23 * a3 - w2 * ALPHN + w3 * BETAN;
                 TL(z, 2 * N + i) = TI31 * a1 + TI32 * a2 + TI33 * a3 - w3 * ALPHN - w2 * BETAN;
             }
-            solve3(g1, g2, z, z + N * 32, z + 2 * N * 32, N, ip1, ip2);
+            if constexpr (NT > 0) solve3_t<NT>(g1, g2, z, ip1, ip2); else solve3(g1, g2, z, z + N * 32, z + 2 * N * 32, N, ip1, ip2);
             nsol++;
             NEWT++;
             double dy = 0.0;
 #pragma unroll 2
             for (int i = 0; i < N; i++) {
-                const double d = TL(isc, i);
+                const double d = iscal(i);
                 const double q1 = TL(z, i) * d, q2 = TL(z, N + i) * d, q3 = TL(z, 2 * N + i) * d;
                 dy += q1 * q1 + q2 * q2 + q3 * q3;
             }
@@ -156,29 +163,30 @@ __global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __gri
         }
         }
         // ------------------------------------------------------------------ error estimate, step-size controller (R9)
+        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
         if (act == A_ERR) {
             const double invH = rcp_f(H);
-            double *a1 = av, *a2 = av + N * 32;
+            double *f2v = gAv + N * 32;                      // (dd1 z1 + dd2 z2 + dd3 z3) / h, kept for the second pass
 #pragma unroll 2
             for (int i = 0; i < N; i++) {
                 const double f2 = (DD1 * TL(z, i) + DD2 * TL(z, N + i) + DD3 * TL(z, 2 * N + i)) * invH;
-                TL(a2, i) = f2;
-                TL(a1, i) = f2 + TL(gF, i);
+                TL(f2v, i) = f2;
+                TL(U, i) = f2 + TL(gF, i);
             }
-            solve_real(g1, a1, N, ip1);
+            solve_e1(U);
             double e = 0.0;
 #pragma unroll 2
-            for (int i = 0; i < N; i++) { const double q = TL(a1, i) * TL(isc, i); e = fma(q, q, e); }
+            for (int i = 0; i < N; i++) { const double q = TL(U, i) * iscal(i); e = fma(q, q, e); }
             double ERR = fmax(sqrt_s(e * invN), 1.0e-10);
             if (ERR >= 1.0 && (FIRST || REJECT)) {
-                rhs(tab, sm, N, NR, oC, tmid, P, invP, oA(N), 1.0, oA(N) + 2 * N);       // f(y + cont) -> a3
+                rhs(tab, sm, N, NR, tmid, P, invP, U, 1.0, gAv + 2 * N * 32);            // f(y + cont); U is read first, then scratch
                 nfcn++;
 #pragma unroll 2
-                for (int i = 0; i < N; i++) TL(a1, i) = TL(av, 2 * N + i) + TL(a2, i);
-                solve_real(g1, a1, N, ip1);
+                for (int i = 0; i < N; i++) TL(U, i) = TL(gAv, 2 * N + i) + TL(f2v, i);
+                solve_e1(U);
                 e = 0.0;
 #pragma unroll 2
-                for (int i = 0; i < N; i++) { const double q = TL(a1, i) * TL(isc, i); e = fma(q, q, e); }
+                for (int i = 0; i < N; i++) { const double q = TL(U, i) * iscal(i); e = fma(q, q, e); }
                 ERR = fmax(sqrt_s(e * invN), 1.0e-10);
             }
             if (!isfinite(ERR)) {                                                         // R11
@@ -206,14 +214,12 @@ __global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __gri
 #pragma unroll 2
                     for (int i = 0; i < N; i++) {
                         const double z1 = TL(z, i), z2 = TL(z, N + i), z3 = TL(z, 2 * N + i);
-                        const double yn = TL(y, i) + z3;
-                        TL(y, i) = yn;
+                        TL(y, i) += z3;
                         const double k1 = (z2 - z3) * (1.0 / C2M1);
                         const double AK = (z1 - z2) * (1.0 / C1MC2);
                         const double ACONT3 = (AK - z1 * (1.0 / C1)) * (1.0 / C2);
                         const double k2 = (AK - k1) * (1.0 / C1M1);
                         TL(gC, i) = k1; TL(gC, N + i) = k2; TL(gC, 2 * N + i) = k2 - ACONT3;
-                        TL(isc, i) = rcp_f(ATOL + RTOL * fabs(yn));
                     }
                     CALJAC = false;
                     if (fixed ? (++fixed_done >= fixed) : LAST) {
@@ -245,8 +251,19 @@ __global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __gri
                 }
             }
         }
-        // ------------------------------------------------------------------ free lanes pull the next states
+        // ------------------------------------------------------------------ free lanes pull the next states.  States enter
+        // and leave as coalesced rows: the warp copies y of one state at a time between its row of y_in / y_out (N
+        // consecutive doubles, read or written by N lanes at once; these may be mapped host memory, chem_integrate_host) and
+        // the owning lane's column of shared memory.
         {
+            double *wsm = sm - lane;                                     // this warp's block: element e of lane l at wsm[e * 32 + l]
+            for (unsigned m = __ballot_sync(0xffffffffu, pend); m; m &= m - 1) {
+                const int l = __ffs(m) - 1;
+                const int s_out = __shfl_sync(0xffffffffu, sidx, l);
+                if (lane < N) a.y_out[(size_t)s_out * N + lane] = wsm[lane * 32 + l];
+            }
+            pend = false;
+            __syncwarp();
             const unsigned want = __ballot_sync(0xffffffffu, act == A_FREE);
             if (want) {
                 int base = 0;
@@ -256,79 +273,89 @@ __global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __gri
                     base = __shfl_sync(0xffffffffu, base, leader);
                     if (base + __popc(want) >= a.n_states) exhausted = true;
                 } else base = a.n_states;
+                bool fresh = false;
                 if (act == A_FREE) {
                     const int qi = base + __popc(want & ((1u << lane) - 1u));
                     if (qi >= a.n_states) act = A_IDLE;
-                    else {
-                        sidx = a.order ? a.order[qi] : qi;
-                        P = a.P_per_state ? a.P_per_state[sidx] : a.P;
-                        invP = rcp_f(P);
-                        bool bad = false;
+                    else { sidx = a.order ? a.order[qi] : qi; fresh = true; }
+                }
+                for (unsigned m = __ballot_sync(0xffffffffu, fresh); m; m &= m - 1) {
+                    const int l = __ffs(m) - 1;
+                    const int s_in = __shfl_sync(0xffffffffu, sidx, l);
+                    if (lane < N) wsm[lane * 32 + l] = a.y_in[(size_t)s_in * N + lane];
+                }
+                __syncwarp();
+                if (fresh) {
+                    P = a.P_per_state ? a.P_per_state[sidx] : a.P;
+                    invP = rcp_f(P);
+                    bool bad = false;
 #pragma unroll 1
-                        for (int i = 0; i < N; i++) {
-                            const double v = a.y_in[(size_t)sidx * N + i];
-                            bad |= !isfinite(v);
-                            TL(y, i) = v;
-                            TL(isc, i) = rcp_f(ATOL + RTOL * fabs(v));
-                        }
-                        status = 0; nstep = 0; naccpt = 0; nrejct = 0; nfcn = 0; njac = 0; ndec = 0; nsol = 0; nnewt_fail = 0;
-                        h_last = 0.0; NSING = 0; fixed_done = 0;
-                        if (bad || !(XEND > 0.0)) { status = -4; retire(); }              // stays free: pulls again next round
-                        else {
-                            X = 0.0;
-                            H = prm.h0 > 0.0 ? prm.h0 : XEND;
-                            if (fixed) H = XEND / fixed;
-                            H = fmin(H, XEND);
-                            HOLD = H;
-                            REJECT = false; FIRST = true; LAST = false; CALJAC = false;
-                            if (X + H * 1.0001 - XEND >= 0.0) { H = XEND - X; LAST = true; }
-                            FACCON = 1.0; THETA = 0.0; HACC = 0.0; ERRACC = 0.0;
-                            act = A_F0; nxt = A_JAC;
-                        }
+                    for (int i = 0; i < N; i++) bad |= !isfinite(TL(y, i));
+                    status = 0; nstep = 0; naccpt = 0; nrejct = 0; nfcn = 0; njac = 0; ndec = 0; nsol = 0; nnewt_fail = 0;
+                    h_last = 0.0; NSING = 0; fixed_done = 0;
+                    if (bad || !(XEND > 0.0)) { status = -4; retire(); }                  // written out and replaced in the next pass
+                    else {
+                        X = 0.0;
+                        H = prm.h0 > 0.0 ? prm.h0 : XEND;
+                        if (fixed) H = XEND / fixed;
+                        H = fmin(H, XEND);
+                        HOLD = H;
+                        REJECT = false; FIRST = true; LAST = false; CALJAC = false;
+                        if (X + H * 1.0001 - XEND >= 0.0) { H = XEND - X; LAST = true; }
+                        FACCON = 1.0; THETA = 0.0; HACC = 0.0; ERRACC = 0.0;
+                        act = A_F0; nxt = A_JAC;
                     }
                 }
             }
-            if (__all_sync(0xffffffffu, act == A_IDLE)) break;
+            // One CTA-wide barrier per pass: the warps of the CTA then run the same phase at about the same time, so one
+            // instruction-cache fill serves all of them (the kernel's code is ~130 KB; without the barrier the warps drift
+            // apart and 25-40 % of the stall samples are instruction fetches: profiles/r2_mapping_config1.md).  A warp
+            // whose lanes are all idle keeps arriving until every warp of the CTA is done.
+            if (__syncthreads_and(act == A_IDLE && !pend)) break;
         }
         // ------------------------------------------------------------------ f(y) of a new state or after an accepted step
+        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
         if (act == A_F0) {
-            rhs(tab, sm, N, NR, oC, tmid, P, invP, 0, 0.0, oA(N));
+            rhs(tab, sm, N, NR, tmid, P, invP, y, 0.0, gF);
             nfcn++;
-#pragma unroll 4
-            for (int i = 0; i < N; i++) TL(gF, i) = TL(av, i);
             act = nxt;
         }
         // ------------------------------------------------------------------ Jacobian
+        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
         if (act == A_JAC) {
             if (prm.fd_jacobian) {
                 // CVODE-style difference quotient (R13): column j = (f(y + inc_j e_j) - f(y)) / inc_j
+                double *pv = gAv + N * 32;
                 double fn = 0.0;
 #pragma unroll 1
-                for (int i = 0; i < N; i++) { const double r = TL(gF, i) * TL(isc, i); fn = fma(r, r, fn); TL(av, N + i) = 0.0; }
+                for (int i = 0; i < N; i++) { const double r = TL(gF, i) * iscal(i); fn = fma(r, r, fn); TL(pv, i) = 0.0; }
                 const double fnorm = sqrt_s(fn * invN);
                 const double minInc = (fnorm != 0.0) ? 1000.0 * fabs(H) * UROUND * N * fnorm : 1.0;
 #pragma unroll 1
                 for (int j = 0; j < N; j++) {
                     const double yj = TL(y, j);
                     const double inc = fmax(1.4901161193847656e-08 * fabs(yj), minInc * (ATOL + RTOL * fabs(yj)));
-                    TL(av, N + j) = inc;
-                    rhs(tab, sm, N, NR, oC, tmid, P, invP, oA(N) + N, 1.0, oA(N));
-                    TL(av, N + j) = 0.0;
+                    TL(pv, j) = inc;
+                    rhs(tab, sm, N, NR, tmid, P, invP, pv, 1.0, gAv);
+                    TL(pv, j) = 0.0;
 #pragma unroll 1
-                    for (int i = 0; i < N; i++) TL(gJ, i * N + j) = div_f(TL(av, i) - TL(gF, i), inc);
+                    for (int i = 0; i < N; i++) TL(gJ, i * N + j) = div_f(TL(gAv, i) - TL(gF, i), inc);
                 }
                 nfcn += N;
             } else {
-                jacobian(tab, sm, gJ, N, NR, oC, tmid, P, invP);
+                jacobian(tab, sm, gJ, gRd, N, NR, tmid, P, invP);
             }
             njac++;
             CALJAC = true;
             act = A_FACT;
         }
         // ------------------------------------------------------------------ E1, E2 and their LU
+        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
         if (act == A_FACT) {
             const double invH = rcp_f(H);
-            const int ier = lu_pair(gJ, g1, g2, av, N, U1 * invH, ALPH * invH, BETA * invH, ip1, ip2);
+            int ier;
+            if constexpr (NT > 0) ier = lu_pair_t<NT>(gJ, g1, g2, z, U1 * invH, ALPH * invH, BETA * invH, ip1, ip2);
+            else ier = lu_pair(gJ, g1, g2, z, N, U1 * invH, ALPH * invH, BETA * invH, ip1, ip2);
             ndec++;
             if (ier) {
                 NSING++;
@@ -340,6 +367,7 @@ __global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __gri
             } else act = A_STEP;
         }
         // ------------------------------------------------------------------ start of a step attempt
+        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
         if (act == A_STEP) {
             nstep++;
             if (nstep > NMAX) { status = -1; retire(); }
@@ -372,17 +400,34 @@ __global__ void __launch_bounds__(kTpsBlock, 1) integrate_tps_kernel(const __gri
     }
 }
 
+template <int NT, int WARPS>
+cudaError_t launch_tps(const TpsArgs &a, int grid, size_t smem, cudaStream_t st)
+{
+    cudaError_t e = cudaFuncSetAttribute(integrate_tps_kernel<NT, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    integrate_tps_kernel<NT, WARPS><<<grid, 32 * WARPS, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+size_t tps_smem(const chem_mech *m, int warps)
+{
+    const Lay L = make_lay(m->t.n_sp, m->t.n_rx);
+    return ((size_t)((m->fast.blob_doubles + 31) & ~31) + (size_t)warps * L.n_sm * 32) * sizeof(double);
+}
+int tps_warps(const chem_mech *m)
+{
+    return tps_smem(m, 8) <= (size_t)m->max_smem_optin ? 8 : 4;
+}
+
 }  // namespace
 
 int chem_tps_available(const chem_mech *m)
 {
     if (!m->fast.enabled) return 0;
-    const Lay L = make_lay(m->t.n_sp, m->t.n_rx);
-    const size_t smem = ((size_t)((m->fast.blob_doubles + 31) & ~31) + (size_t)kTpsWarps * L.n_sm * 32) * sizeof(double);
-    return smem <= (size_t)m->max_smem_optin;
+    return tps_smem(m, 4) <= (size_t)m->max_smem_optin;
 }
 
-int chem_tps_slots(const chem_mech *m) { return m->n_sm * kTpsBlock; }
+int chem_tps_slots(const chem_mech *m) { return m->n_sm * 32 * tps_warps(m); }
 
 int chem_tps_launch(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
                     const chem_opts *o, chem_stats *stats, const int *order, cudaStream_t st)
@@ -390,16 +435,16 @@ int chem_tps_launch(const chem_mech *m, int n, double P, const RadauParams &prm,
     using chem_host::fail;
     if (!chem_tps_available(m)) return fail(CHEM_E_UNSUPPORTED, "thread-per-state kernel not available for this mechanism");
     const Lay L = make_lay(m->t.n_sp, m->t.n_rx);
-    const size_t smem = ((size_t)((m->fast.blob_doubles + 31) & ~31) + (size_t)kTpsWarps * L.n_sm * 32) * sizeof(double);
-    CUDA_TRY(cudaFuncSetAttribute(integrate_tps_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int grid = (n + kTpsBlock - 1) / kTpsBlock;
+    const int warps = tps_warps(m);
+    const size_t smem = tps_smem(m, warps);
+    int grid = (n + 32 * warps - 1) / (32 * warps);
     if (grid > m->n_sm) grid = m->n_sm;                   // persistent: one CTA per SM, lanes pull states from the queue
-    const size_t ws_bytes = (size_t)grid * kTpsWarps * L.n_gw * 32 * sizeof(double);
+    const size_t ws_bytes = (size_t)grid * warps * L.n_gw * 32 * sizeof(double);
     void *scratch = nullptr;
     int rc = chem_host::scratch_alloc(&scratch, ws_bytes + 256, st);
     if (rc) return rc;
     TpsArgs a;
-    a.n_states = n; a.N = L.N; a.NR = L.NR; a.oC = L.oC; a.n_sm = L.n_sm; a.n_gw = L.n_gw;
+    a.n_states = n; a.N = L.N; a.NR = L.NR; a.n_sm = L.n_sm; a.n_gw = L.n_gw;
     a.P = P; a.tmid = m->fast.tmid;
     a.P_per_state = o ? o->P_per_state : nullptr;
     a.prm = prm;
@@ -410,9 +455,10 @@ int chem_tps_launch(const chem_mech *m, int n, double P, const RadauParams &prm,
     a.blob = m->fast.blob; a.blob_doubles = m->fast.blob_doubles;
     cudaError_t e = cudaMemsetAsync(a.counter, 0, sizeof(int), st);
     if (e == cudaSuccess) {
-        integrate_tps_kernel<<<grid, kTpsBlock, smem, st>>>(a);
+        const bool st13 = L.N == 13;       // compile-time-N instantiations (add sizes here and below as needed)
+        if (warps == 8) e = st13 ? launch_tps<13, 8>(a, grid, smem, st) : launch_tps<0, 8>(a, grid, smem, st);
+        else e = st13 ? launch_tps<13, 4>(a, grid, smem, st) : launch_tps<0, 4>(a, grid, smem, st);
         chem_host::g_launches++;
-        e = cudaGetLastError();
     }
     chem_host::scratch_free(scratch, st);
     if (e != cudaSuccess) return fail(CHEM_E_CUDA, "thread-per-state launch: %s", cudaGetErrorString(e));

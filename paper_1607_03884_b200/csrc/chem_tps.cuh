@@ -25,45 +25,44 @@ typedef unsigned long long u64;
 // lane-private element e of an array whose rows are 32 lanes wide
 #define TL(p, e) (p)[(e) * 32]
 
-// Shared-memory elements per lane: y[N], 1/scal[N], z1..z3[3N], a1..a3[3N], q[QL], C[N+1], row[N+1], S[N].
-// The Jacobian's per-reaction records (4 per reaction) alias z, a and q, which are dead then; QL >= N_rx makes them fit.
+// Shared-memory elements per lane: y[N], z1..z3[3N], C[N+1], U[max(N_rx, 2N+1)] (q of the source term; row and S of the
+// Jacobian); z doubles as the column scratch of the factorisation.  Global elements per lane (L2-resident workspace):
+// J[N^2], E1[N^2], E2[N^2] complex, f0[N], cont[3N], w1..w3[3N], a1..a3[3N], the Jacobian's reaction records[4 N_rx].
 struct Lay {
-    int N, NR, oC, n_sm;   // oC: offset of C; row = oC + N + 1; S = row + N + 1
-    int n_gw;              // global elements per lane: J[N^2], E1[N^2], E2[N^2] complex, f0[N], cont[3N], w1..w3[3N]
+    int N, NR, n_sm, n_gw;
 };
-__host__ __device__ inline Lay make_lay(int N, int NR)
-{
-    Lay L;
-    L.N = N; L.NR = NR;
-    const int need = 4 * NR, have = 6 * N + NR;
-    const int ql = NR + (need > have ? need - have : 0);
-    L.oC = 8 * N + ql;
-    L.n_sm = L.oC + (N + 1) + (N + 1) + N;
-    L.n_gw = 4 * N * N + 7 * N;
-    return L;
-}
-__host__ __device__ inline int oIS(int N) { return N; }
-__host__ __device__ inline int oZ(int N) { return 2 * N; }
-__host__ __device__ inline int oA(int N) { return 5 * N; }
-__host__ __device__ inline int oQ(int N) { return 8 * N; }
+__host__ __device__ inline int oZ(int N) { return N; }
+__host__ __device__ inline int oC(int N) { return 4 * N; }
+__host__ __device__ inline int oU(int N) { return 5 * N + 1; }
 __host__ __device__ inline int gE1(int N) { return N * N; }
 __host__ __device__ inline int gE2(int N) { return 2 * N * N; }   // in doubles; E2 is addressed as double2 from here
 __host__ __device__ inline int gF0(int N) { return 4 * N * N; }
 __host__ __device__ inline int gCT(int N) { return 4 * N * N + N; }
 __host__ __device__ inline int gW(int N) { return 4 * N * N + 4 * N; }
+__host__ __device__ inline int gA(int N) { return 4 * N * N + 7 * N; }
+__host__ __device__ inline int gR(int N) { return 4 * N * N + 10 * N; }
+__host__ __device__ inline Lay make_lay(int N, int NR)
+{
+    Lay L;
+    L.N = N; L.NR = NR;
+    L.n_sm = oU(N) + (NR > 2 * N + 1 ? NR : 2 * N + 1);
+    L.n_gw = gR(N) + 4 * NR;
+    return L;
+}
 
 __device__ __forceinline__ double nan_d() { return __longlong_as_double(0x7ff8000000000000LL); }
 
 // ------------------------------------------------------------------------------------------------ source term
 // f(T, Y; P) at the state y + vs * v (R1-R5; same mathematics as warp_rhs_body, chem_warp.cuh), all lane-private:
-// y = sm[0..N), v = sm[ov..), result -> sm[of..).  tab = staged table blob (shared, read with uniform indices).
-__device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, int oC, double tmid, double P, double invP,
-                                 int ov, double vs, int of)
+// y = sm[0..N), v and the result `out` anywhere (shared or global; v is consumed before the scratch is written).
+// tab = staged table blob (shared, read with uniform indices).
+__device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, double tmid, double P, double invP,
+                                 const double *v, double vs, double *out)
 {
     const int *hdr = reinterpret_cast<const int *>(tab);
     const int4 *desc = reinterpret_cast<const int4 *>(tab + kOffDesc);
-    const double *y = sm, *v = sm + ov * 32;
-    double *C = sm + oC * 32, *q = sm + oQ(N) * 32, *out = sm + of * 32;
+    const double *y = sm;
+    double *C = sm + oC(N) * 32, *q = sm + oU(N) * 32;
     const double *spw = tab + kOffSpLo;                       // W and 1/W are the same in both NASA ranges
     const double T = fma(vs, TL(v, 0), TL(y, 0));
     double sY = 0.0, sYW = 0.0;
@@ -152,17 +151,15 @@ __device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, i
 
 // ------------------------------------------------------------------------------------------------ analytical Jacobian
 // J[i*N + j] = d f_i / d y_j at y -> global gJ (R6; the formulation of warp_jacobian, chem_warp.cuh).  Pass 1
-// leaves four numbers per reaction (c k_f, -c k_r, dq/dT at constant C, dq/d[M]) in shared memory that is dead while a
-// Jacobian is evaluated; pass 2 builds d wdot_k / d C row by row in a lane-private row buffer, applies the chain rule
+// leaves four numbers per reaction (c k_f, -c k_r, dq/dT at constant C, dq/d[M]) in the lane's global workspace; pass 2 builds d wdot_k / d C row by row in a lane-private row buffer, applies the chain rule
 // C -> (T, Y) and writes row k + 1 of J straight to global memory: N^2 global stores, no global read-modify-write.
-__device__ __noinline__ void jacobian(const double *tab, double *sm, double *gJ, int N, int NR, int oC, double tmid, double P,
+__device__ __noinline__ void jacobian(const double *tab, double *sm, double *gJ, double *rd, int N, int NR, double tmid, double P,
                                       double invP)
 {
     const int *hdr = reinterpret_cast<const int *>(tab);
     const int4 *desc = reinterpret_cast<const int4 *>(tab + kOffDesc);
     const double *y = sm;
-    double *C = sm + oC * 32, *row = C + (N + 1) * 32, *S = row + (N + 1) * 32;
-    double *rd = sm + oZ(N) * 32;                              // [4][NR]
+    double *C = sm + oC(N) * 32, *row = sm + oU(N) * 32, *S = row + (N + 1) * 32;   // rd: [4][NR] in global memory
     const double *spw = tab + kOffSpLo;
     const double *eff_dv = tab + hdr[4];
     const int *eff_sp = reinterpret_cast<const int *>(tab + hdr[5]);
@@ -502,6 +499,161 @@ __device__ __noinline__ void solve3(const double *g1, const double2 *g2, double 
         TL(b2, i) = sr * d.x - si * d.y;
         TL(b3, i) = sr * d.y + si * d.x;
     }
+}
+
+// ------------------------------------------------------------------------------------------------ the same for a
+// compile-time N: the column of the factorisation and the right-hand sides of the solves live in REGISTERS (static
+// indices only), every global load has a compile-time offset and no dependence on the arithmetic (the compiler issues
+// them far ahead of their use: the loops of the runtime-N routines above stall on L2 latency), and the row
+// interchanges are carried as a permutation packed four bits per position (perm: position -> original row), applied
+// when a column of J is LOADED, so that finished columns never have to be permuted in registers.
+__device__ __forceinline__ u64 perm_swap(u64 perm, int a, int b)
+{
+    const u64 x = ((perm >> (4 * a)) ^ (perm >> (4 * b))) & 15ull;
+    return perm ^ (x << (4 * a)) ^ (x << (4 * b));
+}
+
+template <int N>
+__device__ __noinline__ int lu_pair_t(const double *gJ, double *g1, double2 *g2, double *col, double fac1, double alphn,
+                                      double betan, u64 &perm1_out, u64 &perm2_out)
+{
+    double *s1 = col, *sr = col + N * 32, *si = col + 2 * N * 32;
+    u64 perm1 = 0xFEDCBA9876543210ull, perm2 = 0xFEDCBA9876543210ull;
+    int ier = 0;
+#pragma unroll 1
+    for (int j = 0; j < N; j++) {
+        double c1[N], cr[N], ci[N];
+        bool bad = false;
+#pragma unroll
+        for (int i = 0; i < N; i++) {
+            const int r1 = (int)(perm1 >> (4 * i)) & 15, r2 = (int)(perm2 >> (4 * i)) & 15;
+            const double v1 = -TL(gJ, r1 * N + j), v2 = -TL(gJ, r2 * N + j);
+            bad |= !isfinite(v1);
+            c1[i] = r1 == j ? v1 + fac1 : v1;
+            cr[i] = r2 == j ? v2 + alphn : v2;
+            ci[i] = r2 == j ? betan : 0.0;
+        }
+#pragma unroll
+        for (int k = 0; k < N - 1; k++) {
+            if (k < j) {
+                const double u1 = c1[k], ur = cr[k], ui = ci[k];
+#pragma unroll
+                for (int i = k + 1; i < N; i++) {
+                    const double a = TL(g1, k * N + i);
+                    const double2 b = TL(g2, k * N + i);
+                    c1[i] = fma(-a, u1, c1[i]);
+                    cr[i] = fma(-b.x, ur, fma(b.y, ui, cr[i]));
+                    ci[i] = fma(-b.x, ui, fma(-b.y, ur, ci[i]));
+                }
+            }
+        }
+        double best1 = -1.0, best2 = -1.0;
+        int p1 = j, p2 = j;
+#pragma unroll
+        for (int i = 0; i < N; i++) {
+            const double v1 = fabs(c1[i]), v2 = fabs(cr[i]) + fabs(ci[i]);
+            TL(s1, i) = c1[i]; TL(sr, i) = cr[i]; TL(si, i) = ci[i];
+            if (i >= j && v1 > best1) { best1 = v1; p1 = i; }
+            if (i >= j && v2 > best2) { best2 = v2; p2 = i; }
+        }
+        if (!ier && (bad || !(best1 > 0.0) || !isfinite(best1) || !(best2 > 0.0) || !isfinite(best2))) ier = j + 1;
+        if (p1 != j) {
+            const double t = TL(s1, j); TL(s1, j) = TL(s1, p1); TL(s1, p1) = t;
+            perm1 = perm_swap(perm1, j, p1);
+#pragma unroll 2
+            for (int k = 0; k < j; k++) { const double s = TL(g1, k * N + j); TL(g1, k * N + j) = TL(g1, k * N + p1); TL(g1, k * N + p1) = s; }
+        }
+        if (p2 != j) {
+            const double t = TL(sr, j), s = TL(si, j);
+            TL(sr, j) = TL(sr, p2); TL(si, j) = TL(si, p2);
+            TL(sr, p2) = t; TL(si, p2) = s;
+            perm2 = perm_swap(perm2, j, p2);
+#pragma unroll 2
+            for (int k = 0; k < j; k++) { const double2 w = TL(g2, k * N + j); TL(g2, k * N + j) = TL(g2, k * N + p2); TL(g2, k * N + p2) = w; }
+        }
+        const double r1 = rcp_f(TL(s1, j));
+        const double pr = TL(sr, j), pi = TL(si, j);
+        const double den = rcp_f(pr * pr + pi * pi);
+        const double qr = pr * den, qi = -pi * den;            // 1 / pivot
+        double *o1 = g1 + j * N * 32;
+        double2 *o2 = g2 + j * N * 32;
+#pragma unroll
+        for (int i = 0; i < N; i++) {
+            double a = TL(s1, i), br = TL(sr, i), bi = TL(si, i);
+            if (i > j) {
+                a *= r1;
+                const double tr = br * qr - bi * qi, ti = br * qi + bi * qr;
+                br = tr; bi = ti;
+            } else if (i == j) {
+                a = r1; br = qr; bi = qi;
+            }
+            TL(o1, i) = a;
+            TL(o2, i) = make_double2(br, bi);
+        }
+    }
+    perm1_out = perm1;
+    perm2_out = perm2;
+    return ier;
+}
+
+// E1 x = b; b is read from `b` through the permutation and x written back to `b` (lane-private, shared memory)
+template <int N>
+__device__ __noinline__ void solve_real_t(const double *g1, double *b, u64 perm)
+{
+    double x[N];
+#pragma unroll
+    for (int i = 0; i < N; i++) x[i] = TL(b, (int)(perm >> (4 * i)) & 15);
+#pragma unroll
+    for (int i = 1; i < N; i++)
+#pragma unroll
+        for (int k = 0; k < i; k++) x[i] = fma(-TL(g1, k * N + i), x[k], x[i]);
+#pragma unroll
+    for (int i = N - 1; i >= 0; i--) {
+#pragma unroll
+        for (int j = i + 1; j < N; j++) x[i] = fma(-TL(g1, j * N + i), x[j], x[i]);
+        x[i] *= TL(g1, i * N + i);
+    }
+#pragma unroll
+    for (int i = 0; i < N; i++) TL(b, i) = x[i];
+}
+
+// E1 x1 = b1 and E2 (x2 + i x3) = b2 + i b3, right-hand sides and solutions in z = [b1 | b2 | b3] (shared memory)
+template <int N>
+__device__ __noinline__ void solve3_t(const double *g1, const double2 *g2, double *z, u64 perm1, u64 perm2)
+{
+    double x1[N], xr[N], xi[N];
+#pragma unroll
+    for (int i = 0; i < N; i++) {
+        const int r1 = (int)(perm1 >> (4 * i)) & 15, r2 = (int)(perm2 >> (4 * i)) & 15;
+        x1[i] = TL(z, r1); xr[i] = TL(z, N + r2); xi[i] = TL(z, 2 * N + r2);
+    }
+#pragma unroll
+    for (int i = 1; i < N; i++)
+#pragma unroll
+        for (int k = 0; k < i; k++) {
+            const double a = TL(g1, k * N + i);
+            const double2 c = TL(g2, k * N + i);
+            x1[i] = fma(-a, x1[k], x1[i]);
+            xr[i] = fma(-c.x, xr[k], fma(c.y, xi[k], xr[i]));
+            xi[i] = fma(-c.x, xi[k], fma(-c.y, xr[k], xi[i]));
+        }
+#pragma unroll
+    for (int i = N - 1; i >= 0; i--) {
+#pragma unroll
+        for (int j = i + 1; j < N; j++) {
+            const double a = TL(g1, j * N + i);
+            const double2 c = TL(g2, j * N + i);
+            x1[i] = fma(-a, x1[j], x1[i]);
+            xr[i] = fma(-c.x, xr[j], fma(c.y, xi[j], xr[i]));
+            xi[i] = fma(-c.x, xi[j], fma(-c.y, xr[j], xi[i]));
+        }
+        const double2 d = TL(g2, i * N + i);
+        x1[i] *= TL(g1, i * N + i);
+        const double tr = xr[i] * d.x - xi[i] * d.y, ti = xr[i] * d.y + xi[i] * d.x;
+        xr[i] = tr; xi[i] = ti;
+    }
+#pragma unroll
+    for (int i = 0; i < N; i++) { TL(z, i) = x1[i]; TL(z, N + i) = xr[i]; TL(z, 2 * N + i) = xi[i]; }
 }
 
 }  // namespace tps

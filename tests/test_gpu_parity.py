@@ -234,7 +234,8 @@ def test_full_size_other_configs_sampled_against_oracle(ci, n_sample, torch_cuda
     assert np.all(st_ref["status"] == 0)
     assert np.all(np.abs(y1[idx] - y_ref) <= 1e-9 + 1e-6 * np.abs(y_ref))
     # step counts of the sampled states (the same states through chem_integrate_ex; results do not depend on the batch)
-    y_s, st = binding.chem_integrate_ex(gpu_mechs[cfg["kind"]], P, cfg["t_end"], RTOL, ATOL, torch.from_numpy(y0[idx].copy()).cuda())
+    y_s, st = binding.chem_integrate_ex(gpu_mechs[cfg["kind"]], P, cfg["t_end"], RTOL, ATOL, torch.from_numpy(y0[idx].copy()).cuda(),
+                                        kernel=binding.chem_last_kernel(gpu_mechs[cfg["kind"]]))   # the kernel auto chose for the full batch
     st = binding.stats_to_numpy(st)
     assert np.array_equal(y_s.cpu().numpy(), y1[idx])
     assert np.all(st["status"] == 0)
