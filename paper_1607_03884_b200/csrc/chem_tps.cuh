@@ -52,6 +52,31 @@ __host__ __device__ inline Lay make_lay(int N, int NR)
 
 __device__ __forceinline__ double nan_d() { return __longlong_as_double(0x7ff8000000000000LL); }
 
+// exp(x) as exp_f (chem_math.cuh: same range reduction, same degree-13 Taylor polynomial, same tails) with the
+// polynomial evaluated by Estrin's scheme: a lane has only its own instruction stream to hide the 8-cycle DFMA latency
+// with, and Horner's rule is a chain of 13 dependent DFMAs; this is 5 levels deep for 4 more multiplications.
+__device__ __forceinline__ double exp_e(double x)
+{
+    const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);
+    const int n = __double2loint(t);
+    const double fn = t - 6755399441055744.0;
+    double r = fma(fn, -6.93147180369123816490e-01, x);
+    r = fma(fn, -1.90821492927058770002e-10, r);
+    const double r2 = r * r, r4 = r2 * r2, r8 = r4 * r4;
+    const double p01 = fma(kExpC[1], r, kExpC[0]), p23 = fma(kExpC[3], r, kExpC[2]), p45 = fma(kExpC[5], r, kExpC[4]);
+    const double p67 = fma(kExpC[7], r, kExpC[6]), p89 = fma(kExpC[9], r, kExpC[8]), pab = fma(kExpC[11], r, kExpC[10]);
+    const double pcd = fma(kExpC[13], r, kExpC[12]);
+    const double q0 = fma(p23, r2, p01), q1 = fma(p67, r2, p45), q2 = fma(pab, r2, p89);
+    const double s0 = fma(q1, r4, q0), s1 = fma(pcd, r4, q2);
+    double p = fma(s1, r8, s0);
+    const int n1 = n >> 1, n2 = n - n1;
+    p *= __hiloint2double((1023 + n1) << 20, 0);
+    p *= __hiloint2double((1023 + n2) << 20, 0);
+    if (x < -700.0) p = 0.0;
+    if (x > 709.0) p = __longlong_as_double(0x7ff0000000000000LL);
+    return p;
+}
+
 // ------------------------------------------------------------------------------------------------ source term
 // f(T, Y; P) at the state y + vs * v (R1-R5; same mathematics as warp_rhs_body, chem_warp.cuh), all lane-private:
 // y = sm[0..N), v and the result `out` anywhere (shared or global; v is consumed before the scratch is written).
@@ -84,15 +109,31 @@ __device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, d
     TL(C, N) = 1.0;                                           // unity factor of unused slots
     const bool lo = T <= tmid;
     const double *jt = tab + (lo ? kOffJobLo : kOffJobHi);
-    // mass-action part of every reaction: two exp jobs (k_f, k_r with K_c folded in) and three factors per side
-#pragma unroll 2
-    for (int i = 0; i < NR; i++) {
-        const double kf = exp_f(job_arg(jt + i * kJobW, T, lnT, invT));
-        const double kr = exp_f(job_arg(jt + (32 + i) * kJobW, T, lnT, invT));
-        const int sl = desc[i].x;
-        const double Rf = kf * (TL(C, min(sl & 31, N)) * TL(C, min((sl >> 5) & 31, N)) * TL(C, min((sl >> 10) & 31, N)));
-        const double Rr = kr * (TL(C, min((sl >> 15) & 31, N)) * TL(C, min((sl >> 20) & 31, N)) * TL(C, min((sl >> 25) & 31, N)));
-        TL(q, i) = Rf - Rr;
+    // mass-action part of every reaction: two exp jobs (k_f, k_r with K_c folded in) and three factors per side; two
+    // reactions per trip, all table and concentration reads before the stores, so that four exponentials overlap
+    {
+        auto ropa = [&](int i, double &kf_arg, double &kr_arg, double &pf, double &pr) {
+            kf_arg = job_arg(jt + i * kJobW, T, lnT, invT);
+            kr_arg = job_arg(jt + (32 + i) * kJobW, T, lnT, invT);
+            const int sl = desc[i].x;
+            pf = TL(C, min(sl & 31, N)) * TL(C, min((sl >> 5) & 31, N)) * TL(C, min((sl >> 10) & 31, N));
+            pr = TL(C, min((sl >> 15) & 31, N)) * TL(C, min((sl >> 20) & 31, N)) * TL(C, min((sl >> 25) & 31, N));
+        };
+        int i = 0;
+#pragma unroll 1
+        for (; i + 1 < NR; i += 2) {
+            double a0, b0, f0, r0, a1, b1, f1, r1;
+            ropa(i, a0, b0, f0, r0);
+            ropa(i + 1, a1, b1, f1, r1);
+            const double q0 = exp_e(a0) * f0 - exp_e(b0) * r0, q1 = exp_e(a1) * f1 - exp_e(b1) * r1;
+            TL(q, i) = q0;
+            TL(q, i + 1) = q1;
+        }
+        if (i < NR) {
+            double a0, b0, f0, r0;
+            ropa(i, a0, b0, f0, r0);
+            TL(q, i) = exp_e(a0) * f0 - exp_e(b0) * r0;
+        }
     }
     // third-body and falloff factors (the reaction type is uniform across the warp)
     const double Ctot = P * invT * (1.0 / kRerg);
@@ -107,16 +148,16 @@ __device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, d
 #pragma unroll 1
         for (int p = d1.x; p < d1.y; p++) cm = fma(eff_dv[p], TL(C, eff_sp[p]), cm);
         if (d0.z >= 2) {
-            const double Pr = exp_f(job_arg(jt + (d0.w & 255) * kJobW, T, lnT, invT)) * cm;
+            const double Pr = exp_e(job_arg(jt + (d0.w & 255) * kJobW, T, lnT, invT)) * cm;
             double F = 1.0;
             if (d0.z == 3) {
                 const double *c = jt + ((d0.w >> 8) & 255) * kJobW;
-                const double Fc = exp_f(job_arg(c, T, lnT, invT)) + exp_f(job_arg(c + kJobW, T, lnT, invT)) +
-                                  exp_f(job_arg(c + 2 * kJobW, T, lnT, invT));
+                const double Fc = exp_e(job_arg(c, T, lnT, invT)) + exp_e(job_arg(c + kJobW, T, lnT, invT)) +
+                                  exp_e(job_arg(c + 2 * kJobW, T, lnT, invT));
                 const double lg = log_f(Fc) * kInvLn10, lPr = log_f(Pr) * kInvLn10;
                 const double At = lPr - 0.4 - 0.67 * lg;
                 const double x = At * rcp_f(0.75 - 1.27 * lg - 0.14 * At);
-                F = exp_f(kLn10 * lg * rcp_f(fma(x, x, 1.0)));
+                F = exp_e(kLn10 * lg * rcp_f(fma(x, x, 1.0)));
             }
             cm = Pr * rcp_f(1.0 + Pr) * F;
         }
@@ -191,8 +232,8 @@ __device__ __noinline__ void jacobian(const double *tab, double *sm, double *gJ,
     for (int i = 0; i < NR; i++) {
         const int4 d0 = desc[i];
         const int sl = d0.x;
-        const double kf = exp_f(job_arg(jt + i * kJobW, T, lnT, invT));
-        const double kr = exp_f(job_arg(jt + (32 + i) * kJobW, T, lnT, invT));
+        const double kf = exp_e(job_arg(jt + i * kJobW, T, lnT, invT));
+        const double kr = exp_e(job_arg(jt + (32 + i) * kJobW, T, lnT, invT));
         const double dlnkf = job_darg(jt + i * kJobW, T, invT), dlnkr = job_darg(jt + (32 + i) * kJobW, T, invT);
         const double Rf = kf * (TL(C, min(sl & 31, N)) * TL(C, min((sl >> 5) & 31, N)) * TL(C, min((sl >> 10) & 31, N)));
         const double Rr = kr * (TL(C, min((sl >> 15) & 31, N)) * TL(C, min((sl >> 20) & 31, N)) * TL(C, min((sl >> 25) & 31, N)));
@@ -207,20 +248,20 @@ __device__ __noinline__ void jacobian(const double *tab, double *sm, double *gJ,
             dc_dM = 1.0;
             if (d0.z >= 2) {
                 const int ks = d0.w & 255;
-                const double k0k = exp_f(job_arg(jt + ks * kJobW, T, lnT, invT)), Pr = k0k * M;
+                const double k0k = exp_e(job_arg(jt + ks * kJobW, T, lnT, invT)), Pr = k0k * M;
                 const double dlnPr = job_darg(jt + ks * kJobW, T, invT);
                 double F = 1.0, dF_dT = 0.0, dF_dPr = 0.0;
                 if (d0.z == 3) {
                     const double *cj = jt + ((d0.w >> 8) & 255) * kJobW;
-                    const double e3 = exp_f(job_arg(cj, T, lnT, invT)), e1 = exp_f(job_arg(cj + kJobW, T, lnT, invT));
-                    const double e2 = exp_f(job_arg(cj + 2 * kJobW, T, lnT, invT));
+                    const double e3 = exp_e(job_arg(cj, T, lnT, invT)), e1 = exp_e(job_arg(cj + kJobW, T, lnT, invT));
+                    const double e2 = exp_e(job_arg(cj + 2 * kJobW, T, lnT, invT));
                     const double Fc = e3 + e1 + e2;
                     const double dFc = e3 * job_darg(cj, T, invT) + e1 * job_darg(cj + kJobW, T, invT) + e2 * job_darg(cj + 2 * kJobW, T, invT);
                     const double L = log_f(Fc) * kInvLn10, dL = dFc * rcp_f(Fc) * kInvLn10;
                     const double At = log_f(Pr) * kInvLn10 - 0.4 - 0.67 * L;
                     const double Bt = 0.75 - 1.27 * L - 0.14 * At, rB = rcp_f(Bt);
                     const double x = At * rB, rden = rcp_f(fma(x, x, 1.0));
-                    F = exp_f(kLn10 * L * rden);
+                    F = exp_e(kLn10 * L * rden);
                     const double dA_T = dlnPr * kInvLn10 - 0.67 * dL, dB_T = -1.27 * dL - 0.14 * dA_T;
                     const double dx_T = (dA_T * Bt - At * dB_T) * rB * rB;
                     const double dx_P = rcp_f(Pr) * kInvLn10 * (Bt + 0.14 * At) * rB * rB;
