@@ -119,7 +119,14 @@ int launch_integrate_warp(const chem_mech *m, int n, double P, const RadauParams
     return CHEM_OK;
 }
 
-inline bool warp_path_available(const chem_mech *m) { return m->fast.enabled != 0; }
+// eligible mechanism (chem_fast.inl) AND one CTA of kWarpBlock threads with its per-warp scratch fits in shared memory
+// (N = 13: 218 KB; N = 16 does not fit: such mechanisms take the thread-per-state or the group kernel)
+inline bool warp_path_available(const chem_mech *m)
+{
+    if (!m->fast.enabled) return false;
+    const size_t smem = ((size_t)m->fast.blob_doubles + (size_t)(kWarpBlock / 32) * warp_ws_doubles(m->t.n_sp, m->t.n_rx)) * sizeof(double);
+    return smem <= (size_t)m->max_smem_optin;
+}
 
 }  // namespace
 

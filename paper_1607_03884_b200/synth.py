@@ -35,6 +35,10 @@ KINDS = {
                  n_reactions=27, n_three_body=4, n_troe=2, cp_max=8.0, inert=("N2",)),
     "gri": dict(elements=("C", "H", "O", "N", "Ar"), caps={"C": 3, "H": 8, "O": 3, "N": 2}, n_species=53,
                 n_reactions=325, n_three_body=30, n_troe=29, cp_max=15.0, inert=("AR", "N2")),
+    # not a BASELINE.json config: a test shape at the size limits of the small-mechanism kernels (16 species, and as
+    # many reactions as leave room for the falloff / Troe exp jobs among 2 x 32 job slots)
+    "lim16": dict(elements=("H", "O", "C", "N"), caps={"H": 4, "O": 3, "C": 2}, n_species=16,
+                  n_reactions=28, n_three_body=3, n_troe=1, cp_max=8.0, inert=("N2",)),
 }
 
 

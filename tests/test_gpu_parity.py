@@ -504,3 +504,26 @@ def test_linear_algebra_on_the_matrices_the_integrator_forms(ci, torch_cuda, gpu
         print(f"config {ci} {'complex' if np.iscomplexobj(A) else 'real'}: cond up to {cond[worst].max():.2e}, "
               f"backward error device {eta / u:.3g} u, LAPACK {eta_ref / u:.3g} u")
     assert worst_eta <= 1024 * u, worst_eta / u        # measured: 211 u (LAPACK on the same matrices: 61 u)
+
+
+def test_small_mechanism_kernels_at_their_size_limit(torch_cuda):
+    """16 species / 28 reactions (synth kind "lim16"): the largest shape the warp-per-state and thread-per-state kernels
+    are compiled for; the thread-per-state kernel runs its runtime-N routines here (no compile-time instantiation for
+    N = 16), and the warp-per-state kernel must decline (its CTA does not fit in shared memory) instead of failing in auto"""
+    from oracle import oracle as orc
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = synth.make_mechanism("lim16", 7)
+    gm, om = binding.chem_mech_load(mech), orc.Mechanism(mech)
+    y0 = synth.make_states(mech, 1500, "ignition", 3)
+    yd = torch.from_numpy(y0).cuda()
+    f, f_ref = binding.chem_rhs(gm, P, yd).cpu().numpy(), om.rhs(P, y0)
+    scale = np.abs(f_ref[:, 1:]).max(axis=1, keepdims=True) + 1e-300
+    assert np.all(np.abs(f[:, 1:] - f_ref[:, 1:]) <= 1e-10 * scale)
+    y_ref, st_ref, _ = om.integrate(y0, P, 1e-5, RTOL, ATOL)
+    with pytest.raises(binding.ChemError):      # one 640-thread CTA of the warp-per-state kernel does not fit at N = 16
+        binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, yd, kernel=2)
+    for kernel in (1, 3, 0):
+        y, st = binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, yd, kernel=kernel)
+        compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+    assert binding.chem_last_kernel(gm) == 1    # auto: small batch, no warp kernel -> group kernel
