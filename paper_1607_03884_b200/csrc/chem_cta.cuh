@@ -96,7 +96,8 @@ __device__ __noinline__ void cta_rhs3(const Tables &tg, const ChemScratch &cs, c
         const double sW = vW + YN * __ldg(&t.invW[N - 1]);
         const double invT = 1.0 / T, rho = P / (kRerg * T * sW);
         double *o = x.X0 + 8 * s;
-        o[0] = T; o[1] = log_f(T); o[2] = invT; o[3] = rho; o[4] = kRerg * T * sW / P; o[5] = P * invT * (1.0 / kRerg);
+        o[0] = T; o[2] = invT; o[3] = rho; o[4] = kRerg * T * sW / P; o[5] = P * invT * (1.0 / kRerg);
+        o[1] = T > 0.0 ? log_f(T) : __longlong_as_double(0x7ff8000000000000LL);   // a stage T <= 0 is a failed step (R11), as with libm's log
         x.C3[64 * s + N - 1] = rho * YN * __ldg(&t.invW[N - 1]);
         x.C3[64 * s + 63] = 1.0;
     }

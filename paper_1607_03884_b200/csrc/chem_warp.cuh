@@ -66,7 +66,7 @@ __device__ __forceinline__ WarpMix warp_front(const double *tab, double *ws, dou
     m.invT = rcp_f(m.T);
     m.rho = P * m.Wbar * m.invT * (1.0 / kRerg);
     m.inv_rho = kRerg * m.T * sW * invP;
-    m.lnT = log_ni(m.T);
+    m.lnT = m.T > 0.0 ? log_ni(m.T) : __longlong_as_double(0x7ff8000000000000LL);
     m.Ck = m.rho * Yk * m.invWk;
     if (lane < N) C[lane] = m.Ck;
     m.jt = tab + (m.lo ? kOffJobLo : kOffJobHi);
@@ -129,7 +129,7 @@ __device__ __forceinline__ D3 warp_rhs_body(const double *tab, double *ws, doubl
 #pragma unroll
     for (int s = 1; s < NS; s++)
         if (sl3 == s) { Tsel = T[s]; Wsel = sW[s]; }
-    const double lnsel = log_f(Tsel);
+    const double lnsel = Tsel > 0.0 ? log_f(Tsel) : __longlong_as_double(0x7ff8000000000000LL);   // a stage T <= 0 is a failed step (R11), as with libm's log
     const double rsel = rcp_f((lane >= NS && lane < 2 * NS) ? Wsel : Tsel);
     double invT[NS], rho[NS], inv_rho[NS], Ck[NS];
 #pragma unroll

@@ -527,3 +527,17 @@ def test_small_mechanism_kernels_at_their_size_limit(torch_cuda):
         y, st = binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, yd, kernel=kernel)
         compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
     assert binding.chem_last_kernel(gm) == 1    # auto: small batch, no warp kernel -> group kernel
+
+
+def test_newton_iterates_with_nonpositive_temperature(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
+    """a huge first step (h0 = t_end = 1e-2 s on ignition states) drives Newton iterates to T <= 0; log T is
+    then NaN on every path (libm in the oracle and the generic source term, an explicit guard around the compact log in
+    the stage-batched ones), the step is rejected (R11) and every kernel takes the oracle's step sequence."""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    y0 = synth.make_states(mech_h2co, 2000, "ignition", 121)
+    y_ref, st_ref, _ = orc_mechs["h2co"].integrate(y0, P, 1e-2, RTOL, ATOL)
+    assert st_ref["nnewt_fail"].sum() > 500                 # the case does exercise failed Newton iterations
+    for kernel in (1, 2, 3):
+        y, st = binding.chem_integrate_ex(gpu_mechs["h2co"], P, 1e-2, RTOL, ATOL, torch.from_numpy(y0).cuda(), kernel=kernel)
+        compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
