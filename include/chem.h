@@ -98,12 +98,14 @@ typedef struct chem_opts {
     int32_t fd_jacobian; /* 1: first-order finite-difference Jacobian "based on that of CVODE" (Sec. 3.4;
                             DESIGN.md R13) instead of the analytical one; costs N extra source terms per Jacobian */
     int32_t fixed_steps; /* > 0: take exactly this many equal internal steps without error control (the solver-verification
-                            experiment of PAPER.md L106-L128, Fig. 2); 0: adaptive (default) */
+                            experiment of PAPER.md L106-L128, Fig. 2); a step that cannot be taken ends the state with
+                            status -5 (R14); 0: adaptive (default) */
 } chem_opts;
 
 /* Per-state result record written by chem_integrate_ex (device array of n_states). */
 typedef struct chem_stats {
-    int32_t status;     /* 0 ok; -1 max_steps exceeded; -2 step size too small; -3 singular matrix 5x; -4 non-finite input */
+    int32_t status;     /* 0 ok; -1 max_steps exceeded; -2 step size too small; -3 singular matrix 5x; -4 non-finite input;
+                           -5 fixed_steps mode: a step could not be taken (singular matrix or non-finite iterate) */
     int32_t nstep;      /* internal step attempts that reached the Newton loop (d_i of PAPER.md Eq. 3) */
     int32_t naccpt;     /* accepted steps                                                              */
     int32_t nrejct;     /* error-test rejections (after the first accepted step)                       */

@@ -763,6 +763,7 @@ next_step:                                          /* label 30 */
         }
     }
 unexpected_rejection:                               /* label 78 */
+    if (fixed) { st->status = -5; goto done; }      /* DESIGN.md R14: a fixed step that cannot be taken ends the state */
     H = H * 0.5;
     REJECT = 1;
     LAST = 0;

@@ -173,6 +173,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
             if (ier) {
                 NSING++;
                 if (NSING >= 5) { st.status = -3; return; }
+                if (fixed) { st.status = -5; return; }             // DESIGN.md R14
                 H *= 0.5; REJECT = true; LAST = false;
                 next = CALJAC ? DO_FACT : DO_JAC;
                 continue;
@@ -281,6 +282,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
         }
         if (outcome != 0) {
             st.nnewt_fail++;
+            if (fixed) { st.status = -5; return; }                 // DESIGN.md R14 (only a non-finite iterate gets here)
             if (outcome == 2) H *= 0.5;
             REJECT = true; LAST = false;
             next = CALJAC ? DO_FACT : DO_JAC;
@@ -316,6 +318,7 @@ __device__ void radau_state(const Tables &t, const Work &w, double P, const Rada
             }
         }
         if (!isfinite(ERR)) {                                                             // DESIGN.md R11
+            if (fixed) { st.status = -5; return; }                 // DESIGN.md R14
             H *= 0.5; REJECT = true; LAST = false;
             next = CALJAC ? DO_FACT : DO_JAC;
             continue;

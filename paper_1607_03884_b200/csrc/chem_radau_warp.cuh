@@ -154,6 +154,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             if (__builtin_expect(ier != 0, 0)) {
                 NSING++;
                 if (NSING >= 5) { st.status = -3; return; }
+                if (fixed) { st.status = -5; return; }             // DESIGN.md R14
                 H *= 0.5; REJECT = true; LAST = false;
                 next = CALJAC ? DO_FACT : DO_JAC;
                 continue;
@@ -238,6 +239,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
         }
         if (__builtin_expect(outcome != 0, 0)) {
             st.nnewt_fail++;
+            if (fixed) { st.status = -5; return; }                 // DESIGN.md R14 (only a non-finite iterate gets here)
             if (outcome == 2) H *= 0.5;
             REJECT = true; LAST = false;
             next = CALJAC ? DO_FACT : DO_JAC;
@@ -262,6 +264,7 @@ __device__ void radau_state_warp(const Tables &t, const double *tab, double *ws,
             }
         }
         if (__builtin_expect(!isfinite(ERR), 0)) {
+            if (fixed) { st.status = -5; return; }                 // DESIGN.md R14
             H *= 0.5; REJECT = true; LAST = false;
             next = CALJAC ? DO_FACT : DO_JAC;
             continue;

@@ -157,9 +157,12 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
             }
             if (outcome != 0) {
                 nnewt_fail++;
-                if (outcome == 2) H *= 0.5;
-                REJECT = true; LAST = false;
-                act = CALJAC ? A_FACT : A_JAC;
+                if (fixed) { status = -5; retire(); }                                     // R14 (only a non-finite iterate gets here)
+                else {
+                    if (outcome == 2) H *= 0.5;
+                    REJECT = true; LAST = false;
+                    act = CALJAC ? A_FACT : A_JAC;
+                }
             }
         }
         }
@@ -191,8 +194,11 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
                 ERR = fmax(sqrt_s(e * invN), 1.0e-10);
             }
             if (!isfinite(ERR)) {                                                         // R11
-                H *= 0.5; REJECT = true; LAST = false;
-                act = CALJAC ? A_FACT : A_JAC;
+                if (fixed) { status = -5; retire(); }                                     // R14
+                else {
+                    H *= 0.5; REJECT = true; LAST = false;
+                    act = CALJAC ? A_FACT : A_JAC;
+                }
             } else {
                 if (fixed) ERR = 0.5;
                 const double FAC = fmin(SAFE, div_f(CFAC, (double)(NEWT + 2 * NIT)));
@@ -361,6 +367,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
             if (ier) {
                 NSING++;
                 if (NSING >= 5) { status = -3; retire(); }
+                else if (fixed) { status = -5; retire(); }                                // R14
                 else {
                     H *= 0.5; REJECT = true; LAST = false;
                     act = CALJAC ? A_FACT : A_JAC;
