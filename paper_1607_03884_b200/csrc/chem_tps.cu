@@ -28,7 +28,8 @@ struct TpsArgs {
 enum Act { A_IDLE = 0, A_FREE, A_F0, A_JAC, A_FACT, A_STEP, A_NEWT, A_ERR };
 
 // NT > 0: number of unknowns known at compile time (register-resident LU column and solve vectors, chem_tps.cuh);
-// NT = 0: any N <= 16 through the runtime-N routines.  WARPS: warps per CTA, one CTA per SM.
+// NT = 0: any N <= 16 through the runtime-N routines.  WARPS: warps per CTA; 8 / WARPS CTAs per SM (8 warps: 93 doubles of
+// shared memory per lane at N = 13).
 template <int NT, int WARPS>
 __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(const __grid_constant__ TpsArgs a)
 {
@@ -97,7 +98,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
         const int n_newt = __popc(__ballot_sync(0xffffffffu, act == A_NEWT));
         const int n_other = __popc(__ballot_sync(0xffffffffu, act != A_NEWT && act != A_IDLE));
         if (n_newt == 0 || 2 * n_newt < n_other) break;
-        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
+        __syncwarp();                              // every phase starts with the warp converged (chem_tps.cuh, header)
         if (act == A_NEWT) {
             const double invH = rcp_f(H);
             const double FAC1 = U1 * invH, ALPHN = ALPH * invH, BETAN = BETA * invH;
@@ -167,7 +168,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
         }
         }
         // ------------------------------------------------------------------ error estimate, step-size controller (R9)
-        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
+        __syncwarp();                              // every phase starts with the warp converged (chem_tps.cuh, header)
         if (act == A_ERR) {
             const double invH = rcp_f(H);
             double *f2v = gAv + N * 32;                      // (dd1 z1 + dd2 z2 + dd3 z3) / h, kept for the second pass
@@ -321,14 +322,14 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
             if (__syncthreads_and(act == A_IDLE && !pend)) break;
         }
         // ------------------------------------------------------------------ f(y) of a new state or after an accepted step
-        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
+        __syncwarp();                              // every phase starts with the warp converged (chem_tps.cuh, header)
         if (act == A_F0) {
             rhs(tab, sm, N, NR, tmid, P, invP, y, 0.0, gF);
             nfcn++;
             act = nxt;
         }
         // ------------------------------------------------------------------ Jacobian
-        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
+        __syncwarp();                              // every phase starts with the warp converged (chem_tps.cuh, header)
         if (act == A_JAC) {
             if (prm.fd_jacobian) {
                 // CVODE-style difference quotient (R13): column j = (f(y + inc_j e_j) - f(y)) / inc_j
@@ -357,7 +358,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
             act = A_FACT;
         }
         // ------------------------------------------------------------------ E1, E2 and their LU
-        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
+        __syncwarp();                              // every phase starts with the warp converged (chem_tps.cuh, header)
         if (act == A_FACT) {
             const double invH = rcp_f(H);
             int ier;
@@ -375,7 +376,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
             } else act = A_STEP;
         }
         // ------------------------------------------------------------------ start of a step attempt
-        __syncwarp();                              // every phase starts with the warp converged (see the header comment)
+        __syncwarp();                              // every phase starts with the warp converged (chem_tps.cuh, header)
         if (act == A_STEP) {
             nstep++;
             if (nstep > NMAX) { status = -1; retire(); }

@@ -11,7 +11,11 @@
 //   * all data of a lane is addressed [element][lane] (structure of arrays across the warp): every access of a warp is
 //     one coalesced 256-byte row, in shared memory (work vectors, conflict-free) and in global memory (the matrices,
 //     L2-resident); element indices are uniform across the warp except for the row interchanges of partial pivoting;
-//   * there is no cross-lane communication at all: no shuffles, no reductions, no barriers after the tables are staged.
+//   * the device routines below have no cross-lane communication at all (no shuffles, no reductions, no barriers), so any
+//     subset of the lanes may call them; the kernel (chem_tps.cu) puts a __syncwarp() in front of every phase -- without it
+//     the compiler lets the lanes that skip a phase run ahead into the next one and every phase runs twice, with
+//     complementary halves of the warp -- and one CTA barrier per pass, so that the warps of a CTA are in the same phase at
+//     the same time and share their instruction-cache fills.
 // The arithmetic is that of chem_warp.cuh (exp-job tables of the mechanism compiler, R1-R12) with plain LU +
 // triangular solves, left-looking so that each factor entry is written once.
 #pragma once
