@@ -139,6 +139,14 @@ int chem_jacobian(const chem_mech *mech, int32_t n_states, double P, const doubl
 int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const double *A, const double *b, double *x,
                   int32_t *info, void *stream);
 
+/* Test hook for the thread-per-state kernel's linear algebra (left-looking LU with partial pivoting +
+ * triangular solves, one system per lane), on the two matrices of one Radau step built from a real n x n matrix J
+ * (1 <= n <= 16):   (fac1 I - J) x1 = b1   and   ((alphn + i betan) I - J)(x2 + i x3) = b2 + i b3.
+ * J: device [batch][n][n] row-major; b, x: device [batch][3][n] (b1, b2, b3 / x1, x2, x3); info: device [batch] or NULL,
+ * 0 or j + 1 if a matrix has no usable pivot in column j (x is then not written). */
+int chem_tps_radau_solve(int32_t n, int32_t batch, const double *J, double fac1, double alphn, double betan,
+                         const double *b, double *x, int32_t *info, void *stream);
+
 /* The hot path: integrate every state from t = 0 to t_end at constant pressure P.
  * y_in, y_out: device [n_states][N] row-major (may alias).  n_states == 0 is a no-op. */
 int chem_integrate(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,

@@ -45,7 +45,7 @@ assert STATS_DTYPE.itemsize == 48
 
 EXPORTS = ["chem_mech_load", "chem_mech_free", "chem_mech_info", "chem_rhs", "chem_jacobian", "chem_lu_solve",
            "chem_integrate", "chem_integrate_ex", "chem_integrate_host", "chem_launch_count", "chem_flop_model",
-           "chem_last_error", "chem_last_kernel", "chem_fp64_probe"]
+           "chem_last_error", "chem_last_kernel", "chem_fp64_probe", "chem_tps_radau_solve"]
 
 _lib = None
 
@@ -77,6 +77,8 @@ def lib():
         L.chem_flop_model.argtypes = [C.c_void_p, _dp]
         L.chem_last_kernel.argtypes = [C.c_void_p]
         L.chem_fp64_probe.argtypes = [C.c_int32, C.c_int32, _dp]
+        L.chem_tps_radau_solve.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_double, C.c_double, C.c_double,
+                                           C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -172,6 +174,18 @@ def chem_lu_solve(A, b, stream=None):
     _check(lib().chem_lu_solve(n, batch, int(cplx), C.c_void_p(Ar.data_ptr()), C.c_void_p(br.data_ptr()),
                                C.c_void_p(x.data_ptr()), C.c_void_p(info.data_ptr()), _stream_ptr(stream)))
     return (torch.view_as_complex(x) if cplx else x), info[:batch]
+
+
+def chem_tps_radau_solve(J, fac1: float, alphn: float, betan: float, b, stream=None):
+    """Thread-per-state linear algebra hook (include/chem.h).  J: [batch, n, n], b: [batch, 3, n] float64 CUDA tensors.
+    Returns (x [batch, 3, n], info [batch])."""
+    import torch
+    batch, n = J.shape[0], J.shape[1]
+    x = torch.zeros_like(b)
+    info = torch.empty(max(batch, 1), dtype=torch.int32, device=J.device)
+    _check(lib().chem_tps_radau_solve(n, batch, _dev_f64(J, (batch, n, n)), fac1, alphn, betan, _dev_f64(b, (batch, 3, n)),
+                                      _dev_f64(x), C.c_void_p(info.data_ptr()), _stream_ptr(stream)))
+    return x, info[:batch]
 
 
 def _opts(h0=0.0, max_steps=0, newton_max=0, kernel=0, reorder=0, P_per_state=None, cost_hint=None, fd_jacobian=0, fixed_steps=0):

@@ -570,3 +570,42 @@ def test_fixed_step_that_cannot_be_taken_ends_the_state(torch_cuda, gpu_mechs, o
             y = y.cpu().numpy()
             good = np.all(np.abs(y[ok0] - y_ref[ok0]) <= 1e-9 + 1e-6 * np.abs(y_ref[ok0]), axis=1)
             assert good.mean() >= 0.97, (steps, kernel, good.mean())
+
+
+@pytest.mark.parametrize("n", [1, 2, 5, 13, 16])
+def test_thread_per_state_linear_algebra_matches_lapack(n, torch_cuda, gpu_mechs, mech_h2co):
+    """PAPER.md L86 (LU factorisation): the thread-per-state kernel's LU + triangular solves (compile-time-N form for
+    n = 13, runtime-N form otherwise) on E1 = fac1 I - J and E2 = (alphn + i betan) I - J against numpy / LAPACK: random
+    matrices with heavy pivoting, stiff matrices of the integrator's shape (n = 13: the Jacobians of config 2 states),
+    and a matrix without a pivot (info)."""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    rng = np.random.default_rng(300 + n)
+    batch = 301                                              # several warps and a ragged tail
+    J = rng.standard_normal((batch, n, n))
+    fac1, alphn, betan = 3.6378e0, 2.6811e0, 3.0504e0        # h = 1: the shift does not dominate, pivots move
+    if n == 13:
+        y0 = synth.make_states(mech_h2co, 150, "ignition", 5)
+        J[:150] = binding.chem_jacobian(gpu_mechs["h2co"], P, torch.from_numpy(y0).cuda()).cpu().numpy() * 1e-5   # h = 1e-5 s
+    J[-1] = 0.0
+    J[-1, 0, 0] = fac1                                       # fac1 I - J has a zero first column: no pivot
+    b = rng.standard_normal((batch, 3, n))
+    x, info = binding.chem_tps_radau_solve(torch.from_numpy(J).cuda(), fac1, alphn, betan, torch.from_numpy(b).cuda())
+    x, info = x.cpu().numpy(), info.cpu().numpy()
+    if n > 1:
+        assert info[-1] != 0
+    assert np.all(info[:-1] == 0)
+    eye = np.eye(n)
+    u = 2.0 ** -53
+    worst, worst_ref = 0.0, 0.0
+    for s in range(batch - 1):
+        E1 = fac1 * eye - J[s]
+        E2 = (alphn + 1j * betan) * eye - J[s]
+        for A, rhs, sol in ((E1, b[s, 0], x[s, 0]), (E2, b[s, 1] + 1j * b[s, 2], x[s, 1] + 1j * x[s, 2])):
+            ref = np.linalg.solve(A, rhs)
+            cond = np.linalg.cond(A)
+            assert np.abs(sol - ref).max() <= 1e-13 * cond * np.abs(ref).max() + 1e-300, (n, s, cond)
+            worst = max(worst, _backward_error(A, sol, rhs) / u)
+            worst_ref = max(worst_ref, _backward_error(A, ref, rhs) / u)
+    print(f"n = {n}: componentwise backward error device {worst:.3g} u, LAPACK {worst_ref:.3g} u")
+    assert worst <= 8.0 * worst_ref + 64.0, (worst, worst_ref)   # that of a pivoted LU solve on the same (badly scaled) matrices
