@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libchem.so")
-SOURCES = ["chem.cu", "chem_tps.cu"]
+SOURCES = ["chem.cu", "chem_tps.cu", "chem_tps_inst_a.cu", "chem_tps_inst_b.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 

@@ -85,7 +85,7 @@ __device__ __forceinline__ double exp_e(double x)
 // f(T, Y; P) at the state y + vs * v (R1-R5; same mathematics as warp_rhs_body, chem_warp.cuh), all lane-private:
 // y = sm[0..N), v and the result `out` anywhere (shared or global; v is consumed before the scratch is written).
 // tab = staged table blob (shared, read with uniform indices).
-__device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, double tmid, double P, double invP,
+static __device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, double tmid, double P, double invP,
                                  const double *v, double vs, double *out)
 {
     const int *hdr = reinterpret_cast<const int *>(tab);
@@ -198,7 +198,7 @@ __device__ __noinline__ void rhs(const double *tab, double *sm, int N, int NR, d
 // J[i*N + j] = d f_i / d y_j at y -> global gJ (R6; the formulation of warp_jacobian, chem_warp.cuh).  Pass 1
 // leaves four numbers per reaction (c k_f, -c k_r, dq/dT at constant C, dq/d[M]) in the lane's global workspace; pass 2 builds d wdot_k / d C row by row in a lane-private row buffer, applies the chain rule
 // C -> (T, Y) and writes row k + 1 of J straight to global memory: N^2 global stores, no global read-modify-write.
-__device__ __noinline__ void jacobian(const double *tab, double *sm, double *gJ, double *rd, int N, int NR, double tmid, double P,
+static __device__ __noinline__ void jacobian(const double *tab, double *sm, double *gJ, double *rd, int N, int NR, double tmid, double P,
                                       double invP)
 {
     const int *hdr = reinterpret_cast<const int *>(tab);
@@ -380,7 +380,7 @@ __device__ __noinline__ void jacobian(const double *tab, double *sm, double *gJ,
 // finished columns k < j -- the same operations in the same order as right-looking elimination, but every factor entry
 // is written once -- then the pivot is searched (|re| + |im| for the complex matrix, first maximum wins: DESIGN.md R10).
 // Returns 0, or j + 1 if a matrix has no usable pivot in column j or J is not finite.
-__device__ __noinline__ int lu_pair(const double *gJ, double *g1, double2 *g2, double *col, int N, double fac1, double alphn,
+static __device__ __noinline__ int lu_pair(const double *gJ, double *g1, double2 *g2, double *col, int N, double fac1, double alphn,
                                     double betan, u64 &ip1_out, u64 &ip2_out)
 {
     double *c1 = col, *cr = col + N * 32, *ci = col + 2 * N * 32;
@@ -481,7 +481,7 @@ __device__ __forceinline__ void apply_perm(double *b, int N, u64 ip)
 }
 
 // E1 x = b in place (b lane-private in shared memory)
-__device__ __noinline__ void solve_real(const double *g1, double *b, int N, u64 ip)
+static __device__ __noinline__ void solve_real(const double *g1, double *b, int N, u64 ip)
 {
     apply_perm(b, N, ip);
 #pragma unroll 1
@@ -501,7 +501,7 @@ __device__ __noinline__ void solve_real(const double *g1, double *b, int N, u64 
 }
 
 // E1 x1 = b1 and E2 (x2 + i x3) = b2 + i b3 in place, one loop nest (three independent dependency chains)
-__device__ __noinline__ void solve3(const double *g1, const double2 *g2, double *b1, double *b2, double *b3, int N, u64 ip1, u64 ip2)
+static __device__ __noinline__ void solve3(const double *g1, const double2 *g2, double *b1, double *b2, double *b3, int N, u64 ip1, u64 ip2)
 {
     apply_perm(b1, N, ip1);
 #pragma unroll 1

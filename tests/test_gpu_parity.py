@@ -609,3 +609,21 @@ def test_thread_per_state_linear_algebra_matches_lapack(n, torch_cuda, gpu_mechs
             worst_ref = max(worst_ref, _backward_error(A, ref, rhs) / u)
     print(f"n = {n}: componentwise backward error device {worst:.3g} u, LAPACK {worst_ref:.3g} u")
     assert worst <= 8.0 * worst_ref + 64.0, (worst, worst_ref)   # that of a pivoted LU solve on the same (badly scaled) matrices
+
+
+def test_other_small_mechanism_sizes(torch_cuda):
+    """a 9-species / 20-reaction hydrogen-oxygen sized shape (synth kind "h2_9"): the thread-per-state kernel has a
+    compile-time-N instantiation for every 8 <= N <= 16 (13 is the one the BASELINE.json configs exercise); this is N = 9,
+    and the warp-per-state and group kernels at a size other than the benchmark's"""
+    from oracle import oracle as orc
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = synth.make_mechanism("h2_9", 1)
+    gm, om = binding.chem_mech_load(mech), orc.Mechanism(mech)
+    y0 = synth.make_states(mech, 3000, "ignition", 3)
+    yd = torch.from_numpy(y0).cuda()
+    y_ref, st_ref, _ = om.integrate(y0, P, 1e-5, RTOL, ATOL)
+    assert np.all(st_ref["status"] == 0)
+    for kernel in (1, 2, 3):
+        y, st = binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, yd, kernel=kernel)
+        compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
