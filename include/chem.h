@@ -27,7 +27,9 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).
  *     Calls taking a stream are asynchronous with respect to the host.  Every launch takes its work-queue head and
  *     scratch from the stream-ordered allocator (cudaMallocAsync on `stream`), so calls on different streams may run
- *     concurrently with the same chem_mech.
+ *     concurrently with the same chem_mech.  The library lifts the release threshold of the device's default memory
+ *     pool once, so that this scratch (a few bytes; 277 MB for a full launch of the thread-per-state kernel) is reused
+ *     from call to call instead of going back to the driver.
  *   - there is NO CPU fallback: without a CUDA device every compute call fails
  *     with CHEM_E_CUDA.
  */
