@@ -627,3 +627,46 @@ def test_other_small_mechanism_sizes(torch_cuda):
     for kernel in (1, 2, 3):
         y, st = binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, yd, kernel=kernel)
         compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+
+
+def test_thread_per_state_kernel_options_and_reproducibility(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
+    """the thread-per-state kernel (what auto takes for the full-size h2co configs) with the options and properties the
+    other kernels are tested for: per-state pressure, cost ordering (bit-identical results), bit-reproducible results that
+    do not depend on what else is in the batch or on how the lanes were refilled, exact zeros in the state"""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    m = gpu_mechs["h2co"]
+    y0 = synth.make_states(mech_h2co, 20011, "ignition", 91)
+    y0[::97, 3] = 0.0                                                     # some exact zeros among the mass fractions
+    yd = torch.from_numpy(y0).cuda()
+    y_a, st_a = binding.chem_integrate_ex(m, P, 1e-5, RTOL, ATOL, yd, kernel=3)
+    y_b, st_b = binding.chem_integrate_ex(m, P, 1e-5, RTOL, ATOL, yd, kernel=3)
+    assert torch.equal(y_a, y_b) and torch.equal(st_a, st_b)
+    sa = binding.stats_to_numpy(st_a)
+    assert np.all(sa["status"] == 0)
+    # a shuffled third of the batch: other neighbours in the warp, other refill pattern, same bits
+    perm = np.random.default_rng(5).permutation(20011)[:6667]
+    y_c, st_c = binding.chem_integrate_ex(m, P, 1e-5, RTOL, ATOL, torch.from_numpy(y0[perm].copy()).cuda(), kernel=3)
+    assert np.array_equal(y_c.cpu().numpy(), y_a.cpu().numpy()[perm])
+    assert np.array_equal(binding.stats_to_numpy(st_c), sa[perm])
+    # cost ordering only changes when a state starts
+    nstep = torch.from_numpy(sa["nstep"].copy()).cuda()
+    y_d, st_d = binding.chem_integrate_ex(m, P, 1e-5, RTOL, ATOL, yd, kernel=3, reorder=1, cost_hint=nstep)
+    assert torch.equal(y_a, y_d) and torch.equal(st_a, st_d)
+    # against the oracle on a sample (including states with zeros), and per-state pressure
+    idx = np.r_[np.arange(0, 20011, 97)[:60], np.arange(1, 400, 7)]
+    y_ref, st_ref, _ = orc_mechs["h2co"].integrate(y0[idx], P, 1e-5, RTOL, ATOL)
+    compare_integration(y_a.cpu().numpy()[idx], sa[idx], y_ref, st_ref)
+    Ps = np.linspace(0.5, 5.0, 20011) * P
+    y_p, _ = binding.chem_integrate_ex(m, P, 1e-6, RTOL, ATOL, yd, kernel=3, P_per_state=torch.from_numpy(Ps).cuda())
+    y_p = y_p.cpu().numpy()
+    for s in (0, 9999, 20010):
+        yr, _, _ = orc_mechs["h2co"].integrate(y0[s:s + 1], float(Ps[s]), 1e-6, RTOL, ATOL)
+        assert np.all(np.abs(y_p[s] - yr[0]) <= 1e-9 + 1e-6 * np.abs(yr[0]))
+    # host entry point: pinned buffers are read and written through their device mapping, pageable ones are staged
+    y_pin = torch.from_numpy(y0).pin_memory()
+    o_pin = torch.empty(y_pin.shape, dtype=torch.float64, pin_memory=True)
+    binding.chem_integrate_host(m, P, 1e-5, RTOL, ATOL, y_pin.numpy(), o_pin.numpy(), kernel=3)
+    assert np.array_equal(o_pin.numpy(), y_a.cpu().numpy())
+    y_h, st_h = binding.chem_integrate_host(m, P, 1e-5, RTOL, ATOL, y0, want_stats=True, kernel=3)
+    assert np.array_equal(y_h, y_a.cpu().numpy()) and np.array_equal(st_h, sa)
