@@ -167,6 +167,42 @@ int chem_integrate_ex(const chem_mech *mech, int32_t n_states, double P, double 
 int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
                         const double *y_in_host, double *y_out_host, const chem_opts *opts, chem_stats *stats_host);
 
+/* The hot path for callers that must not allocate device memory at call time.
+ *
+ * Every other compute call of this library takes a little device memory per launch from CUDA's stream-ordered allocator
+ * (the work-queue head, the start order, the thread-per-state workspace).  Some hosts cannot afford that: an application
+ * that claimed the whole card for its own memory arena at start-up (a flow solver, a training framework with a caching
+ * allocator), so that a driver allocation fails or forces the arena to shrink; a process held to a fixed memory budget
+ * on a shared or partitioned GPU; a time-critical loop in which a call that may take a driver lock or synchronise the
+ * device is not acceptable.  chem_integrate_noalloc is chem_integrate_ex for them.  It runs the same shared-memory
+ * kernels (chem_opts.kernel 0, 1 or 2; 0 picks the warp-per-state kernel where the mechanism allows it, else the group
+ * kernel) and gives bit-identical y_out and stats for the same kernel id, but keeps its scratch in a fixed array that is
+ * part of the library image.  It calls no cudaMalloc / cudaMallocAsync / cudaFree and no library routine that does.
+ * The caller owns every buffer it passes (y_in, y_out, stats, opts->P_per_state, opts->cost_hint: device memory);
+ * chem_mech_load DOES allocate, so load the mechanism at set-up time, before the no-allocation phase begins.
+ *
+ * Limits and rules:
+ *   - at most CHEM_NOALLOC_MAX_STATES states per call (the array has one start-order slot per state); a larger n_states
+ *     returns CHEM_E_UNSUPPORTED with a message and launches nothing.  Split a larger batch into several calls on one
+ *     stream: the states are independent.
+ *   - chem_opts.kernel = 3 (thread-per-state) returns CHEM_E_UNSUPPORTED: its workspace is 7 KB per resident state.
+ *   - the array costs 4 MiB + 4352 B of device memory on EVERY GPU that loads libchem.so, from load until the process
+ *     exits, whether or not this function is ever called.
+ *   - the first call on each device looks up the array's device address (with that device current) and sets kernel
+ *     attributes; CUDA may also load the kernels' code on a first launch.  Make one call per device during set-up
+ *     (n_states = 1 is enough), before any stream capture and before the phase in which allocation is off limits.
+ *   - all calls on a device share the one array, and it keeps the previous call's contents; each call clears, on its own
+ *     stream, the part it starts from.  Calls that can overlap on the GPU (different streams, several host threads)
+ *     race on the work queue and return wrong results or skip states: issue them on one stream or order them with events.
+ *     This applies across mechanisms too.  chem_integrate / chem_integrate_ex do not use the array and may overlap freely.
+ *   - opts->reorder = 1 with opts->cost_hint orders the start of the states by decreasing cost with a counting sort over
+ *     1024 cost classes (no sort library); as with chem_integrate_ex the results do not depend on it.
+ * Otherwise as chem_integrate_ex: asynchronous on `stream`, y_in / y_out may alias, stats may be NULL, n_states == 0 is a
+ * no-op.  PAPER.md L47-L49, L86, L134 (the operation), L194 (reordering). */
+#define CHEM_NOALLOC_MAX_STATES 1048576
+int chem_integrate_noalloc(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
+                           const double *y_in, double *y_out, const chem_opts *opts, chem_stats *stats, void *stream);
+
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 int64_t chem_launch_count(void);
 

@@ -45,7 +45,7 @@ assert STATS_DTYPE.itemsize == 48
 
 EXPORTS = ["chem_mech_load", "chem_mech_free", "chem_mech_info", "chem_rhs", "chem_jacobian", "chem_lu_solve",
            "chem_integrate", "chem_integrate_ex", "chem_integrate_host", "chem_launch_count", "chem_flop_model",
-           "chem_last_error", "chem_last_kernel", "chem_fp64_probe", "chem_tps_radau_solve"]
+           "chem_last_error", "chem_last_kernel", "chem_fp64_probe", "chem_tps_radau_solve", "chem_integrate_noalloc"]
 
 _lib = None
 
@@ -72,6 +72,7 @@ def lib():
                                      C.c_void_p, C.c_void_p, C.c_void_p]
         L.chem_integrate_ex.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
                                         C.c_void_p, C.c_void_p, C.POINTER(chem_opts), C.c_void_p, C.c_void_p]
+        L.chem_integrate_noalloc.argtypes = L.chem_integrate_ex.argtypes
         L.chem_integrate_host.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
                                           C.c_void_p, C.c_void_p, C.POINTER(chem_opts), C.c_void_p]
         L.chem_flop_model.argtypes = [C.c_void_p, _dp]
@@ -224,6 +225,27 @@ def chem_integrate_ex(mech: Mechanism, P: float, t_end: float, rtol: float, atol
                                    _dev_f64(y_out, (n, mech.n_species)), C.byref(o),
                                    C.c_void_p(stats.data_ptr()) if want_stats else None, _stream_ptr(stream)))
     return y_out, (stats[:n] if want_stats else None)
+
+
+NOALLOC_MAX_STATES = 1048576     # CHEM_NOALLOC_MAX_STATES of include/chem.h
+
+
+def chem_integrate_noalloc(mech: Mechanism, P: float, t_end: float, rtol: float, atol: float, y_in, y_out, stats=None,
+                           stream=None, **opts):
+    """chem_integrate_ex for callers that may not allocate device memory while they run (an application whose own arena
+    holds the whole GPU, a fixed memory budget, a time-critical loop): the library's scratch is a fixed 4 MiB array inside
+    libchem.so instead of a per-launch allocation.  This wrapper allocates nothing either: `y_out` [n, N] float64 and the
+    optional `stats` (uint8 [n, 48], see stats_to_numpy) are CUDA tensors the caller made beforehand.  At most
+    NOALLOC_MAX_STATES states per call (ChemError beyond that), kernel 0, 1 or 2 only, and no two calls may overlap on
+    the GPU (they share the array): see include/chem.h.  Returns (y_out, stats)."""
+    n = y_in.shape[0]
+    o = _opts(**opts)
+    if stats is not None and not (stats.is_cuda and stats.is_contiguous() and stats.numel() * stats.element_size() >= n * STATS_DTYPE.itemsize):
+        raise ChemError("stats must be a contiguous CUDA tensor of at least n * 48 bytes")
+    _check(lib().chem_integrate_noalloc(mech._h, n, P, t_end, rtol, atol, _dev_f64(y_in, (n, mech.n_species)),
+                                        _dev_f64(y_out, (n, mech.n_species)), C.byref(o),
+                                        C.c_void_p(stats.data_ptr()) if stats is not None else None, _stream_ptr(stream)))
+    return y_out, stats
 
 
 def stats_to_numpy(stats):

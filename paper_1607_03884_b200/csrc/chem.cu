@@ -454,3 +454,188 @@ extern "C" int64_t chem_launch_count(void) { return g_launches.load(); }
 extern "C" const char *chem_last_error(void) { return chem_host::g_err.c_str(); }
 
 #include "chem_kernels.inl"
+
+// ------------------------------------------------------------------------------------------------ no-allocation entry point
+// chem_integrate_noalloc (include/chem.h): the shared-memory integration kernels of chem_kernels.inl, launched with their
+// global scratch -- the work-queue head and, when the caller asks for cost ordering, the start order -- in a fixed array
+// that is part of the library image instead of a block from the stream-ordered allocator.  It is for hosts whose device
+// memory is not theirs to ask for at call time: a flow solver or a training framework that took the whole card for its
+// own arena at start-up (cudaMallocAsync then fails or makes that arena give memory back), a process held to a hard
+// memory budget on a shared or partitioned card, a time-critical loop in which an allocator call that may take a driver
+// lock or synchronise the device is not acceptable.  Everything below uses memory that exists from the moment the
+// library is loaded: no cudaMalloc / cudaMallocAsync / cudaFree, no cub, no memory pool.
+//
+// The array: kNoAllocBytes (4 MiB + 4352 B) on EVERY device that loads libchem.so, held until the process exits, whether
+// or not this entry point is ever called.  Layout: [0, 256) queue head (one int), [256, 4352) 1024 bucket counters of the
+// ordering pass, [4352, ...) start order, one int per state -- hence the limit CHEM_NOALLOC_MAX_STATES per call.
+// All calls on one device share it and it keeps whatever the last call left there: each call zeroes the head (and the
+// counters when it orders) on its own stream before it launches, and two calls that overlap in time on the GPU
+// (different streams, or different host threads without a common stream) corrupt each other's queue.
+namespace {
+
+constexpr int kNoAllocBuckets = 1024;
+constexpr size_t kNoAllocHeadBytes = 256;
+constexpr size_t kNoAllocOrderOff = kNoAllocHeadBytes + kNoAllocBuckets * sizeof(unsigned);   // 4352 = 17 x 256
+constexpr size_t kNoAllocBytes = kNoAllocOrderOff + (size_t)CHEM_NOALLOC_MAX_STATES * sizeof(int);
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+// In host code the name g_noalloc_scratch is only a handle for the runtime (a host-side shadow object), NOT the device
+// address: handing it to a kernel would make the kernel read and write unrelated memory.  The address is looked up once
+// per device, with that device current, and cached.
+constexpr int kNoAllocMaxDev = 64;
+std::mutex g_noalloc_mu;
+void *g_noalloc_ptr[kNoAllocMaxDev] = {};
+
+int noalloc_scratch_ptr(unsigned char **p)
+{
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDev) return fail(CHEM_E_UNSUPPORTED, "chem_integrate_noalloc: device ordinal %d not supported (max %d)", dev, kNoAllocMaxDev - 1);
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void *q = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&q, g_noalloc_scratch));
+        if (!q) return fail(CHEM_E_CUDA, "chem_integrate_noalloc: no device address for the scratch array on device %d", dev);
+        g_noalloc_ptr[dev] = q;
+    }
+    *p = static_cast<unsigned char *>(g_noalloc_ptr[dev]);
+    return CHEM_OK;
+}
+
+// Start order by decreasing cost without a sort library: a counting sort over 1024 cost classes (costs are internal step
+// counts; anything above 1023 shares the first class).  Bucket 0 holds the most expensive states.  The order inside a
+// class depends on the timing of the atomics; results do not depend on the order at all (it only decides WHEN a state
+// starts), so that is harmless.  Equal keys inside a warp are combined into one atomic.
+__device__ __forceinline__ int noalloc_bucket(int32_t c)
+{
+    c = c < 0 ? 0 : (c > kNoAllocBuckets - 1 ? kNoAllocBuckets - 1 : c);
+    return kNoAllocBuckets - 1 - c;
+}
+
+__global__ void __launch_bounds__(256) noalloc_count_kernel(int n, const int32_t *__restrict__ cost, unsigned *bucket)
+{
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    const int b = i < n ? noalloc_bucket(cost[i]) : kNoAllocBuckets;        // kNoAllocBuckets: lane without a state
+    const unsigned peers = __match_any_sync(0xffffffffu, b);
+    if (i < n && (int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&bucket[b], (unsigned)__popc(peers));
+}
+
+__global__ void __launch_bounds__(kNoAllocBuckets) noalloc_offsets_kernel(unsigned *bucket)   // one CTA: counts -> first slots
+{
+    __shared__ unsigned s[kNoAllocBuckets];
+    const int t = threadIdx.x;
+    const unsigned mine = bucket[t];
+    s[t] = mine;
+    __syncthreads();
+    for (int d = 1; d < kNoAllocBuckets; d <<= 1) {
+        const unsigned v = t >= d ? s[t - d] : 0u;
+        __syncthreads();
+        s[t] += v;
+        __syncthreads();
+    }
+    bucket[t] = s[t] - mine;
+}
+
+__global__ void __launch_bounds__(256) noalloc_place_kernel(int n, const int32_t *__restrict__ cost, unsigned *bucket, int *order)
+{
+    const int i = blockIdx.x * 256 + threadIdx.x, lane = threadIdx.x & 31;
+    const int b = i < n ? noalloc_bucket(cost[i]) : kNoAllocBuckets;
+    const unsigned peers = __match_any_sync(0xffffffffu, b);
+    const int leader = __ffs(peers) - 1;
+    unsigned base = 0;
+    if (i < n && lane == leader) base = atomicAdd(&bucket[b], (unsigned)__popc(peers));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (i < n) order[base + __popc(peers & ((1u << lane) - 1u))] = i;
+}
+
+template <int G>
+int noalloc_launch_group(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
+                         const chem_opts *o, chem_stats *stats, int *head, const int *order, cudaStream_t st)
+{
+    const size_t smem = work_doubles(m->t.n_sp, m->t.n_rx, G / 32, m->t.n_fo) * sizeof(double) * (block_of<G>() / G);
+    int occ = 0;
+    const int rc = configure(integrate_kernel<G>, m, smem, &occ, block_of<G>());
+    if (rc) return rc;
+    const int gpb = block_of<G>() / G;
+    int grid = (n + gpb - 1) / gpb;
+    if (grid > m->n_sm * occ) grid = m->n_sm * occ;
+    integrate_kernel<G><<<grid, block_of<G>(), smem, st>>>(m->t, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats, head, order);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return CHEM_OK;
+}
+
+int noalloc_launch_warp(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, double *y_out,
+                        const chem_opts *o, chem_stats *stats, int *head, const int *order, cudaStream_t st)
+{
+    const int wpb = kWarpBlock / 32;
+    const size_t smem = ((size_t)m->fast.blob_doubles + (size_t)wpb * warp_ws_doubles(m->t.n_sp, m->t.n_rx)) * sizeof(double);
+    CUDA_TRY(cudaFuncSetAttribute(integrate_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, integrate_warp_kernel, kWarpBlock, smem));
+    if (occ < 1) return fail(CHEM_E_UNSUPPORTED, "warp kernel does not fit on an SM");
+    int grid = (n + wpb - 1) / wpb;
+    if (grid > m->n_sm * occ) grid = m->n_sm * occ;
+    integrate_warp_kernel<<<grid, kWarpBlock, smem, st>>>(m->t, m->fast, n, P, o ? o->P_per_state : nullptr, prm, y_in, y_out, stats,
+                                                          head, order);
+    g_launches++;
+    CUDA_TRY(cudaGetLastError());
+    return CHEM_OK;
+}
+
+}  // namespace
+
+extern "C" int chem_integrate_noalloc(const chem_mech *m, int32_t n, double P, double t_end, double rtol, double atol,
+                                      const double *y_in, double *y_out, const chem_opts *o, chem_stats *stats, void *stream)
+{
+    if (!m || n < 0 || (n > 0 && (!y_in || !y_out))) return fail(CHEM_E_ARG, "bad argument");
+    if (!(t_end > 0.0) || !(rtol > 0.0) || !(atol > 0.0)) return fail(CHEM_E_ARG, "t_end, rtol and atol must be positive");
+    if (o && (o->kernel < 0 || o->kernel > 3)) return fail(CHEM_E_ARG, "chem_opts.kernel must be 0..3");
+    if (n > CHEM_NOALLOC_MAX_STATES)
+        return fail(CHEM_E_UNSUPPORTED, "chem_integrate_noalloc: n_states = %d is more than the fixed scratch array holds "
+                    "(CHEM_NOALLOC_MAX_STATES = %d); split the batch into several calls on one stream", n, CHEM_NOALLOC_MAX_STATES);
+    int kernel = o ? o->kernel : 0;
+    if (kernel == 3)
+        return fail(CHEM_E_UNSUPPORTED, "chem_integrate_noalloc: the thread-per-state kernel needs a per-launch workspace of 7 KB per "
+                    "resident state (277 MB) and is not offered without allocation; use kernel 0, 1 or 2");
+    if (kernel == 0) kernel = warp_path_available(m) ? 2 : 1;
+    if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "warp-per-state kernel not available for this mechanism");
+    if (n == 0) return CHEM_OK;
+    RadauParams prm;      // same derived quantities as integrate_impl (chem_launch.inl)
+    prm.t_end = t_end; prm.rtol = rtol; prm.atol = atol;
+    prm.h0 = o ? o->h0 : 0.0;
+    prm.max_steps = o ? o->max_steps : 0;
+    prm.newton_max = o ? o->newton_max : 0;
+    prm.fd_jacobian = o ? o->fd_jacobian : 0;
+    prm.fixed_steps = o ? o->fixed_steps : 0;
+    prm.rtol_t = 0.1 * std::pow(rtol, 2.0 / 3.0);
+    prm.atol_t = prm.rtol_t * (atol / rtol);
+    prm.fnewt = std::fmax(10.0 * 2.220446049250313e-16 / prm.rtol_t, std::fmin(0.03, std::sqrt(prm.rtol_t)));
+    prm.inv_fnewt = 1.0 / prm.fnewt; prm.inv_n = 1.0 / m->t.n_sp; prm.inv_3n = 1.0 / (3 * m->t.n_sp);
+
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned char *scratch = nullptr;
+    int rc = noalloc_scratch_ptr(&scratch);      // first call on this device: looks the address up (see chem.h)
+    if (rc) return rc;
+    int *head = reinterpret_cast<int *>(scratch);
+    unsigned *bucket = reinterpret_cast<unsigned *>(scratch + kNoAllocHeadBytes);
+    int *order = nullptr;
+    const bool ordered = o && o->reorder && o->cost_hint;
+    // the array still holds the previous call's queue head and counters: clear what this call starts from
+    CUDA_TRY(cudaMemsetAsync(scratch, 0, ordered ? kNoAllocOrderOff : kNoAllocHeadBytes, st));
+    if (ordered) {
+        order = reinterpret_cast<int *>(scratch + kNoAllocOrderOff);
+        const int g = (n + 255) / 256;
+        noalloc_count_kernel<<<g, 256, 0, st>>>(n, o->cost_hint, bucket);
+        noalloc_offsets_kernel<<<1, kNoAllocBuckets, 0, st>>>(bucket);
+        noalloc_place_kernel<<<g, 256, 0, st>>>(n, o->cost_hint, bucket, order);
+        g_launches += 3;
+        CUDA_TRY(cudaGetLastError());
+    }
+    if (kernel == 2) rc = noalloc_launch_warp(m, n, P, prm, y_in, y_out, o, stats, head, order, st);
+    else rc = group_size(m) == 32 ? noalloc_launch_group<32>(m, n, P, prm, y_in, y_out, o, stats, head, order, st)
+                                  : noalloc_launch_group<128>(m, n, P, prm, y_in, y_out, o, stats, head, order, st);
+    if (rc == CHEM_OK) const_cast<chem_mech *>(m)->last_kernel = kernel;
+    return rc;
+}
