@@ -26,10 +26,11 @@
  *     call returns except inside the opaque chem_mech.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).
  *     Calls taking a stream are asynchronous with respect to the host.  Every launch takes its work-queue head and
- *     scratch from the stream-ordered allocator (cudaMallocAsync on `stream`), so calls on different streams may run
- *     concurrently with the same chem_mech.  The library lifts the release threshold of the device's default memory
- *     pool once, so that this scratch (a few bytes; 277 MB for a full launch of the thread-per-state kernel) is reused
- *     from call to call instead of going back to the driver.
+ *     scratch from the stream-ordered allocator (cudaMallocFromPoolAsync on `stream`), so calls on different streams may
+ *     run concurrently with the same chem_mech.  The memory comes from a pool the library creates for itself on each
+ *     device it is used on; the device's default pool (the application's) is not touched.  The pool keeps its blocks (a
+ *     few bytes; 277 MB for a full launch of the thread-per-state kernel) from call to call; chem_scratch_trim() or
+ *     chem_mech_free() returns the unused ones to the driver.  chem_integrate_noalloc uses no allocator at all.
  *   - there is NO CPU fallback: without a CUDA device every compute call fails
  *     with CHEM_E_CUDA.
  */
@@ -92,7 +93,10 @@ typedef struct chem_opts {
     int32_t max_steps;   /* limit on internal step attempts per state; 0 -> 100000                    */
     int32_t newton_max;  /* max simplified-Newton iterations per step; 0 -> 7                         */
     int32_t kernel;      /* 0 auto; 1 shared-memory group kernel (warp or CTA per state); 2 warp-per-state kernel and
-                            3 thread-per-state kernel (both: small mechanisms only, N_sp <= 16, N_rx <= 32) */
+                            3 thread-per-state kernel (both: small mechanisms only, N_sp <= 16, N_rx <= 32).
+                            Results are bit-reproducible PER KERNEL ID.  Auto chooses by mechanism AND batch size (n_states),
+                            so with kernel = 0 the bits of one state may differ between a small and a large batch (always
+                            within the tolerance); chem_last_kernel tells which ran.  Fix the id where bits must not move. */
     int32_t reorder;     /* 1: start the states in order of decreasing cost_hint ("reordering IVPs"); 0 off */
     const double *P_per_state;  /* device [n_states] or NULL: per-state pressure overriding P        */
     const int32_t *cost_hint;   /* device [n_states] or NULL: predicted cost per state, e.g. chem_stats.nstep of the
@@ -162,8 +166,9 @@ int chem_integrate_ex(const chem_mech *mech, int32_t n_states, double P, double 
  * of y_in_host into y_out_host (and stats_host if not NULL) and synchronises.  Page-locked (pinned) buffers are read and
  * written by the kernel itself through their device mapping, state by state, so the transfers overlap the integration;
  * pageable buffers are staged through device memory in two chunks on two internal streams.  The buffers may alias.
- * `reorder` is ignored here.  The internal streams belong to the mechanism object: one chem_integrate_host call per
- * mechanism at a time. */
+ * `reorder` is ignored here.  The kernel is chosen once from n_states, as chem_integrate_ex would, whether or not the
+ * buffers are pinned (the chunks of the pageable path all run that kernel).  The internal streams belong to the mechanism
+ * object: one chem_integrate_host call per mechanism at a time. */
 int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
                         const double *y_in_host, double *y_out_host, const chem_opts *opts, chem_stats *stats_host);
 
@@ -202,6 +207,10 @@ int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, doubl
 #define CHEM_NOALLOC_MAX_STATES 1048576
 int chem_integrate_noalloc(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
                            const double *y_in, double *y_out, const chem_opts *opts, chem_stats *stats, void *stream);
+
+/* Returns the launch scratch that the library's memory pool caches for the CURRENT device to the driver (blocks still in
+ * use by queued work stay).  chem_mech_free does the same.  The next launch simply allocates again. */
+int chem_scratch_trim(void);
 
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 int64_t chem_launch_count(void);

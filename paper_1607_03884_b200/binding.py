@@ -45,7 +45,7 @@ assert STATS_DTYPE.itemsize == 48
 
 EXPORTS = ["chem_mech_load", "chem_mech_free", "chem_mech_info", "chem_rhs", "chem_jacobian", "chem_lu_solve",
            "chem_integrate", "chem_integrate_ex", "chem_integrate_host", "chem_launch_count", "chem_flop_model",
-           "chem_last_error", "chem_last_kernel", "chem_fp64_probe", "chem_tps_radau_solve", "chem_integrate_noalloc"]
+           "chem_last_error", "chem_last_kernel", "chem_fp64_probe", "chem_tps_radau_solve", "chem_integrate_noalloc", "chem_scratch_trim"]
 
 _lib = None
 
@@ -280,6 +280,11 @@ def chem_fp64_probe(iters: int = 1 << 16, reps: int = 5) -> float:
     out = C.c_double(0.0)
     _check(lib().chem_fp64_probe(iters, reps, C.byref(out)))
     return float(out.value)
+
+
+def chem_scratch_trim() -> None:
+    """return the launch scratch cached by the library's memory pool on the current device to the driver"""
+    _check(lib().chem_scratch_trim())
 
 
 def chem_launch_count() -> int:

@@ -30,26 +30,61 @@ int fail(int code, const char *fmt, ...)
     return code;
 }
 
-// Stream-ordered scratch: the default memory pool of the device with its release threshold lifted once, so that the
-// blocks of one launch are reused by the next without going back to the driver.
+// Stream-ordered scratch from a memory pool of the library's own, one per device (created on first use with that device
+// current, release threshold lifted so that the blocks of one launch are reused by the next without going back to the
+// driver).  The device's default pool -- the host application's -- is left as it is.  chem_scratch_trim gives the cached
+// blocks back.
+namespace {
+constexpr int kMaxPoolDev = 64;
+std::mutex g_pool_mu;
+cudaMemPool_t g_pool[kMaxPoolDev] = {};
+}  // namespace
+
+int scratch_pool(cudaMemPool_t *pool)
+{
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxPoolDev) return fail(CHEM_E_UNSUPPORTED, "device ordinal %d not supported (max %d)", dev, kMaxPoolDev - 1);
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (!g_pool[dev]) {
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t p = nullptr;
+        CUDA_TRY(cudaMemPoolCreate(&p, &props));
+        uint64_t keep = UINT64_MAX;
+        const cudaError_t e = cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) { cudaMemPoolDestroy(p); return fail(CHEM_E_CUDA, "cudaMemPoolSetAttribute: %s", cudaGetErrorString(e)); }
+        g_pool[dev] = p;
+    }
+    *pool = g_pool[dev];
+    return CHEM_OK;
+}
+
 int scratch_alloc(void **p, size_t bytes, cudaStream_t st)
 {
-    static std::once_flag once;
-    std::call_once(once, [] {
-        int dev = 0;
-        cudaMemPool_t pool;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            uint64_t keep = UINT64_MAX;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
-    });
     *p = nullptr;
-    CUDA_TRY(cudaMallocAsync(p, bytes, st));
+    cudaMemPool_t pool = nullptr;
+    const int rc = scratch_pool(&pool);
+    if (rc) return rc;
+    CUDA_TRY(cudaMallocFromPoolAsync(p, bytes, pool, st));
     return CHEM_OK;
 }
 void scratch_free(void *p, cudaStream_t st)
 {
     if (p) cudaFreeAsync(p, st);
+}
+// cached blocks of the current device's pool back to the driver (blocks still in use by queued work stay)
+int scratch_trim()
+{
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxPoolDev) return CHEM_OK;
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (g_pool[dev]) CUDA_TRY(cudaMemPoolTrimTo(g_pool[dev], 0));
+    return CHEM_OK;
 }
 
 }  // namespace chem_host
@@ -425,9 +460,12 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     return CHEM_OK;
 }
 
+extern "C" int chem_scratch_trim(void) { return chem_host::scratch_trim(); }
+
 extern "C" void chem_mech_free(chem_mech *m)
 {
     if (!m) return;
+    chem_host::scratch_trim();      // the launch scratch cached for this device goes back to the driver with the mechanism
     if (m->dev_blob) cudaFree(m->dev_blob);
     if (m->fast_blob) cudaFree(m->fast_blob);
     for (int i = 0; i < 2; i++)

@@ -36,10 +36,11 @@ struct chem_mech {
 };
 
 // Per-launch scratch (work-queue head, cost ordering, thread-per-state workspace) comes from the stream-ordered
-// allocator, so concurrent launches on different streams never share state.
+// allocator (a memory pool of the library's own per device), so concurrent launches on different streams never share state.
 namespace chem_host {
 int scratch_alloc(void **p, size_t bytes, cudaStream_t st);
 void scratch_free(void *p, cudaStream_t st);
+int scratch_trim();
 }  // namespace chem_host
 
 // thread-per-state path (chem_tps.cu)

@@ -286,26 +286,36 @@ extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, doub
     void *buf = nullptr;
     int rc = chem_host::scratch_alloc(&buf, ybytes + sbytes + 256, mm->hs[0]);
     if (rc) return rc;
-    CUDA_TRY(cudaStreamSynchronize(mm->hs[0]));       // the block is used from both streams
+    {                                                   // the block is used from both streams
+        const cudaError_t es = cudaStreamSynchronize(mm->hs[0]);
+        if (es != cudaSuccess) {
+            chem_host::scratch_free(buf, mm->hs[0]);
+            return fail(CHEM_E_CUDA, "chem_integrate_host: %s", cudaGetErrorString(es));
+        }
+    }
     double *d_y = static_cast<double *>(buf);
     chem_stats *d_st = stats_host ? reinterpret_cast<chem_stats *>(static_cast<char *>(buf) + ((ybytes + 255) & ~size_t(255))) : nullptr;
     const int n_chunks = n >= 65536 ? 2 : 1;
+    // the kernel is chosen once, from the whole batch: a chunk must not fall back to another mapping (and other bits)
+    // just because it is half as long (pick_kernel depends on n)
+    const int kernel_all = pick_kernel(m, n, o);
     cudaError_t e = cudaSuccess;
     for (int c = 0; c < n_chunks && rc == CHEM_OK && e == cudaSuccess; c++) {
         const int lo = (int)((long long)n * c / n_chunks), hi = (int)((long long)n * (c + 1) / n_chunks);
         if (hi == lo) continue;
         cudaStream_t st = mm->hs[c % kStreams];
-        chem_opts oc;
+        chem_opts oc{};
         if (o) {
             oc = *o;
             if (oc.P_per_state) oc.P_per_state += lo;
             oc.reorder = 0;          // cost hints are device arrays of the whole batch; chunks are short anyway
             oc.cost_hint = nullptr;
         }
+        oc.kernel = kernel_all;
         const size_t off = (size_t)lo * N, cnt = (size_t)(hi - lo) * N;
         e = cudaMemcpyAsync(d_y + off, y_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) break;
-        rc = integrate_impl(m, hi - lo, P, t_end, rtol, atol, d_y + off, d_y + off, o ? &oc : nullptr, d_st ? d_st + lo : nullptr, st);
+        rc = integrate_impl(m, hi - lo, P, t_end, rtol, atol, d_y + off, d_y + off, &oc, d_st ? d_st + lo : nullptr, st);
         if (rc != CHEM_OK) break;
         e = cudaMemcpyAsync(y_out_host + off, d_y + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess && stats_host)

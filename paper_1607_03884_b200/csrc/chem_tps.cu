@@ -73,36 +73,10 @@ int chem_tps_launch(const chem_mech *m, int n, double P, const RadauParams &prm,
 }
 
 // ------------------------------------------------------------------------------------------------ test hook
-// The linear algebra of one Radau step exactly as the integration kernel runs it (chem_tps.cuh: lu_pair / solve3, or
-// their compile-time-N forms for the instantiated N), one system per lane:  (fac1 I - J) x1 = b1  and
-// ((alphn + i betan) I - J)(x2 + i x3) = b2 + i b3.
-namespace {
-template <int NT>
-__global__ void __launch_bounds__(128) tps_solve_kernel(int n, int batch, const double *J, double fac1, double alphn, double betan,
-                                                        const double *b, double *x, int *info, double *gws)
-{
-    extern __shared__ double smem[];
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int N = NT > 0 ? NT : n;
-    const int s = (blockIdx.x * 4 + wib) * 32 + lane;
-    double *z = smem + (size_t)wib * 6 * N * 32 + lane, *col = z + 3 * N * 32;
-    double *gw = gws + ((size_t)blockIdx.x * 4 + wib) * (size_t)(4 * N * N) * 32 + lane;
-    double *gJ = gw, *g1 = gw + gE1(N) * 32;
-    double2 *g2 = reinterpret_cast<double2 *>(gw + gE2(N) * 32 - lane) + lane;
-    if (s >= batch) return;
-    for (int e = 0; e < N * N; e++) TL(gJ, e) = J[(size_t)s * N * N + e];
-    u64 ip1 = 0, ip2 = 0;
-    int ier;
-    if constexpr (NT > 0) ier = lu_pair_t<NT>(gJ, g1, g2, col, fac1, alphn, betan, ip1, ip2);
-    else ier = lu_pair(gJ, g1, g2, col, N, fac1, alphn, betan, ip1, ip2);
-    if (info) info[s] = ier;
-    if (ier) return;
-    for (int e = 0; e < 3 * N; e++) TL(z, e) = b[(size_t)s * 3 * N + e];
-    if constexpr (NT > 0) solve3_t<NT>(g1, g2, z, ip1, ip2); else solve3(g1, g2, z, z + N * 32, z + 2 * N * 32, N, ip1, ip2);
-    for (int e = 0; e < 3 * N; e++) x[(size_t)s * 3 * N + e] = TL(z, e);
-}
-}  // namespace
-
+// The linear algebra of one Radau step exactly as the integration kernel runs it (chem_tps.cuh: lu_pair_t<N> / solve3_t<N>
+// for 8 <= N <= 16, the runtime-N lu_pair / solve3 below that -- the same table as chem_tps_launch), one system per lane:
+// (fac1 I - J) x1 = b1  and  ((alphn + i betan) I - J)(x2 + i x3) = b2 + i b3.  The kernel is tps_solve_kernel<NT> in
+// chem_tps_kernel.cuh, instantiated beside the integration kernel of the same N.
 extern "C" int chem_tps_radau_solve(int32_t n, int32_t batch, const double *J, double fac1, double alphn, double betan,
                                     const double *b, double *x, int32_t *info, void *stream)
 {
@@ -115,14 +89,14 @@ extern "C" int chem_tps_radau_solve(int32_t n, int32_t batch, const double *J, d
     void *ws = nullptr;
     const int rc = chem_host::scratch_alloc(&ws, (size_t)grid * 4 * 4 * n * n * 32 * sizeof(double), st);
     if (rc) return rc;
-    cudaError_t e;
-    if (n == 13) {
-        e = cudaFuncSetAttribute(tps_solve_kernel<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) tps_solve_kernel<13><<<grid, 128, smem, st>>>(n, batch, J, fac1, alphn, betan, b, x, info, static_cast<double *>(ws));
-    } else {
-        e = cudaFuncSetAttribute(tps_solve_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) tps_solve_kernel<0><<<grid, 128, smem, st>>>(n, batch, J, fac1, alphn, betan, b, x, info, static_cast<double *>(ws));
-    }
+    typedef cudaError_t (*solve_fn)(int, int, const double *, double, double, double, const double *, double *, int *, double *, int,
+                                    size_t, cudaStream_t);
+    static const solve_fn table[17] = {chem_tps_solve_nt0, chem_tps_solve_nt0, chem_tps_solve_nt0, chem_tps_solve_nt0,
+                                       chem_tps_solve_nt0, chem_tps_solve_nt0, chem_tps_solve_nt0, chem_tps_solve_nt0,
+                                       chem_tps_solve_nt8, chem_tps_solve_nt9, chem_tps_solve_nt10, chem_tps_solve_nt11,
+                                       chem_tps_solve_nt12, chem_tps_solve_nt13, chem_tps_solve_nt14, chem_tps_solve_nt15,
+                                       chem_tps_solve_nt16};
+    cudaError_t e = table[n](n, batch, J, fac1, alphn, betan, b, x, info, static_cast<double *>(ws), grid, smem, st);
     if (e == cudaSuccess) { chem_host::g_launches++; e = cudaGetLastError(); }
     chem_host::scratch_free(ws, st);
     if (e != cudaSuccess) return fail(CHEM_E_CUDA, "chem_tps_radau_solve: %s", cudaGetErrorString(e));

@@ -266,6 +266,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
         // the owning lane's column of shared memory.
         {
             double *wsm = sm - lane;                                     // this warp's block: element e of lane l at wsm[e * 32 + l]
+            __syncwarp();        // lane l's y column was written by lane l in this pass (ballot / shuffle do not order memory)
             for (unsigned m = __ballot_sync(0xffffffffu, pend); m; m &= m - 1) {
                 const int l = __ffs(m) - 1;
                 const int s_out = __shfl_sync(0xffffffffu, sidx, l);
@@ -419,15 +420,63 @@ cudaError_t launch_tps(const TpsArgs &a, int grid, size_t smem, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// Test hook kernel of chem_tps_radau_solve (chem_tps.cu): factorises and solves one Radau step's two matrices per lane
+// with the routines of the integration kernel of the same NT.
+template <int NT>
+__global__ void __launch_bounds__(128) tps_solve_kernel(int n, int batch, const double *J, double fac1, double alphn, double betan,
+                                                        const double *b, double *x, int *info, double *gws)
+{
+    extern __shared__ double smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int N = NT > 0 ? NT : n;
+    const int s = (blockIdx.x * 4 + wib) * 32 + lane;
+    double *z = smem + (size_t)wib * 6 * N * 32 + lane, *col = z + 3 * N * 32;
+    double *gw = gws + ((size_t)blockIdx.x * 4 + wib) * (size_t)(4 * N * N) * 32 + lane;
+    double *gJ = gw, *g1 = gw + gE1(N) * 32;
+    double2 *g2 = reinterpret_cast<double2 *>(gw + gE2(N) * 32 - lane) + lane;
+    if (s >= batch) return;
+    for (int e = 0; e < N * N; e++) TL(gJ, e) = J[(size_t)s * N * N + e];
+    u64 ip1 = 0, ip2 = 0;
+    int ier;
+    if constexpr (NT > 0) ier = lu_pair_t<NT>(gJ, g1, g2, col, fac1, alphn, betan, ip1, ip2);
+    else ier = lu_pair(gJ, g1, g2, col, N, fac1, alphn, betan, ip1, ip2);
+    if (info) info[s] = ier;
+    if (ier) return;
+    for (int e = 0; e < 3 * N; e++) TL(z, e) = b[(size_t)s * 3 * N + e];
+    if constexpr (NT > 0) solve3_t<NT>(g1, g2, z, ip1, ip2); else solve3(g1, g2, z, z + N * 32, z + 2 * N * 32, N, ip1, ip2);
+    for (int e = 0; e < 3 * N; e++) x[(size_t)s * 3 * N + e] = TL(z, e);
+}
+
+template <int NT>
+cudaError_t launch_tps_solve(int n, int batch, const double *J, double fac1, double alphn, double betan, const double *b, double *x,
+                             int *info, double *gws, int grid, size_t smem, cudaStream_t st)
+{
+    const cudaError_t e = cudaFuncSetAttribute(tps_solve_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    tps_solve_kernel<NT><<<grid, 128, smem, st>>>(n, batch, J, fac1, alphn, betan, b, x, info, gws);
+    return cudaSuccess;
+}
+
 }  // namespace tps
 }  // namespace chem
 
-// defines the launcher of one instantiation: cudaError_t chem_tps_launch_nt<NT>(args, grid, smem, stream)
+// defines the launchers of one instantiation: cudaError_t chem_tps_launch_nt<NT>(args, grid, smem, stream) and the test
+// hook's chem_tps_solve_nt<NT>(...)
 #define CHEM_TPS_INSTANTIATE(NT)                                                                                          \
     cudaError_t chem_tps_launch_nt##NT(const chem::tps::TpsArgs &a, int grid, size_t smem, cudaStream_t st)              \
     {                                                                                                                     \
         return chem::tps::launch_tps<NT, 4>(a, grid, smem, st);                                                          \
+    }                                                                                                                     \
+    cudaError_t chem_tps_solve_nt##NT(int n, int batch, const double *J, double fac1, double alphn, double betan,         \
+                                      const double *b, double *x, int *info, double *gws, int grid, size_t smem,         \
+                                      cudaStream_t st)                                                                    \
+    {                                                                                                                     \
+        return chem::tps::launch_tps_solve<NT>(n, batch, J, fac1, alphn, betan, b, x, info, gws, grid, smem, st);        \
     }
-#define CHEM_TPS_DECLARE(NT) cudaError_t chem_tps_launch_nt##NT(const chem::tps::TpsArgs &a, int grid, size_t smem, cudaStream_t st);
+#define CHEM_TPS_DECLARE(NT)                                                                                              \
+    cudaError_t chem_tps_launch_nt##NT(const chem::tps::TpsArgs &a, int grid, size_t smem, cudaStream_t st);             \
+    cudaError_t chem_tps_solve_nt##NT(int n, int batch, const double *J, double fac1, double alphn, double betan,         \
+                                      const double *b, double *x, int *info, double *gws, int grid, size_t smem,         \
+                                      cudaStream_t st);
 CHEM_TPS_DECLARE(0) CHEM_TPS_DECLARE(8) CHEM_TPS_DECLARE(9) CHEM_TPS_DECLARE(10) CHEM_TPS_DECLARE(11) CHEM_TPS_DECLARE(12)
 CHEM_TPS_DECLARE(13) CHEM_TPS_DECLARE(14) CHEM_TPS_DECLARE(15) CHEM_TPS_DECLARE(16)

@@ -35,13 +35,17 @@ KINDS = {
                  n_reactions=27, n_three_body=4, n_troe=2, cp_max=8.0, inert=("N2",)),
     "gri": dict(elements=("C", "H", "O", "N", "Ar"), caps={"C": 3, "H": 8, "O": 3, "N": 2}, n_species=53,
                 n_reactions=325, n_three_body=30, n_troe=29, cp_max=15.0, inert=("AR", "N2")),
-    # not a BASELINE.json config: a test shape at the size limits of the small-mechanism kernels (16 species, and as
-    # many reactions as leave room for the falloff / Troe exp jobs among 2 x 32 job slots)
-    # not a BASELINE.json config either: a hydrogen / oxygen sized test shape (H, O, H2, O2, OH, H2O, H2O2, HO2 + N2)
+    # not BASELINE.json configs: test shapes for the small-mechanism kernels.  "h2_9": a hydrogen / oxygen sized shape (H, O,
+    # H2, O2, OH, H2O, H2O2, HO2 + N2); "lim16": the size limits of those kernels (16 species, and as many reactions as
+    # leave room for the falloff / Troe exp jobs among 2 x 32 job slots); "sz<N>": one shape per remaining compile-time-N
+    # instantiation of the thread-per-state kernel (8 <= N <= 16)
     "h2_9": dict(elements=("H", "O", "N"), caps={"H": 2, "O": 2}, n_species=9,
                  n_reactions=20, n_three_body=3, n_troe=1, cp_max=7.0, inert=("N2",)),
     "lim16": dict(elements=("H", "O", "C", "N"), caps={"H": 4, "O": 3, "C": 2}, n_species=16,
                   n_reactions=28, n_three_body=3, n_troe=1, cp_max=8.0, inert=("N2",)),
+    **{f"sz{n}": dict(elements=("H", "O", "C", "N"), caps={"H": 4, "O": 3, "C": 1}, n_species=n,
+                      n_reactions=8 if n == 8 else min(2 * n, 28), n_three_body=3, n_troe=1, cp_max=8.0, inert=("N2",))
+       for n in (8, 10, 11, 12, 14, 15)},
 }
 
 

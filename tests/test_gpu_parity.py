@@ -185,6 +185,7 @@ def test_full_size_config1_sampled_against_oracle(torch_cuda, gpu_mechs, orc_mec
     y0 = synth.make_states(mech_h2co, cfg["n_states"], cfg["dist"], synth.STATE_SEED)
     y_dev = torch.from_numpy(y0).cuda()
     y1 = binding.chem_integrate(gpu_mechs["h2co"], P, cfg["t_end"], RTOL, ATOL, y_dev).cpu().numpy()
+    assert binding.chem_last_kernel(gpu_mechs["h2co"]) == 3     # the headline runs on the thread-per-state kernel
     assert np.all(np.isfinite(y1))
     # all states: element mass fractions are linear invariants of the method; mass fractions stay in [-atol-ish, 1]
     W = mech_h2co["mol_weight"]
@@ -511,8 +512,8 @@ def test_linear_algebra_on_the_matrices_the_integrator_forms(ci, torch_cuda, gpu
 
 def test_small_mechanism_kernels_at_their_size_limit(torch_cuda):
     """16 species / 28 reactions (synth kind "lim16"): the largest shape the warp-per-state and thread-per-state kernels
-    are compiled for; the thread-per-state kernel runs its runtime-N routines here (no compile-time instantiation for
-    N = 16), and the warp-per-state kernel must decline (its CTA does not fit in shared memory) instead of failing in auto"""
+    are compiled for; the thread-per-state kernel runs its compile-time-N instantiation <16, 4> here, and the
+    warp-per-state kernel must decline (its CTA does not fit in shared memory) instead of failing in auto"""
     from oracle import oracle as orc
     from paper_1607_03884_b200 import binding
     torch = torch_cuda
@@ -572,12 +573,13 @@ def test_fixed_step_that_cannot_be_taken_ends_the_state(torch_cuda, gpu_mechs, o
             assert good.mean() >= 0.97, (steps, kernel, good.mean())
 
 
-@pytest.mark.parametrize("n", [1, 2, 5, 13, 16])
+@pytest.mark.parametrize("n", [1, 2, 5, 8, 9, 10, 11, 12, 13, 14, 15, 16])
 def test_thread_per_state_linear_algebra_matches_lapack(n, torch_cuda, gpu_mechs, mech_h2co):
-    """PAPER.md L86 (LU factorisation): the thread-per-state kernel's LU + triangular solves (compile-time-N form for
-    n = 13, runtime-N form otherwise) on E1 = fac1 I - J and E2 = (alphn + i betan) I - J against numpy / LAPACK: random
-    matrices with heavy pivoting, stiff matrices of the integrator's shape (n = 13: the Jacobians of config 2 states),
-    and a matrix without a pivot (info)."""
+    """PAPER.md L86 (LU factorisation): the thread-per-state kernel's LU + triangular solves -- lu_pair_t<n> / solve3_t<n>
+    for every 8 <= n <= 16, the runtime-N forms below that: the hook dispatches through the same table as the integration
+    kernel -- on E1 = fac1 I - J and E2 = (alphn + i betan) I - J against numpy / LAPACK: random matrices with heavy
+    pivoting, stiff matrices of the integrator's shape (n = 13: the Jacobians of config 2 states), and a matrix without
+    a pivot (info)."""
     from paper_1607_03884_b200 import binding
     torch = torch_cuda
     rng = np.random.default_rng(300 + n)
@@ -627,6 +629,48 @@ def test_other_small_mechanism_sizes(torch_cuda):
     for kernel in (1, 2, 3):
         y, st = binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, yd, kernel=kernel)
         compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+
+
+@pytest.mark.parametrize("n_sp", [8, 10, 11, 12, 14, 15])
+def test_every_compile_time_size_of_the_thread_per_state_kernel(n_sp, torch_cuda):
+    """integrate_tps_kernel<N, 4> for the N that no other test reaches (synth kinds "sz<N>"; 9, 13 and 16 run elsewhere):
+    integration parity against the oracle, beside the group kernel on the same states"""
+    from oracle import oracle as orc
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    mech = synth.make_mechanism(f"sz{n_sp}", 1)
+    assert mech["n_species"] == n_sp
+    gm, om = binding.chem_mech_load(mech), orc.Mechanism(mech)
+    y0 = synth.make_states(mech, 1300, "ignition", 3)
+    yd = torch.from_numpy(y0).cuda()
+    y_ref, st_ref, _ = om.integrate(y0, P, 1e-5, RTOL, ATOL)
+    assert np.all(st_ref["status"] == 0)
+    for kernel in (3, 1):
+        y, st = binding.chem_integrate_ex(gm, P, 1e-5, RTOL, ATOL, yd, kernel=kernel)
+        assert binding.chem_last_kernel(gm) == kernel
+        compare_integration(y.cpu().numpy(), binding.stats_to_numpy(st), y_ref, st_ref)
+
+
+def test_host_entry_point_picks_one_kernel_for_the_whole_batch(torch_cuda, gpu_mechs, mech_h2co):
+    """with kernel = 0 the choice depends on the batch size; the pageable path of chem_integrate_host splits
+    the batch in two chunks and must still run the kernel the whole batch selects (400,000 states: thread per state; a
+    200,000-state chunk alone would select warp per state), so that pinned and pageable buffers give the same bits"""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    m = gpu_mechs["h2co"]
+    y0 = synth.make_states(mech_h2co, 400_000, "uniform", 77)
+    y_dev = binding.chem_integrate(m, P, 1e-6, RTOL, ATOL, torch.from_numpy(y0).cuda()).cpu().numpy()
+    assert binding.chem_last_kernel(m) == 3
+    y_pageable = binding.chem_integrate_host(m, P, 1e-6, RTOL, ATOL, y0)
+    assert binding.chem_last_kernel(m) == 3
+    pin_in = torch.from_numpy(y0).pin_memory()
+    pin_out = torch.empty(pin_in.shape, dtype=torch.float64, pin_memory=True)
+    binding.chem_integrate_host(m, P, 1e-6, RTOL, ATOL, pin_in.numpy(), pin_out.numpy())
+    assert binding.chem_last_kernel(m) == 3
+    assert np.array_equal(y_pageable, y_dev) and np.array_equal(pin_out.numpy(), y_dev)
+    binding.chem_scratch_trim()                     # the pool gives its blocks back and the next launch still works
+    y_again = binding.chem_integrate(m, P, 1e-6, RTOL, ATOL, torch.from_numpy(y0[:5000]).cuda(), ).cpu().numpy()
+    assert y_again.shape == (5000, 13) and np.all(np.isfinite(y_again))
 
 
 def test_thread_per_state_kernel_options_and_reproducibility(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
