@@ -28,8 +28,8 @@ from paper_1607_03884_b200 import diagnostics, shard, synth  # noqa: E402
 
 METRIC = "states integrated/sec per global step (fp64)"
 UNIT = "states/s"
-# ALU roofline: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz; measured 36.3 TFLOP/s
-# (profiles/r2_fp64_peak.md)
+# ALU roofline: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz = 37.2 TFLOP/s; the library's DFMA
+# probe measures 34.8 TFLOP/s (profiles/r2_fp64_peak.md) and is rerun and printed by every bench run
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the integration kernel from the committed
 # `ncu --set full` captures, keyed by (config index, kernel id); None where no capture of that pair is on file.
@@ -81,6 +81,9 @@ class ClockSampler:
         reasons = [n for i, n in enumerate(names) if any(len(r) >= 7 and r[3 + i] == "Active" for r in self.rows)]
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "reasons": reasons, "samples": len(sm)}
+
+
+FLOP_CONVENTION = "+,-,*,/ = 1, fma = 2, exp/log/pow/sqrt = 20 flop each (chem_flop_model; frac_transcendental_1: 1 each)"
 
 
 def algorithmic_flops(stats, fm):
@@ -176,8 +179,8 @@ def time_config(torch, binding, gm, mech, cfg, steps, warmup, kernel, rank, worl
     stats = binding.stats_to_numpy(st)
     failed = int((stats["status"] != 0).sum())
     flops_per_launch = algorithmic_flops(stats, gm.flop_model())
+    flops_per_launch_t1 = algorithmic_flops(stats, gm.flop_model(transcendental_1=True))
     D = diagnostics.divergence_summary(stats["nstep"])
-    steps_hist = np.bincount(np.minimum(stats["nstep"], 64), minlength=65)
 
     for _ in range(warmup):
         run()
@@ -220,27 +223,54 @@ def time_config(torch, binding, gm, mech, cfg, steps, warmup, kernel, rank, worl
     torch.cuda.empty_cache()
     return dict(n=n, N=N, total_s=total_s, units=units, kernel_s=float(step_ms.mean()) * 1e-3, launches=int(launches),
                 clocks=clocks, e2e_s=e2e_s, e2e_units=e2e_units, e2e_steps=e2e_steps, failed=failed,
-                flops_per_launch=flops_per_launch, D=D, used_kernel=used_kernel, y0=y0,
-                mean_steps=float(stats["nstep"].mean()), max_steps=int(stats["nstep"].max()),
-                steps_hist=[int(v) for v in steps_hist])
+                flops_per_launch=flops_per_launch, flops_per_launch_t1=flops_per_launch_t1, D=D, used_kernel=used_kernel, y0=y0,
+                mean_steps=float(stats["nstep"].mean()), max_steps=int(stats["nstep"].max()))
 
 
 _probe = {}
 
 
 def roofline(binding, ci, r, peaks, which):
+    """The roofline record of one config.  `bound` is the roof the ALGORITHM is nearer to (algorithmic flops against the
+    fp64 peak, algorithmic bytes against the HBM peak), and achieved / peak / frac follow it.  Beside it: `hbm_frac`, the
+    share of the HBM bandwidth the kernel actually used (DRAM bytes of the committed ncu capture of this config and kernel
+    over the live kernel time; the algorithmic figure when no capture is on file), `hbm_frac_algorithmic`, and `limiter`,
+    which says "latency" when the kernel is near neither roof."""
     if "tf" not in _probe:
         _probe["tf"] = binding.chem_fp64_probe()          # outside every timed region
     achieved = r["flops_per_launch"] / r["kernel_s"] / 1e12
+    alu_frac = achieved / FP64_PEAK_TFLOPS
     traffic = NCU_TRAFFIC.get((ci, r["used_kernel"]))
-    return {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-            "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic[0] if traffic else None,
-            "traffic_source": traffic[1] if traffic else None,
-            "kernel": binding.KERNEL_NAMES.get(r["used_kernel"], "?"), "kernel_ms": 1e3 * r["kernel_s"],
-            "flops_per_launch": r["flops_per_launch"],
-            "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7, profiles/r2_fp64_peak.md)",
-            "peak_measured_dfma_probe": _probe["tf"],
-            "hbm_frac": (2 * r["n"] * r["N"] * 8 / r["kernel_s"] / 1e9) / peaks["hbm_gbs"], "hbm_peak_source": which}
+    alg_bytes = 2 * r["n"] * r["N"] * 8
+    alg_gbs = alg_bytes / r["kernel_s"] / 1e9
+    hbm_frac_alg = alg_gbs / peaks["hbm_gbs"]
+    hbm_frac = (traffic[0] / r["kernel_s"] / 1e9) / peaks["hbm_gbs"] if traffic else hbm_frac_alg
+    if alu_frac >= hbm_frac_alg:
+        head = {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": alu_frac}
+    else:
+        head = {"bound": "hbm", "achieved": alg_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm_frac_alg}
+    nearest = max(alu_frac, hbm_frac)
+    limiter = ("latency: %.0f %% of the fp64 peak and %.0f %% of the HBM bandwidth in use, neither roof is near (DESIGN.md 7)"
+               % (100 * alu_frac, 100 * hbm_frac)) if nearest < 0.5 else ("hbm" if hbm_frac > alu_frac else "alu")
+    head.update({
+        "traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None,
+        "traffic_over_algorithmic": traffic[0] / alg_bytes if traffic else None,
+        "kernel": binding.KERNEL_NAMES.get(r["used_kernel"], "?"), "kernel_ms": 1e3 * r["kernel_s"],
+        "flops_per_launch": r["flops_per_launch"], "flop_convention": FLOP_CONVENTION,
+        "alu_frac": alu_frac, "frac_transcendental_1": r["flops_per_launch_t1"] / r["kernel_s"] / 1e12 / FP64_PEAK_TFLOPS,
+        "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7, profiles/r2_fp64_peak.md)",
+        "peak_measured_dfma_probe": _probe["tf"],
+        "hbm_frac": hbm_frac, "hbm_frac_source": "ncu dram bytes / live kernel time" if traffic else "algorithmic bytes (no ncu capture on file)",
+        "hbm_frac_algorithmic": hbm_frac_alg, "hbm_peak_source": which, "limiter": limiter})
+    return head
+
+
+def summary_row(ci, name, r, roof, total_s, units, steps):
+    """compact per-config record for the `summary` array, the LAST key of the line (it survives a truncated tail)"""
+    return {"i": ci, "workload": name, "kernel": r["used_kernel"], "ms_per_step": round(1e3 * total_s / steps, 3),
+            "value": round(units / total_s, 1), "frac": round(roof["frac"], 4), "frac_t1": round(roof["frac_transcendental_1"], 4),
+            "hbm_frac": round(roof["hbm_frac"], 4), "e2e_over_device": round((r["e2e_units"] / r["e2e_s"]) / (units / total_s), 3),
+            "failed": r["failed"], "D_mean": round(r["D"]["mean"], 3) if r["D"].get("mean") is not None else None}
 
 
 def main():
@@ -286,7 +316,9 @@ def main():
     gm, _ = gm_of(cfg["kind"])
     r = time_config(torch, binding, gm, mech, cfg, args.steps, warmup, args.kernel, rank, world,
                     max(3, min(args.steps, 5)), sampler=ClockSampler(local_rank))
-    others = []
+    others, summary = [], []
+    roof = roofline(binding, args.config, r, peaks, which)
+    summary.append(summary_row(args.config, cfg["name"], r, roof, r["total_s"], r["units"], args.steps))
     if world == 1 and not args.only and args.states == 0:
         for ci, c in enumerate(synth.CONFIGS):
             if ci == args.config:
@@ -294,11 +326,13 @@ def main():
             g2, m2 = gm_of(c["kind"])
             steps2 = 20 if c["n_states"] <= 65536 else 3
             r2 = time_config(torch, binding, g2, m2, c, steps2, 3, args.kernel, rank, world, 3)
+            roof2 = roofline(binding, ci, r2, peaks, which)
+            summary.append(summary_row(ci, c["name"], r2, roof2, r2["total_s"], r2["units"], steps2))
             others.append({
                 "index": ci, "workload": c["name"], "config": config_dict(c, r2["N"], g2.n_reactions, world),
                 "value": r2["units"] / r2["total_s"], "unit": UNIT, "steps": steps2, "warmup": 3,
                 "ms_per_step": 1e3 * r2["total_s"] / steps2, "us_per_state": 1e6 * r2["total_s"] / r2["units"],
-                "roofline": roofline(binding, ci, r2, peaks, which),
+                "roofline": roof2,
                 "e2e": {"value": r2["e2e_units"] / r2["e2e_s"], "unit": UNIT, "h2d_bytes_per_step": r2["n"] * r2["N"] * 8,
                         "d2h_bytes_per_step": r2["n"] * r2["N"] * 8, "steps": r2["e2e_steps"], "host_memory": "pinned"},
                 "gpu_launches": r2["launches"], "failed_states": r2["failed"],
@@ -316,13 +350,14 @@ def main():
         "e2e": {"value": r["e2e_units"] / r["e2e_s"], "unit": UNIT, "h2d_bytes_per_step": n * N * 8, "d2h_bytes_per_step": n * N * 8,
                 "steps": r["e2e_steps"], "host_memory": "pinned"},
         "gpu_launches": r["launches"],
-        "roofline": roofline(binding, args.config, r, peaks, which),
+        "roofline": roof,
         "internal_steps": {"mean": r["mean_steps"], "max": r["max_steps"]}, "D": r["D"],
     }
     if others:
         out["configs"] = others
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(mech, cfg, r["y0"])
+    out["summary"] = sorted(summary, key=lambda x: x["i"])       # last key on purpose: one short row per config
     print(json.dumps(out))
 
 

@@ -223,6 +223,9 @@ int chem_last_kernel(const chem_mech *mech);
  * out[0] = one source-term evaluation, out[1] = one Jacobian evaluation, out[2] = one LU pair (real + complex),
  * out[3] = one Newton iteration's solves and vector work (excluding its 3 source terms), out[4] = error estimate. */
 int chem_flop_model(const chem_mech *mech, double out[5]);
+/* The same counts with every exp / log / pow / sqrt counted as 1 flop instead of the 20 of chem_flop_model's convention
+ * (bench.py reports the roofline fraction both ways). */
+int chem_flop_model_t1(const chem_mech *mech, double out[5]);
 
 /* Diagnostic, not on the hot path: the fp64 FMA rate of the device measured with dependent-free DFMA streams
  * (`iters` fused multiply-adds x 8 accumulators per thread, 8 CTAs of 256 threads per SM, best of `reps` launches, in

@@ -45,7 +45,7 @@ assert STATS_DTYPE.itemsize == 48
 
 EXPORTS = ["chem_mech_load", "chem_mech_free", "chem_mech_info", "chem_rhs", "chem_jacobian", "chem_lu_solve",
            "chem_integrate", "chem_integrate_ex", "chem_integrate_host", "chem_launch_count", "chem_flop_model",
-           "chem_last_error", "chem_last_kernel", "chem_fp64_probe", "chem_tps_radau_solve", "chem_integrate_noalloc", "chem_scratch_trim"]
+           "chem_last_error", "chem_last_kernel", "chem_fp64_probe", "chem_tps_radau_solve", "chem_integrate_noalloc", "chem_scratch_trim", "chem_flop_model_t1"]
 
 _lib = None
 
@@ -76,6 +76,7 @@ def lib():
         L.chem_integrate_host.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double,
                                           C.c_void_p, C.c_void_p, C.POINTER(chem_opts), C.c_void_p]
         L.chem_flop_model.argtypes = [C.c_void_p, _dp]
+        L.chem_flop_model_t1.argtypes = [C.c_void_p, _dp]
         L.chem_last_kernel.argtypes = [C.c_void_p]
         L.chem_fp64_probe.argtypes = [C.c_int32, C.c_int32, _dp]
         L.chem_tps_radau_solve.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_double, C.c_double, C.c_double,
@@ -137,9 +138,10 @@ class Mechanism:
         except Exception:
             pass
 
-    def flop_model(self):
+    def flop_model(self, transcendental_1=False):
+        """algorithmic flops per operation; exp/log/pow/sqrt count 20 each (the roofline convention) or 1 each"""
         out = np.empty(5)
-        _check(lib().chem_flop_model(self._h, out.ctypes.data_as(_dp)))
+        _check((lib().chem_flop_model_t1 if transcendental_1 else lib().chem_flop_model)(self._h, out.ctypes.data_as(_dp)))
         return dict(rhs=out[0], jac=out[1], lu=out[2], newton=out[3], err=out[4])
 
 

@@ -441,19 +441,25 @@ extern "C" int chem_mech_load(const chem_mech_desc *d, chem_mech **out)
     m->n_sm = n_sm;
     m->max_smem_optin = optin;
 
-    // Algorithmic flop model: +,-,*,/ count 1; exp/log/pow/log10/exp10/sqrt count kTrans each.
-    const double kTrans = 20.0, N = ns;
-    const double thermo = ns * (8.0 + 11.0 + 12.0 + 1.0) + kTrans;                      // cp, h, s (Horner), g; one log T
-    const double front = 4.0 * ns + 6.0 + ns * 2.0;                                      // closure, Wbar, rho, C_k
-    const double rx = nr * (5.0 + 2.0 * kTrans + 4.0 + 3.0) + n_slots_used * 3.0        // ln kf, Kc, 2 exp, products, q
-                      + n_tb * 2.0 + n_eff * 2.0 + n_fall * (8.0 + kTrans) + n_troe * (25.0 + 5.0 * kTrans);
-    const double wd = 2.0 * inc_rx.size() + 6.0 * ns + 4.0;                              // wdot gather, Tdot, Ydot
-    m->flops[0] = thermo + front + rx + wd + 2.0 * kTrans;
-    m->flops[1] = m->flops[0] + ns * 7.0 + nr * 40.0 + n_troe * 40.0 + 12.0 * inc_rx.size() + 2.0 * n_eff * 3.0
-                  + ns * (2.0 * N + 6.0 * N) + N * (2.0 * N + 6.0 * N);                 // derivative slots, rows, columns
-    m->flops[2] = (2.0 / 3.0) * N * N * N * 5.0 + 3.0 * N * N;                           // real LU + complex LU (4x) + forming E1, E2
-    m->flops[3] = 2.0 * N * N * 5.0 + N * (15.0 + 9.0 + 15.0 + 9.0 + 3.0);               // real + complex solves, transforms, norm
-    m->flops[4] = 2.0 * N * N + N * 10.0;                                                // error estimate: one real solve + norm
+    // Algorithmic flop model: +,-,*,/ count 1; exp/log/pow/log10/exp10/sqrt count kTrans each:
+    // 20 in flops[] (chem_flop_model, the roofline convention), 1 in flops_t1[] (chem_flop_model_t1, for the reader who
+    // wants the fraction without that convention).
+    auto flop_model = [&](double kTrans, double *fl) {
+        const double N = ns;
+        const double thermo = ns * (8.0 + 11.0 + 12.0 + 1.0) + kTrans;                      // cp, h, s (Horner), g; one log T
+        const double front = 4.0 * ns + 6.0 + ns * 2.0;                                      // closure, Wbar, rho, C_k
+        const double rx = nr * (5.0 + 2.0 * kTrans + 4.0 + 3.0) + n_slots_used * 3.0        // ln kf, Kc, 2 exp, products, q
+                          + n_tb * 2.0 + n_eff * 2.0 + n_fall * (8.0 + kTrans) + n_troe * (25.0 + 5.0 * kTrans);
+        const double wd = 2.0 * inc_rx.size() + 6.0 * ns + 4.0;                              // wdot gather, Tdot, Ydot
+        fl[0] = thermo + front + rx + wd + 2.0 * kTrans;
+        fl[1] = fl[0] + ns * 7.0 + nr * 40.0 + n_troe * 40.0 + 12.0 * inc_rx.size() + 2.0 * n_eff * 3.0
+                + ns * (2.0 * N + 6.0 * N) + N * (2.0 * N + 6.0 * N);                       // derivative slots, rows, columns
+        fl[2] = (2.0 / 3.0) * N * N * N * 5.0 + 3.0 * N * N;                                 // real LU + complex LU (4x) + forming E1, E2
+        fl[3] = 2.0 * N * N * 5.0 + N * (15.0 + 9.0 + 15.0 + 9.0 + 3.0);                     // real + complex solves, transforms, norm
+        fl[4] = 2.0 * N * N + N * 10.0;                                                      // error estimate: one real solve + norm
+    };
+    flop_model(20.0, m->flops);
+    flop_model(1.0, m->flops_t1);
     const int rcf = build_fast(d, m);
     if (rcf != CHEM_OK) { chem_mech_free(m); return rcf; }
     *out = m;
@@ -485,6 +491,13 @@ extern "C" int chem_flop_model(const chem_mech *m, double out[5])
 {
     if (!m || !out) return fail(CHEM_E_ARG, "null argument");
     for (int i = 0; i < 5; i++) out[i] = m->flops[i];
+    return CHEM_OK;
+}
+
+extern "C" int chem_flop_model_t1(const chem_mech *m, double out[5])
+{
+    if (!m || !out) return fail(CHEM_E_ARG, "null argument");
+    for (int i = 0; i < 5; i++) out[i] = m->flops_t1[i];
     return CHEM_OK;
 }
 

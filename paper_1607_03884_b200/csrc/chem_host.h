@@ -28,6 +28,7 @@ struct chem_mech {
     int max_smem_optin = 0;
     // algorithmic flop model
     double flops[5] = {0, 0, 0, 0, 0};
+    double flops_t1[5] = {0, 0, 0, 0, 0};   // the same with 1 flop per transcendental instead of 20
     chem::FastTables fast{};    // exp-job tables of the warp-per-state and thread-per-state paths, if eligible
     void *fast_blob = nullptr;
     // host-buffer entry point: two streams for chunked copy/compute overlap (created on first use)
