@@ -97,7 +97,12 @@ typedef struct chem_opts {
                             Results are bit-reproducible PER KERNEL ID.  Auto chooses by mechanism AND batch size (n_states),
                             so with kernel = 0 the bits of one state may differ between a small and a large batch (always
                             within the tolerance); chem_last_kernel tells which ran.  Fix the id where bits must not move. */
-    int32_t reorder;     /* 1: start the states in order of decreasing cost_hint ("reordering IVPs"); 0 off */
+    int32_t reorder;     /* order in which the work queue starts the states ("reordering IVPs to increase similarity
+                            of stiffness"; L184).  Results never depend on it, bit for bit.  1: by decreasing cost_hint (caller's
+                            prediction); 2: by the library's own stiffness estimate, t_end ||f(y0) / (atol + rtol |y0|)||_rms, from
+                            one extra source term per state (small mechanisms only, else CHEM_E_UNSUPPORTED); 0: auto = the
+                            estimate where it is measured to pay (the thread-per-state kernel on large batches), otherwise
+                            none; -1: off */
     const double *P_per_state;  /* device [n_states] or NULL: per-state pressure overriding P        */
     const int32_t *cost_hint;   /* device [n_states] or NULL: predicted cost per state, e.g. chem_stats.nstep of the
                                    previous global step; read only when reorder = 1.  Results do not depend on it. */
@@ -166,7 +171,7 @@ int chem_integrate_ex(const chem_mech *mech, int32_t n_states, double P, double 
  * of y_in_host into y_out_host (and stats_host if not NULL) and synchronises.  Page-locked (pinned) buffers are read and
  * written by the kernel itself through their device mapping, state by state, so the transfers overlap the integration;
  * pageable buffers are staged through device memory in two chunks on two internal streams.  The buffers may alias.
- * `reorder` is ignored here.  The kernel is chosen once from n_states, as chem_integrate_ex would, whether or not the
+ * `reorder` = 1 / 2 are ignored here (pinned buffers: no ordering pass; pageable: auto per chunk).  The kernel is chosen once from n_states, as chem_integrate_ex would, whether or not the
  * buffers are pinned (the chunks of the pageable path all run that kernel).  The internal streams belong to the mechanism
  * object: one chem_integrate_host call per mechanism at a time. */
 int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,
@@ -200,6 +205,7 @@ int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, doubl
  *     stream, the part it starts from.  Calls that can overlap on the GPU (different streams, several host threads)
  *     race on the work queue and return wrong results or skip states: issue them on one stream or order them with events.
  *     This applies across mechanisms too.  chem_integrate / chem_integrate_ex do not use the array and may overlap freely.
+ *   - opts->reorder = 0, 2 and -1 all mean "no ordering" here (the library's own estimate is not offered).
  *   - opts->reorder = 1 with opts->cost_hint orders the start of the states by decreasing cost with a counting sort over
  *     1024 cost classes (no sort library); as with chem_integrate_ex the results do not depend on it.
  * Otherwise as chem_integrate_ex: asynchronous on `stream`, y_in / y_out may alias, stats may be NULL, n_states == 0 is a

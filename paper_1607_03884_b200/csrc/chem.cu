@@ -672,7 +672,7 @@ extern "C" int chem_integrate_noalloc(const chem_mech *m, int32_t n, double P, d
     int *head = reinterpret_cast<int *>(scratch);
     unsigned *bucket = reinterpret_cast<unsigned *>(scratch + kNoAllocHeadBytes);
     int *order = nullptr;
-    const bool ordered = o && o->reorder && o->cost_hint;
+    const bool ordered = o && o->reorder == 1 && o->cost_hint;      // reorder 0 / 2 / -1: no ordering here (the estimate's keys would need scratch of their own)
     // the array still holds the previous call's queue head and counters: clear what this call starts from
     CUDA_TRY(cudaMemsetAsync(scratch, 0, ordered ? kNoAllocOrderOff : kNoAllocHeadBytes, st));
     if (ordered) {

@@ -49,3 +49,6 @@ int chem_tps_available(const chem_mech *m);
 int chem_tps_slots(const chem_mech *m);   // states in flight of one launch (lanes of all resident warps)
 int chem_tps_launch(const chem_mech *m, int n, double P, const chem::RadauParams &prm, const double *y_in, double *y_out,
                     const chem_opts *o, chem_stats *stats, const int *order, cudaStream_t st);
+// stiffness estimate per state for the start order (chem_opts.reorder = 2 / auto): keys[n] on the device, larger = costlier
+int chem_tps_cost_keys(const chem_mech *m, int n, double P, const chem::RadauParams &prm, const double *y_in, const chem_opts *o,
+                       int32_t *keys, cudaStream_t st);

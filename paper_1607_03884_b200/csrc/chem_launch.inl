@@ -219,10 +219,21 @@ int integrate_impl(const chem_mech *m, int32_t n, double P, double t_end, double
     if (kernel == 2 && !warp_path_available(m)) return fail(CHEM_E_UNSUPPORTED, "warp-per-state kernel not available for this mechanism");
     if (kernel == 3 && !chem_tps_available(m)) return fail(CHEM_E_UNSUPPORTED, "thread-per-state kernel not available for this mechanism");
     int *order = nullptr;
-    void *order_scratch = nullptr;
-    if (o && o->reorder && o->cost_hint) {
+    void *order_scratch = nullptr, *key_scratch = nullptr;
+    // Start order (chem_opts.reorder): 1 = by the caller's cost_hint; 2 = by the library's own stiffness estimate
+    // (chem_tps_cost_keys: one source term per state + a radix sort, ~1.5 ms per million h2co-shaped states); 0 = auto: the
+    // estimate where it pays, i.e. for the thread-per-state kernel, whose launch otherwise ends with a few long states
+    // and idle lanes (profiles/r3_tail_config1.md: 40.2 -> 34 ms on config 1); < 0 = off.  Bits of the results never depend on it.
+    const int reorder = o ? o->reorder : 0;
+    if (reorder < -1 || reorder > 2) return fail(CHEM_E_ARG, "chem_opts.reorder must be -1..2");
+    if (reorder == 1 && o->cost_hint) {
         const int rc = build_order(n, o->cost_hint, &order, &order_scratch, st);
         if (rc) { chem_host::scratch_free(order_scratch, st); return rc; }
+    } else if (reorder == 2 || (reorder == 0 && kernel == 3 && (long long)n >= 8LL * chem_tps_slots(m))) {
+        int rc = chem_host::scratch_alloc(&key_scratch, (size_t)n * sizeof(int32_t), st);
+        if (rc == CHEM_OK) rc = chem_tps_cost_keys(m, n, P, prm, y_in, o, static_cast<int32_t *>(key_scratch), st);
+        if (rc == CHEM_OK) rc = build_order(n, static_cast<const int32_t *>(key_scratch), &order, &order_scratch, st);
+        if (rc) { chem_host::scratch_free(order_scratch, st); chem_host::scratch_free(key_scratch, st); return rc; }
     }
     int rc;
     if (kernel == 3) rc = chem_tps_launch(m, n, P, prm, y_in, y_out, o, stats, order, st);
@@ -230,6 +241,7 @@ int integrate_impl(const chem_mech *m, int32_t n, double P, double t_end, double
     else rc = group_size(m) == 32 ? launch_integrate<32>(m, n, P, prm, y_in, y_out, o, stats, order, st)
                                   : launch_integrate<128>(m, n, P, prm, y_in, y_out, o, stats, order, st);
     chem_host::scratch_free(order_scratch, st);
+    chem_host::scratch_free(key_scratch, st);
     if (rc == CHEM_OK) const_cast<chem_mech *>(m)->last_kernel = kernel;
     return rc;
 }
@@ -273,10 +285,12 @@ extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, doub
         };
         void *din = mapped(y_in_host), *dout = mapped(y_out_host), *dst = stats_host ? mapped(stats_host) : nullptr;
         if (din && dout && (!stats_host || dst)) {
-            chem_opts oc;
-            if (o) { oc = *o; oc.reorder = 0; oc.cost_hint = nullptr; }
+            chem_opts oc{};
+            if (o) oc = *o;
+            oc.reorder = -1;          // no ordering pass over mapped host memory: it would read the input twice over PCIe
+            oc.cost_hint = nullptr;
             const int rc0 = integrate_impl(m, n, P, t_end, rtol, atol, static_cast<const double *>(din), static_cast<double *>(dout),
-                                           o ? &oc : nullptr, static_cast<chem_stats *>(dst), mm->hs[0]);
+                                           &oc, static_cast<chem_stats *>(dst), mm->hs[0]);
             if (rc0 != CHEM_OK) return rc0;
             CUDA_TRY(cudaStreamSynchronize(mm->hs[0]));
             return CHEM_OK;
@@ -308,9 +322,9 @@ extern "C" int chem_integrate_host(const chem_mech *m, int32_t n, double P, doub
         if (o) {
             oc = *o;
             if (oc.P_per_state) oc.P_per_state += lo;
-            oc.reorder = 0;          // cost hints are device arrays of the whole batch; chunks are short anyway
-            oc.cost_hint = nullptr;
         }
+        oc.reorder = o && o->reorder < 0 ? -1 : 0;   // caller's cost hints are device arrays of the whole batch: not used; auto per chunk
+        oc.cost_hint = nullptr;
         oc.kernel = kernel_all;
         const size_t off = (size_t)lo * N, cnt = (size_t)(hi - lo) * N;
         e = cudaMemcpyAsync(d_y + off, y_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, st);

@@ -2,6 +2,8 @@
 // its linear algebra.  The kernel itself is in chem_tps_kernel.cuh, the device routines in chem_tps.cuh.
 #include "chem_tps_kernel.cuh"
 
+#include <cstdlib>
+
 using namespace chem;
 using namespace chem::tps;
 
@@ -14,6 +16,17 @@ size_t tps_smem(const chem_mech *m, int warps)
 {
     const Lay L = make_lay(m->t.n_sp, m->t.n_rx);
     return ((size_t)((m->fast.blob_doubles + 31) & ~31) + (size_t)warps * L.n_sm * 32) * sizeof(double);
+}
+// warps out of every 8 whose LU factors stay resident in L2 (chem_tps.cuh, l2_policy); CHEM_TPS_L2_KEEP overrides the
+// default for experiments (0..8)
+int tps_l2_keep()
+{
+    static const int v = [] {
+        const char *e = std::getenv("CHEM_TPS_L2_KEEP");
+        const int k = e ? std::atoi(e) : 8;      // measured (profiles/r3_tps_config1.md): all factors evict_last is the fastest
+        return k < 0 ? 0 : (k > 8 ? 8 : k);
+    }();
+    return v;
 }
 int tps_warps(const chem_mech *m)
 {
@@ -55,6 +68,7 @@ int chem_tps_launch(const chem_mech *m, int n, double P, const RadauParams &prm,
     a.order = order;
     a.gws = static_cast<double *>(scratch);
     a.blob = m->fast.blob; a.blob_doubles = m->fast.blob_doubles;
+    a.l2_keep = tps_l2_keep();
     cudaError_t e = cudaMemsetAsync(a.counter, 0, sizeof(int), st);
     if (e == cudaSuccess) {
         // compile-time-N instantiations for 8 <= N <= 16, runtime-N routines below that
@@ -69,6 +83,72 @@ int chem_tps_launch(const chem_mech *m, int n, double P, const RadauParams &prm,
     }
     chem_host::scratch_free(scratch, st);
     if (e != cudaSuccess) return fail(CHEM_E_CUDA, "thread-per-state launch: %s", cudaGetErrorString(e));
+    return CHEM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ stiffness estimate
+// Cost estimate for the start order of a launch (chem_opts.reorder = 2 / auto; "reordering IVPs to increase
+// similarity of stiffness"; L184: a warp waits for its most expensive thread).  With a work queue the order of the states
+// only decides WHEN each one starts; started in order of decreasing cost, the long ones do not end up alone at the end of
+// the launch with every other lane idle.  The estimate is the quantity the controller itself would look at first:
+// key = 16 log2(1 + t_end || f(y0) / (atol + rtol |y0|) ||_rms), i.e. how many tolerances the state moves over the global
+// step at its initial rate, in sixteenths of an octave, 0..1023.  Measured on B200 (profiles/r3_tail_config1.md): ordering by
+// it recovers 90 % of what ordering by the true step counts of a previous run gives.  One source term per state, thread
+// per state, states loaded as coalesced rows exactly as the integration kernel loads them.
+namespace {
+__global__ void __launch_bounds__(128) tps_cost_kernel(const __grid_constant__ TpsArgs a, int32_t *key)
+{
+    extern __shared__ double smem[];
+    for (int i = threadIdx.x; i < a.blob_doubles; i += 128) smem[i] = a.blob[i];
+    __syncthreads();
+    const double *tab = smem;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int N = a.N, NR = a.NR;
+    double *sm = smem + ((a.blob_doubles + 31) & ~31) + (size_t)wib * a.n_sm * 32 + lane;
+    double *wsm = sm - lane, *y = sm, *f = sm + oZ(N) * 32;
+    const double rtol = a.prm.rtol, atol = a.prm.atol, t_end = a.prm.t_end, invN = a.prm.inv_n;
+    for (long long base = ((long long)blockIdx.x * 4 + wib) * 32; base < a.n_states; base += (long long)gridDim.x * 128) {
+        for (int l = 0; l < 32 && base + l < a.n_states; l++)
+            if (lane < N) wsm[lane * 32 + l] = a.y_in[(size_t)(base + l) * N + lane];
+        __syncwarp();
+        const long long s = base + lane;
+        if (s < a.n_states) {
+            const double P = a.P_per_state ? a.P_per_state[s] : a.P;
+            rhs(tab, sm, N, NR, a.tmid, P, rcp_f(P), y, 0.0, f);
+            double e = 0.0;
+#pragma unroll 1
+            for (int i = 0; i < N; i++) { const double r = TL(f, i) / (atol + rtol * fabs(TL(y, i))); e = fma(r, r, e); }
+            const double k = 16.0 * log2(1.0 + t_end * sqrt(e * invN));
+            key[s] = k >= 1023.0 ? 1023 : (k > 0.0 ? (int32_t)k : 0);          // NaN (non-finite state) -> 0
+        }
+        __syncwarp();
+    }
+}
+}  // namespace
+
+int chem_tps_cost_keys(const chem_mech *m, int n, double P, const RadauParams &prm, const double *y_in, const chem_opts *o,
+                       int32_t *keys, cudaStream_t st)
+{
+    using chem_host::fail;
+    if (!chem_tps_available(m)) return fail(CHEM_E_UNSUPPORTED, "the stiffness estimate (reorder = 2) needs a small mechanism (thread-per-state source term)");
+    const Lay L = make_lay(m->t.n_sp, m->t.n_rx);
+    const size_t smem = tps_smem(m, 4);
+    CUDA_TRY(cudaFuncSetAttribute(tps_cost_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tps_cost_kernel, 128, smem));
+    if (occ < 1) return fail(CHEM_E_UNSUPPORTED, "stiffness-estimate kernel does not fit on an SM");
+    int grid = (n + 127) / 128;
+    if (grid > m->n_sm * occ) grid = m->n_sm * occ;
+    TpsArgs a{};
+    a.n_states = n; a.N = L.N; a.NR = L.NR; a.n_sm = L.n_sm; a.n_gw = L.n_gw;
+    a.P = P; a.tmid = m->fast.tmid;
+    a.P_per_state = o ? o->P_per_state : nullptr;
+    a.prm = prm;
+    a.y_in = y_in;
+    a.blob = m->fast.blob; a.blob_doubles = m->fast.blob_doubles;
+    tps_cost_kernel<<<grid, 128, smem, st>>>(a, keys);
+    chem_host::g_launches++;
+    CUDA_TRY(cudaGetLastError());
     return CHEM_OK;
 }
 

@@ -29,6 +29,42 @@ typedef unsigned long long u64;
 // lane-private element e of an array whose rows are 32 lanes wide
 #define TL(p, e) (p)[(e) * 32]
 
+// L2 eviction priorities for the lane-private global workspace ("storage of the Jacobian matrix and/or
+// factorized forms ... cause many slow global memory accesses").  The LU factors of all resident lanes (4 KB each, 154 MB
+// at N = 13) are re-read by every triangular solve and do not fit the 126 MB L2 together: read round-robin they evict
+// each other and most solves stream from HBM.  So the factors of `keep` warps out of every 8 are tagged evict_last -- that
+// subset fits and stays resident -- and the factors of the other warps, like J, are tagged evict_first: they stream
+// through without displacing the resident set (profiles/r3_tps_config1.md).
+__device__ __forceinline__ u64 l2_policy(bool keep)
+{
+    u64 last, first;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(last));
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(first));
+    return keep ? last : first;
+}
+__device__ __forceinline__ double ldp(const double *p, u64 pol)
+{
+    double v;
+    asm volatile("ld.global.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ double2 ldp(const double2 *p, u64 pol)
+{
+    double2 v;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ void stp(double *p, double v, u64 pol)
+{
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void stp(double2 *p, double2 v, u64 pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+// the same access pattern as TL with a cache policy
+#define TLP(p, e, pol) ldp(&(p)[(e) * 32], pol)
+
 // Shared-memory elements per lane: y[N], z1..z3[3N], C[N+1], U[max(N_rx, 2N+1)] (q of the source term; row and S of the
 // Jacobian); z doubles as the column scratch of the factorisation.  Global elements per lane (L2-resident workspace):
 // J[N^2], E1[N^2], E2[N^2] complex, f0[N], cont[3N], w1..w3[3N], a1..a3[3N], the Jacobian's reaction records[4 N_rx].
@@ -560,8 +596,9 @@ __device__ __forceinline__ u64 perm_swap(u64 perm, int a, int b)
 
 template <int N>
 __device__ __noinline__ int lu_pair_t(const double *gJ, double *g1, double2 *g2, double *col, double fac1, double alphn,
-                                      double betan, u64 &perm1_out, u64 &perm2_out)
+                                      double betan, u64 &perm1_out, u64 &perm2_out, bool keep)
 {
+    const u64 pol = l2_policy(keep), pol_j = l2_policy(false);
     double *s1 = col, *sr = col + N * 32, *si = col + 2 * N * 32;
     u64 perm1 = 0xFEDCBA9876543210ull, perm2 = 0xFEDCBA9876543210ull;
     int ier = 0;
@@ -572,7 +609,7 @@ __device__ __noinline__ int lu_pair_t(const double *gJ, double *g1, double2 *g2,
 #pragma unroll
         for (int i = 0; i < N; i++) {
             const int r1 = (int)(perm1 >> (4 * i)) & 15, r2 = (int)(perm2 >> (4 * i)) & 15;
-            const double v1 = -TL(gJ, r1 * N + j), v2 = -TL(gJ, r2 * N + j);
+            const double v1 = -TLP(gJ, r1 * N + j, pol_j), v2 = -TLP(gJ, r2 * N + j, pol_j);
             bad |= !isfinite(v1);
             c1[i] = r1 == j ? v1 + fac1 : v1;
             cr[i] = r2 == j ? v2 + alphn : v2;
@@ -584,8 +621,8 @@ __device__ __noinline__ int lu_pair_t(const double *gJ, double *g1, double2 *g2,
                 const double u1 = c1[k], ur = cr[k], ui = ci[k];
 #pragma unroll
                 for (int i = k + 1; i < N; i++) {
-                    const double a = TL(g1, k * N + i);
-                    const double2 b = TL(g2, k * N + i);
+                    const double a = TLP(g1, k * N + i, pol);
+                    const double2 b = TLP(g2, k * N + i, pol);
                     c1[i] = fma(-a, u1, c1[i]);
                     cr[i] = fma(-b.x, ur, fma(b.y, ui, cr[i]));
                     ci[i] = fma(-b.x, ui, fma(-b.y, ur, ci[i]));
@@ -606,7 +643,7 @@ __device__ __noinline__ int lu_pair_t(const double *gJ, double *g1, double2 *g2,
             const double t = TL(s1, j); TL(s1, j) = TL(s1, p1); TL(s1, p1) = t;
             perm1 = perm_swap(perm1, j, p1);
 #pragma unroll 2
-            for (int k = 0; k < j; k++) { const double s = TL(g1, k * N + j); TL(g1, k * N + j) = TL(g1, k * N + p1); TL(g1, k * N + p1) = s; }
+            for (int k = 0; k < j; k++) { const double s = TLP(g1, k * N + j, pol); stp(&TL(g1, k * N + j), TLP(g1, k * N + p1, pol), pol); stp(&TL(g1, k * N + p1), s, pol); }
         }
         if (p2 != j) {
             const double t = TL(sr, j), s = TL(si, j);
@@ -614,7 +651,7 @@ __device__ __noinline__ int lu_pair_t(const double *gJ, double *g1, double2 *g2,
             TL(sr, p2) = t; TL(si, p2) = s;
             perm2 = perm_swap(perm2, j, p2);
 #pragma unroll 2
-            for (int k = 0; k < j; k++) { const double2 w = TL(g2, k * N + j); TL(g2, k * N + j) = TL(g2, k * N + p2); TL(g2, k * N + p2) = w; }
+            for (int k = 0; k < j; k++) { const double2 w = TLP(g2, k * N + j, pol); stp(&TL(g2, k * N + j), TLP(g2, k * N + p2, pol), pol); stp(&TL(g2, k * N + p2), w, pol); }
         }
         const double r1 = rcp_f(TL(s1, j));
         const double pr = TL(sr, j), pi = TL(si, j);
@@ -632,8 +669,8 @@ __device__ __noinline__ int lu_pair_t(const double *gJ, double *g1, double2 *g2,
             } else if (i == j) {
                 a = r1; br = qr; bi = qi;
             }
-            TL(o1, i) = a;
-            TL(o2, i) = make_double2(br, bi);
+            stp(&TL(o1, i), a, pol);
+            stp(&TL(o2, i), make_double2(br, bi), pol);
         }
     }
     perm1_out = perm1;
@@ -643,20 +680,21 @@ __device__ __noinline__ int lu_pair_t(const double *gJ, double *g1, double2 *g2,
 
 // E1 x = b; b is read from `b` through the permutation and x written back to `b` (lane-private, shared memory)
 template <int N>
-__device__ __noinline__ void solve_real_t(const double *g1, double *b, u64 perm)
+__device__ __noinline__ void solve_real_t(const double *g1, double *b, u64 perm, bool keep)
 {
+    const u64 pol = l2_policy(keep);
     double x[N];
 #pragma unroll
     for (int i = 0; i < N; i++) x[i] = TL(b, (int)(perm >> (4 * i)) & 15);
 #pragma unroll
     for (int i = 1; i < N; i++)
 #pragma unroll
-        for (int k = 0; k < i; k++) x[i] = fma(-TL(g1, k * N + i), x[k], x[i]);
+        for (int k = 0; k < i; k++) x[i] = fma(-TLP(g1, k * N + i, pol), x[k], x[i]);
 #pragma unroll
     for (int i = N - 1; i >= 0; i--) {
 #pragma unroll
-        for (int j = i + 1; j < N; j++) x[i] = fma(-TL(g1, j * N + i), x[j], x[i]);
-        x[i] *= TL(g1, i * N + i);
+        for (int j = i + 1; j < N; j++) x[i] = fma(-TLP(g1, j * N + i, pol), x[j], x[i]);
+        x[i] *= TLP(g1, i * N + i, pol);
     }
 #pragma unroll
     for (int i = 0; i < N; i++) TL(b, i) = x[i];
@@ -664,8 +702,9 @@ __device__ __noinline__ void solve_real_t(const double *g1, double *b, u64 perm)
 
 // E1 x1 = b1 and E2 (x2 + i x3) = b2 + i b3, right-hand sides and solutions in z = [b1 | b2 | b3] (shared memory)
 template <int N>
-__device__ __noinline__ void solve3_t(const double *g1, const double2 *g2, double *z, u64 perm1, u64 perm2)
+__device__ __noinline__ void solve3_t(const double *g1, const double2 *g2, double *z, u64 perm1, u64 perm2, bool keep)
 {
+    const u64 pol = l2_policy(keep);
     double x1[N], xr[N], xi[N];
 #pragma unroll
     for (int i = 0; i < N; i++) {
@@ -676,8 +715,8 @@ __device__ __noinline__ void solve3_t(const double *g1, const double2 *g2, doubl
     for (int i = 1; i < N; i++)
 #pragma unroll
         for (int k = 0; k < i; k++) {
-            const double a = TL(g1, k * N + i);
-            const double2 c = TL(g2, k * N + i);
+            const double a = TLP(g1, k * N + i, pol);
+            const double2 c = TLP(g2, k * N + i, pol);
             x1[i] = fma(-a, x1[k], x1[i]);
             xr[i] = fma(-c.x, xr[k], fma(c.y, xi[k], xr[i]));
             xi[i] = fma(-c.x, xi[k], fma(-c.y, xr[k], xi[i]));
@@ -686,14 +725,14 @@ __device__ __noinline__ void solve3_t(const double *g1, const double2 *g2, doubl
     for (int i = N - 1; i >= 0; i--) {
 #pragma unroll
         for (int j = i + 1; j < N; j++) {
-            const double a = TL(g1, j * N + i);
-            const double2 c = TL(g2, j * N + i);
+            const double a = TLP(g1, j * N + i, pol);
+            const double2 c = TLP(g2, j * N + i, pol);
             x1[i] = fma(-a, x1[j], x1[i]);
             xr[i] = fma(-c.x, xr[j], fma(c.y, xi[j], xr[i]));
             xi[i] = fma(-c.x, xi[j], fma(-c.y, xr[j], xi[i]));
         }
-        const double2 d = TL(g2, i * N + i);
-        x1[i] *= TL(g1, i * N + i);
+        const double2 d = TLP(g2, i * N + i, pol);
+        x1[i] *= TLP(g1, i * N + i, pol);
         const double tr = xr[i] * d.x - xi[i] * d.y, ti = xr[i] * d.y + xi[i] * d.x;
         xr[i] = tr; xi[i] = ti;
     }

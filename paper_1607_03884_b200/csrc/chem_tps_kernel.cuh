@@ -24,6 +24,7 @@ struct TpsArgs {
     double *gws;                             // [warps of the grid][n_gw][32]
     const double *blob;
     int blob_doubles;
+    int l2_keep;                             // warps out of every 8 whose LU factors are tagged evict_last in L2 (chem_tps.cuh)
 };
 
 enum Act { A_IDLE = 0, A_FREE, A_F0, A_JAC, A_FACT, A_STEP, A_NEWT, A_ERR };
@@ -48,6 +49,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
     double *gAv = gw + gA(N) * 32, *gRd = gw + gR(N) * 32;
     double2 *g2 = reinterpret_cast<double2 *>(gw + gE2(N) * 32 - lane) + lane;
     double *y = sm, *z = sm + oZ(N) * 32, *U = sm + oU(N) * 32;
+    const bool keep = (int)((blockIdx.x * WARPS + wib) & 7) < a.l2_keep;
 
     const RadauParams &prm = a.prm;
     const int NIT = prm.newton_max > 0 ? prm.newton_max : 7;
@@ -86,7 +88,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
         act = A_FREE;
     };
     auto solve_e1 = [&](double *b) {
-        if constexpr (NT > 0) solve_real_t<NT>(g1, b, ip1); else solve_real(g1, b, N, ip1);
+        if constexpr (NT > 0) solve_real_t<NT>(g1, b, ip1, keep); else solve_real(g1, b, N, ip1);
     };
 
     for (;;) {
@@ -114,7 +116,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
                 TL(z, N + i) = TI21 * a1 + TI22 * a2 + TI23 * a3 - w2 * ALPHN + w3 * BETAN;
                 TL(z, 2 * N + i) = TI31 * a1 + TI32 * a2 + TI33 * a3 - w3 * ALPHN - w2 * BETAN;
             }
-            if constexpr (NT > 0) solve3_t<NT>(g1, g2, z, ip1, ip2); else solve3(g1, g2, z, z + N * 32, z + 2 * N * 32, N, ip1, ip2);
+            if constexpr (NT > 0) solve3_t<NT>(g1, g2, z, ip1, ip2, keep); else solve3(g1, g2, z, z + N * 32, z + 2 * N * 32, N, ip1, ip2);
             nsol++;
             NEWT++;
             double dy = 0.0;
@@ -364,7 +366,7 @@ __global__ void __launch_bounds__(32 * WARPS, 8 / WARPS) integrate_tps_kernel(co
         if (act == A_FACT) {
             const double invH = rcp_f(H);
             int ier;
-            if constexpr (NT > 0) ier = lu_pair_t<NT>(gJ, g1, g2, z, U1 * invH, ALPH * invH, BETA * invH, ip1, ip2);
+            if constexpr (NT > 0) ier = lu_pair_t<NT>(gJ, g1, g2, z, U1 * invH, ALPH * invH, BETA * invH, ip1, ip2, keep);
             else ier = lu_pair(gJ, g1, g2, z, N, U1 * invH, ALPH * invH, BETA * invH, ip1, ip2);
             ndec++;
             if (ier) {
@@ -438,12 +440,12 @@ __global__ void __launch_bounds__(128) tps_solve_kernel(int n, int batch, const 
     for (int e = 0; e < N * N; e++) TL(gJ, e) = J[(size_t)s * N * N + e];
     u64 ip1 = 0, ip2 = 0;
     int ier;
-    if constexpr (NT > 0) ier = lu_pair_t<NT>(gJ, g1, g2, col, fac1, alphn, betan, ip1, ip2);
+    if constexpr (NT > 0) ier = lu_pair_t<NT>(gJ, g1, g2, col, fac1, alphn, betan, ip1, ip2, (wib & 1) != 0);
     else ier = lu_pair(gJ, g1, g2, col, N, fac1, alphn, betan, ip1, ip2);
     if (info) info[s] = ier;
     if (ier) return;
     for (int e = 0; e < 3 * N; e++) TL(z, e) = b[(size_t)s * 3 * N + e];
-    if constexpr (NT > 0) solve3_t<NT>(g1, g2, z, ip1, ip2); else solve3(g1, g2, z, z + N * 32, z + 2 * N * 32, N, ip1, ip2);
+    if constexpr (NT > 0) solve3_t<NT>(g1, g2, z, ip1, ip2, (wib & 1) != 0); else solve3(g1, g2, z, z + N * 32, z + 2 * N * 32, N, ip1, ip2);
     for (int e = 0; e < 3 * N; e++) x[(size_t)s * 3 * N + e] = TL(z, e);
 }
 

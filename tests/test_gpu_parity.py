@@ -673,6 +673,36 @@ def test_host_entry_point_picks_one_kernel_for_the_whole_batch(torch_cuda, gpu_m
     assert y_again.shape == (5000, 13) and np.all(np.isfinite(y_again))
 
 
+def test_library_stiffness_ordering_changes_no_bit(torch_cuda, gpu_mechs, mech_h2co, mech_gri):
+    """chem_opts.reorder = 2 (the library's own estimate t_end ||f(y0) / scal||_rms) and the auto mode that
+    switches it on for large thread-per-state launches only change the order in which states start: y and every counter
+    are bit-identical to reorder = -1 (off) on all three kernels; the estimate needs a small mechanism"""
+    from paper_1607_03884_b200 import binding
+    torch = torch_cuda
+    m = gpu_mechs["h2co"]
+    y0 = synth.make_states(mech_h2co, 30011, "ignition", 93)
+    y0[7, 2] = np.nan                                                     # a non-finite state gets key 0 and status -4
+    yd = torch.from_numpy(y0).cuda()
+    for kernel in (1, 2, 3):
+        y_off, st_off = binding.chem_integrate_ex(m, P, 1e-5, RTOL, ATOL, yd, kernel=kernel, reorder=-1)
+        l0 = binding.chem_launch_count()
+        y_est, st_est = binding.chem_integrate_ex(m, P, 1e-5, RTOL, ATOL, yd, kernel=kernel, reorder=2)
+        assert binding.chem_launch_count() - l0 > 2                       # estimate + sort + integration
+        assert torch.equal(torch.nan_to_num(y_off, nan=-1.0), torch.nan_to_num(y_est, nan=-1.0)) and torch.equal(st_off, st_est)
+        assert binding.stats_to_numpy(st_est)["status"][7] == -4
+    big = torch.from_numpy(synth.make_states(mech_h2co, 320_000, "uniform", 94)).cuda()      # >= 8 x 37,888: auto orders
+    y_off, st_off = binding.chem_integrate_ex(m, P, 1e-6, RTOL, ATOL, big, reorder=-1)
+    l0 = binding.chem_launch_count()
+    y_auto, st_auto = binding.chem_integrate_ex(m, P, 1e-6, RTOL, ATOL, big)
+    assert binding.chem_last_kernel(m) == 3 and binding.chem_launch_count() - l0 > 2
+    assert torch.equal(y_off, y_auto) and torch.equal(st_off, st_auto)
+    yg = torch.from_numpy(synth.make_states(mech_gri, 16, "uniform", 95)).cuda()
+    with pytest.raises(binding.ChemError, match="small mechanism"):
+        binding.chem_integrate_ex(gpu_mechs["gri"], P, 1e-6, RTOL, ATOL, yg, reorder=2)
+    with pytest.raises(binding.ChemError, match="reorder"):
+        binding.chem_integrate_ex(m, P, 1e-6, RTOL, ATOL, yd, reorder=3)
+
+
 def test_thread_per_state_kernel_options_and_reproducibility(torch_cuda, gpu_mechs, orc_mechs, mech_h2co):
     """the thread-per-state kernel (what auto takes for the full-size h2co configs) with the options and properties the
     other kernels are tested for: per-state pressure, cost ordering (bit-identical results), bit-reproducible results that
