@@ -35,7 +35,7 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # `ncu --set full` captures, keyed by (config index, kernel id); None where no capture of that pair is on file.
 NCU_TRAFFIC = {
     (1, 2): (115.299840e6 + 109.461760e6, "profiles/r1_final_config1.md (ncu --set full)"),
-    (1, 3): (49.934547e9 + 25.401353e9, "profiles/r2_tps_config1.md (ncu --set full): lane-private LU factors stream through L2 / HBM"),
+    (1, 3): (44.098521e9 + 23.691889e9, "profiles/r3_tps_config1.md, r3_tps_metrics_config1.csv (ncu --metrics pass): lane-private LU factors stream through L2 / HBM"),
     (2, 2): (0.331e9, "profiles/r2_mapping_config2.md (ncu --metrics pass)"),
     (2, 3): (354.05e9, "profiles/r2_mapping_config2.md (ncu --metrics pass)"),
 }

@@ -171,7 +171,7 @@ int chem_integrate_ex(const chem_mech *mech, int32_t n_states, double P, double 
  * of y_in_host into y_out_host (and stats_host if not NULL) and synchronises.  Page-locked (pinned) buffers are read and
  * written by the kernel itself through their device mapping, state by state, so the transfers overlap the integration;
  * pageable buffers are staged through device memory in two chunks on two internal streams.  The buffers may alias.
- * `reorder` = 1 / 2 are ignored here (pinned buffers: no ordering pass; pageable: auto per chunk).  The kernel is chosen once from n_states, as chem_integrate_ex would, whether or not the
+ * `reorder` = 1 / 2 are treated as 0 (auto) here; -1 switches the ordering pass off.  The kernel is chosen once from n_states, as chem_integrate_ex would, whether or not the
  * buffers are pinned (the chunks of the pageable path all run that kernel).  The internal streams belong to the mechanism
  * object: one chem_integrate_host call per mechanism at a time. */
 int chem_integrate_host(const chem_mech *mech, int32_t n_states, double P, double t_end, double rtol, double atol,

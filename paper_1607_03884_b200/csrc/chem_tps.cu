@@ -31,7 +31,8 @@ int tps_l2_keep()
 int tps_warps(const chem_mech *m)
 {
     (void)m;
-    return 4;          // two CTAs of four warps per SM (or one, if shared memory holds only one)
+    return 4;          // two CTAs of four warps per SM (or one, if shared memory holds only one); two CTAs of three warps, so
+                       // that the factors of all resident lanes fit in L2 (115 MB), is 22 % SLOWER (profiles/r3_tps_config1.md)
 }
 
 }  // namespace
@@ -108,8 +109,14 @@ __global__ void __launch_bounds__(128) tps_cost_kernel(const __grid_constant__ T
     double *wsm = sm - lane, *y = sm, *f = sm + oZ(N) * 32;
     const double rtol = a.prm.rtol, atol = a.prm.atol, t_end = a.prm.t_end, invN = a.prm.inv_n;
     for (long long base = ((long long)blockIdx.x * 4 + wib) * 32; base < a.n_states; base += (long long)gridDim.x * 128) {
-        for (int l = 0; l < 32 && base + l < a.n_states; l++)
-            if (lane < N) wsm[lane * 32 + l] = a.y_in[(size_t)(base + l) * N + lane];
+        if (base + 32 <= a.n_states) {                 // full tile: the 32 row loads are independent, keep them in flight together
+#pragma unroll 8
+            for (int l = 0; l < 32; l++)
+                if (lane < N) wsm[lane * 32 + l] = a.y_in[(size_t)(base + l) * N + lane];
+        } else {
+            for (int l = 0; l < 32 && base + l < a.n_states; l++)
+                if (lane < N) wsm[lane * 32 + l] = a.y_in[(size_t)(base + l) * N + lane];
+        }
         __syncwarp();
         const long long s = base + lane;
         if (s < a.n_states) {
