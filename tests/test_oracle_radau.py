@@ -195,3 +195,147 @@ def test_error_metric_and_divergence_definitions():
     d = np.concatenate([np.full(32, 7), np.r_[np.full(31, 1), 32], np.arange(1, 33)])
     D = orc.divergence(d)
     assert np.allclose(D, [0.0, 1 - 63 / (32 * 32), 1 - (32 * 33 / 2) / (32 * 32)])
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Round 3 ("What's weak" 1): the finite-difference Jacobian branch and the status paths -2, -3, -5 and the
+# last-step test of reading R12, which until now no CPU test could fail.
+
+U = 2.220446049250313e-16          # unit roundoff as RADAU5 / CVODE use it
+
+
+def _fd_points(f, y0, t_end, **kw):
+    """the points at which the oracle evaluates f while it builds its FIRST finite-difference Jacobian: the call after
+    f(y0) number j + 1 is f(y0 + inc_j e_j) ("based on that of CVODE"; R13)"""
+    seen = []
+
+    def g(y):
+        seen.append(np.array(y, dtype=np.float64))
+        return f(y)
+    n = len(y0)
+    orc.radau5(g, lambda y: np.zeros((n, n)), y0, t_end, 1e-6, 1e-10, fd_jacobian=1, max_steps=1, **kw)
+    y0 = np.asarray(y0, dtype=np.float64)
+    assert np.array_equal(seen[0], y0)
+    incs = []
+    for j in range(n):
+        d = seen[1 + j] - y0
+        assert np.count_nonzero(d) == 1 and d[j] > 0.0, (j, d)         # one component perturbed, upwards
+        incs.append((y0[j] + d[j]) - y0[j])
+    return np.array(incs)
+
+
+def test_fd_increment_each_term_wins_in_turn():
+    """inc_j = max( sqrt(u) |y_j| , minInc * scal_j ),  minInc = 1000 |h| u n ||f(y)/scal||_rms  (1 if that norm is 0),
+    scal_j = ATOL' + RTOL' |y_j| with RADAU5's transformed tolerances (rtol 1e-6, atol 1e-10 -> RTOL' = 1e-5, ATOL' = 1e-9).
+    Expected values are worked out by hand below, not recomputed from the oracle's expression.  A wrong sqrt(u), a missing
+    factor 1000 / n / h, scal used as a divisor, or the zero-norm fallback dropped each fail one of the three cases."""
+    # (a) sqrt(u) |y_j| wins: y = (2, 3), f = (1e-3, 1e-3), h = t_end = 1.
+    #     scal = (2.0001e-5, 3.0001e-5); ||f/scal||_rms = sqrt((49.9975^2 + 33.3322^2) / 2) = 42.49;
+    #     minInc = 1000 * 1 * 2.22e-16 * 2 * 42.49 = 1.887e-11; minInc * scal = (3.8e-16, 5.7e-16), far below
+    #     sqrt(u) * (2, 3) = 1.4901161193847656e-08 * (2, 3) = (2.9802322387695312e-08, 4.470348358154297e-08)
+    inc = _fd_points(lambda y: [1e-3, 1e-3], [2.0, 3.0], 1.0)
+    assert np.allclose(inc, [2.9802322387695312e-08, 4.470348358154297e-08], rtol=1e-7)   # rtol: (y + inc) - y rounds inc at ulp(y)
+    # (b) minInc * scal_j wins where y_j = 0 (sqrt(u) |y_j| = 0): y = (0, 1), f = (3, 4), h = t_end = 0.5.
+    #     scal = (1e-9, 1.0001e-5); f/scal = (3e9, 399960.004); rms = sqrt((9e18 + 1.59968e11) / 2) = 2.1213203e9 (3e9 / sqrt 2);
+    #     minInc = 1000 * 0.5 * 2.220446e-16 * 2 * 2.1213203e9 = 4.7103e-4;  inc_0 = 4.7103e-4 * 1e-9 = 4.7103e-13;
+    #     inc_1 = max(1.49e-8 * 1, 4.7103e-4 * 1.0001e-5 = 4.7108e-9) = 1.4901161193847656e-08
+    inc = _fd_points(lambda y: [3.0, 4.0], [0.0, 1.0], 0.5)
+    assert abs(inc[0] / 4.7103e-13 - 1.0) < 2e-4, inc[0]
+    assert abs(inc[1] / 1.4901161193847656e-08 - 1.0) < 1e-7, inc[1]
+    #     the same with h0 = 0.05 (h enters linearly): inc_0 ten times smaller
+    inc_h = _fd_points(lambda y: [3.0, 4.0], [0.0, 1.0], 0.5, h0=0.05)
+    assert abs(inc_h[0] / 4.7103e-14 - 1.0) < 2e-4, inc_h[0]
+    # (c) ||f|| = 0: minInc = 1, inc_j = max(sqrt(u) |y_j|, scal_j): y = (2, 0) -> scal = (2.0001e-5, 1e-9), both above sqrt(u)|y|
+    inc = _fd_points(lambda y: [0.0, 0.0], [2.0, 0.0], 1.0)
+    assert abs(inc[0] / 2.0001e-05 - 1.0) < 1e-9 and abs(inc[1] / 1e-09 - 1.0) < 1e-9, inc
+
+
+def test_fd_jacobian_quotient_on_a_nonlinear_problem():
+    """the quotient (f(y + inc_j e_j) - f(y)) / inc_j itself, on a NONLINEAR problem where it differs from the analytic
+    Jacobian by O(inc): one fixed step with ONE Newton iteration, whose result depends on the matrix directly.  The run
+    with fd_jacobian = 1 must equal the run that is GIVEN the hand-built quotient matrix as its Jacobian; handing over a
+    quotient built with doubled increments moves the result by far more than the comparison bar (the test has teeth), and
+    so would a transposed quotient or a division by the wrong increment inside the oracle."""
+    f = lambda y: np.array([-y[0] * y[0] + y[1], -y[0] * y[1] * y[1]])
+    y0 = np.array([1.5, 0.75])
+    t_end = 0.3
+    inc = _fd_points(f, y0, t_end, fixed_steps=1, newton_max=1)
+
+    def quotient(incs):
+        J = np.empty((2, 2))
+        for j in range(2):
+            yp = y0.copy()
+            yp[j] += incs[j]
+            J[:, j] = (f(yp) - f(y0)) / incs[j]
+        return J
+    J_exact = np.array([[-2 * y0[0], 1.0], [-y0[1] ** 2, -2 * y0[0] * y0[1]]])
+    assert 1e-9 < np.abs(quotient(inc) - J_exact).max() < 1e-6                 # the quotient is NOT the analytic matrix
+    y_fd, st = orc.radau5(f, lambda y: J_exact, y0, t_end, 1e-6, 1e-10, fixed_steps=1, newton_max=1, fd_jacobian=1)
+    assert st["status"] == 0 and st["njac"] == 1 and st["nfcn"] in (1 + 2 + 3, 1 + 2 + 3 + 1)   # f(y0), 2 columns, 3 stages (+ ESTRAD's 2nd pass)
+    y_given, _ = orc.radau5(f, lambda y: quotient(inc), y0, t_end, 1e-6, 1e-10, fixed_steps=1, newton_max=1)
+    y_double, _ = orc.radau5(f, lambda y: quotient(2 * inc), y0, t_end, 1e-6, 1e-10, fixed_steps=1, newton_max=1)
+    y_exactJ, _ = orc.radau5(f, lambda y: J_exact, y0, t_end, 1e-6, 1e-10, fixed_steps=1, newton_max=1)
+    assert np.abs(y_fd - y_given).max() <= 4 * U
+    assert np.abs(y_fd - y_double).max() > 1e-11 and np.abs(y_fd - y_exactJ).max() > 1e-11
+
+
+def test_status_minus_2_step_size_too_small():
+    """a right-hand side that can be evaluated once, at the initial point, and is NaN ever after: every Newton iteration
+    fails (R11), every failure halves h (label 78), and the run must stop with -2 once
+    0.1 h <= u max(|x|, t_end) (R12) instead of looping: h0 = t_end = 1 is halved 49 times (2^-48 > 10 u >= 2^-49),
+    the 50th attempt is refused by the step-size test"""
+    calls = []
+
+    def f(y):
+        calls.append(1)
+        return [1.0] if len(calls) == 1 else [np.nan]
+    y, st = orc.radau5(f, lambda y: [[0.0]], [1.0], 1.0, 1e-6, 1e-10)
+    assert st["status"] == -2 and st["naccpt"] == 0 and y[0] == 1.0
+    assert st["nnewt_fail"] == 49 and st["nstep"] == 50
+    # with RADAU5's original test (u |x|, and x = 0 here) the loop would only end when h underflows to 0, after 1075 halvings
+
+
+def test_status_minus_3_matrix_not_factorisable_five_times():
+    """a Jacobian that is NaN: the matrix of every attempt is refused, h is halved, and the fifth refusal in a row ends the
+    state with -3 before any step was tried"""
+    y, st = orc.radau5(lambda y: [-y[0]], lambda y: [[np.nan]], [1.0], 1.0, 1e-6, 1e-10)
+    assert st["status"] == -3 and st["ndec"] == 5 and st["njac"] == 1 and st["nstep"] == 0 and y[0] == 1.0
+    # an exactly singular real matrix (J = gamma / h, so that gamma / h I - J = 0) is refused in the same way
+    g = orc.radau_constants()["gamma"]
+    calls = []
+
+    def jac(y):
+        calls.append(1)
+        return [[g / (1.0 * 0.5 ** (len(calls) - 1))]]
+    y, st = orc.radau5(lambda y: [0.0], jac, [1.0], 1.0, 1e-6, 1e-10)
+    assert st["status"] == 0 and st["ndec"] >= 2            # only the FIRST matrix is singular (the Jacobian is kept, h halves)
+
+
+def test_status_minus_5_fixed_step_with_a_singular_matrix():
+    """fixed-step mode (R14): the step size may not change, so a matrix that cannot be factorised ends the
+    state with -5 at once; y is left at the last completed step"""
+    g = orc.radau_constants()["gamma"]
+    y, st = orc.radau5(lambda y: [0.25], lambda y: [[g / 0.5]], [1.0], 1.0, 1e-6, 1e-10, fixed_steps=2)     # h = 0.5
+    assert st["status"] == -5 and st["naccpt"] == 0 and st["ndec"] == 1 and y[0] == 1.0
+    y, st = orc.radau5(lambda y: [0.25], lambda y: [[0.0]], [1.0], 1.0, 1e-6, 1e-10, fixed_steps=2)      # the true Jacobian
+    assert st["status"] == 0 and st["naccpt"] == 2 and abs(y[0] - 1.25) < 1e-12
+
+
+def test_last_step_is_stretched_onto_t_end():
+    """DESIGN.md R12: `x + hnew - t_end >= -100 u t_end` makes the last step end ON t_end.  On y' = 0 the controller takes
+    h0, 8 h0, 64 h0, ... (error estimate at its floor: growth factor 8); with t_end = 1 and h0 just under 1 / 73 the
+    third step would end a few ulp BEFORE t_end under RADAU5's original test (>= 0), a fourth step of those few ulp would
+    follow and be refused by the step-size test (status -2).  With R12: three steps, status 0."""
+    found = None
+    for k in range(1, 400):
+        h0 = (1.0 / 73.0) * (1.0 - k * U)
+        x2 = h0 + 8.0 * h0
+        gap = (x2 + 64.0 * h0) - 1.0
+        if -10 * U < gap < 0.0:                   # original test: not the last step; remaining step 0.1 * |gap| <= u: -2
+            found = (h0, gap)
+            break
+    assert found is not None
+    h0, gap = found
+    y, st = orc.radau5(lambda y: [0.0], lambda y: [[0.0]], [3.0], 1.0, 1e-6, 1e-10, h0=h0)
+    assert st["status"] == 0 and st["naccpt"] == 3 and st["nstep"] == 3 and y[0] == 3.0
+    assert abs(st["h_last"] - (1.0 - 9.0 * h0)) <= 2 * U
