@@ -101,8 +101,8 @@ typedef struct chem_opts {
                             of stiffness"; L184).  Results never depend on it, bit for bit.  1: by decreasing cost_hint (caller's
                             prediction); 2: by the library's own stiffness estimate, t_end ||f(y0) / (atol + rtol |y0|)||_rms, from
                             one extra source term per state (small mechanisms only, else CHEM_E_UNSUPPORTED); 0: auto = the
-                            estimate where it is measured to pay (the thread-per-state kernel on large batches), otherwise
-                            none; -1: off */
+                            estimate where it is measured to pay (small mechanisms: the thread-per-state kernel from ~150,000
+                            states on, the warp-per-state kernel from ~12,000), otherwise none; -1: off */
     const double *P_per_state;  /* device [n_states] or NULL: per-state pressure overriding P        */
     const int32_t *cost_hint;   /* device [n_states] or NULL: predicted cost per state, e.g. chem_stats.nstep of the
                                    previous global step; read only when reorder = 1.  Results do not depend on it. */

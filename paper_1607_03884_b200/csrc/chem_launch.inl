@@ -183,16 +183,16 @@ extern "C" int chem_lu_solve(int32_t n, int32_t batch, int32_t is_complex, const
 
 namespace {
 // Kernel ids (chem_opts.kernel, chem_last_kernel): 1 shared-memory group kernel, 2 warp-per-state, 3 thread-per-state.
-// Auto picks the fastest measured mapping (profiles/r2_mapping_config1.md, r2_mapping_config2.md): for an eligible small
-// mechanism the thread-per-state kernel when the batch fills its lanes at least eight times over (it processes a state
-// in ~36 us of SM time against ~56 us for the warp-per-state kernel, but the end of a launch, when the queue is empty
-// and every warp waits for its slowest lanes, costs it ~6 ms more: break-even at ~300,000 states at dt = 1e-6 s), else
-// the warp-per-state kernel; the group kernel for everything else.
+// Auto picks the fastest measured mapping (profiles/r2_mapping_config1.md, r2_mapping_config2.md, r3_tail_config1.md): for an
+// eligible small mechanism the thread-per-state kernel when the batch fills its lanes at least six times over -- with the
+// ordered start it takes 11.7 ms for 262,144 states at dt = 1e-6 s against 14.5 ms for the warp-per-state kernel, 10.0 against
+// 3.7 ms for 65,536: break-even near 200,000 states (it was 300,000 without the ordering) -- else the warp-per-state
+// kernel; the group kernel for everything else.
 int pick_kernel(const chem_mech *m, int n, const chem_opts *o)
 {
     const int want = o ? o->kernel : 0;
     if (want != 0) return want;
-    if (chem_tps_available(m) && (long long)n >= 8LL * chem_tps_slots(m)) return 3;
+    if (chem_tps_available(m) && (long long)n >= 6LL * chem_tps_slots(m)) return 3;
     if (warp_path_available(m)) return 2;
     return 1;
 }
@@ -221,15 +221,22 @@ int integrate_impl(const chem_mech *m, int32_t n, double P, double t_end, double
     int *order = nullptr;
     void *order_scratch = nullptr, *key_scratch = nullptr;
     // Start order (chem_opts.reorder): 1 = by the caller's cost_hint; 2 = by the library's own stiffness estimate
-    // (chem_tps_cost_keys: one source term per state + a radix sort, ~1.5 ms per million h2co-shaped states); 0 = auto: the
-    // estimate where it pays, i.e. for the thread-per-state kernel, whose launch otherwise ends with a few long states
-    // and idle lanes (profiles/r3_tail_config1.md: 40.2 -> 34 ms on config 1); < 0 = off.  Bits of the results never depend on it.
+    // (chem_tps_cost_keys: one source term per state + a radix sort, 1.8 ms per million h2co-shaped states); 0 = auto: the
+    // estimate where it is measured to pay (profiles/r3_tail_config1.md): the thread-per-state kernel from four times its
+    // lanes on (its launch otherwise ends with a few long states and idle lanes: 40.2 -> 34.9 ms on config 1) and the
+    // warp-per-state kernel from four waves of its warps on (16,384 states: 1.49 -> 1.22 ms; at 4,096 states the extra
+    // launches cost more than the order gives); < 0 = off.  Bits of the results never depend on it.
     const int reorder = o ? o->reorder : 0;
+    bool auto_order = false;
+    if (reorder == 0 && chem_tps_available(m)) {
+        if (kernel == 3) auto_order = (long long)n >= 4LL * chem_tps_slots(m);
+        else if (kernel == 2) auto_order = (long long)n >= 4LL * m->n_sm * (kWarpBlock / 32);
+    }
     if (reorder < -1 || reorder > 2) return fail(CHEM_E_ARG, "chem_opts.reorder must be -1..2");
     if (reorder == 1 && o->cost_hint) {
         const int rc = build_order(n, o->cost_hint, &order, &order_scratch, st);
         if (rc) { chem_host::scratch_free(order_scratch, st); return rc; }
-    } else if (reorder == 2 || (reorder == 0 && kernel == 3 && (long long)n >= 8LL * chem_tps_slots(m))) {
+    } else if (reorder == 2 || auto_order) {
         int rc = chem_host::scratch_alloc(&key_scratch, (size_t)n * sizeof(int32_t), st);
         if (rc == CHEM_OK) rc = chem_tps_cost_keys(m, n, P, prm, y_in, o, static_cast<int32_t *>(key_scratch), st);
         if (rc == CHEM_OK) rc = build_order(n, static_cast<const int32_t *>(key_scratch), &order, &order_scratch, st);
