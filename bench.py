@@ -34,10 +34,13 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the integration kernel from the committed
 # `ncu --set full` captures, keyed by (config index, kernel id); None where no capture of that pair is on file.
 NCU_TRAFFIC = {
+    (0, 2): (1.842944e6 + 0.225536e6, "profiles/r3_metrics_all_configs.md (ncu --metrics pass)"),
     (1, 2): (115.299840e6 + 109.461760e6, "profiles/r1_final_config1.md (ncu --set full)"),
     (1, 3): (44.098521e9 + 23.691889e9, "profiles/r3_tps_config1.md, r3_tps_metrics_config1.csv (ncu --metrics pass): lane-private LU factors stream through L2 / HBM"),
     (2, 2): (0.331e9, "profiles/r2_mapping_config2.md (ncu --metrics pass)"),
-    (2, 3): (354.05e9, "profiles/r2_mapping_config2.md (ncu --metrics pass)"),
+    (2, 3): (208.304123e9 + 113.344515e9, "profiles/r3_metrics_all_configs.md (ncu --metrics pass)"),
+    (3, 1): (253.852416e6 + 234.944512e6, "profiles/r3_metrics_all_configs.md (ncu --metrics pass)"),
+    (4, 1): (259.344640e6 + 239.524864e6, "profiles/r3_metrics_all_configs.md (ncu --metrics pass)"),
 }
 
 
